@@ -1,0 +1,197 @@
+/* nif.h -- C ABI of libnif.so: batched inference of the voxel-deformation-aware neural
+ * intersection query (arxiv 2604.24666) on one NVIDIA B200 (sm_100a).
+ *
+ * Citations: P:NN = PAPER.md line NN; B:NN = BASELINE.json line NN; R# = DESIGN.md section 3
+ * (readings adopted where the paper is silent).
+ *
+ * The query, per ray (Fig. 2; B:5):
+ *   (1) find the nearest deformed voxel with its entry/exit parameters t_in, t_out by
+ *       traversing a BVH built over the occupied voxels after the pose's deformation,
+ *   (2) map entry and exit points back to rest space with the inverse deformation,
+ *   (3) encode both with psi(x) = phi(gamma(x)) (Eq. 1),
+ *   (4) run the shared MLP, (5) decode the heads.
+ *
+ * General conventions
+ *   - Every pointer inside a descriptor struct is a DEVICE pointer owned by the caller unless
+ *     the field comment says HOST.  The library never frees caller memory.  Large buffers
+ *     (BVH, per-query scratch) live in caller-provided workspaces; the library itself only
+ *     allocates the small repacked weight images of a nif_net (< 2 MiB) and the staging
+ *     buffers of a nif_stage.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  nif_query only
+ *     enqueues work and returns; calls documented as "synchronises" wait for the stream.
+ *   - Return value: NIF_OK (0) or a negative nif_status.  On error no output is written.
+ *     No exceptions, no abort(), nothing printed.
+ *   - There is no CPU fallback: on a device that is not compute capability 10.x every entry
+ *     point that would launch a kernel returns NIF_ERR_UNSUPPORTED.
+ */
+#ifndef NIF_H_
+#define NIF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    NIF_OK = 0,
+    NIF_ERR_INVALID_ARG = -1,      /* null pointer, negative count, size out of range          */
+    NIF_ERR_UNSUPPORTED = -2,      /* shape/dtype the kernels do not cover, or not an sm_100 GPU */
+    NIF_ERR_DEFORM_SINGULAR = -3,  /* bend folds over: some occupied corner has k*y >= 1 - 1e-3 (R7) */
+    NIF_ERR_WORKSPACE = -4,        /* workspace too small or misaligned                        */
+    NIF_ERR_CUDA = -5              /* a CUDA runtime call failed                               */
+} nif_status;
+
+enum { NIF_F32 = 0, NIF_F16 = 1 };            /* nif_net_desc.dtype */
+
+/* nif_query flags */
+enum {
+    NIF_OCCLUSION_ONLY = 1u,   /* decode only the occlusion head (B:10); other head outputs untouched */
+    NIF_ENGINE_FFMA    = 2u,   /* force the scalar-FMA encode+MLP kernel even for NIF_F16 nets        */
+    NIF_TRAVERSE_ONLY  = 4u    /* step (1) only: voxel_id, t_in, t_out                                */
+};
+
+#define NIF_N_OUT 12   /* logits per ray: occlusion 1, distance 1, normal 3, albedo 3, material 4 (B:7) */
+
+typedef struct nif_bvh nif_bvh;       /* opaque host object; its device data lives in the caller's workspace */
+typedef struct nif_net nif_net;       /* opaque host object: table pointer + repacked weights               */
+typedef struct nif_stage nif_stage;   /* opaque: device staging buffers + streams for nif_query_host        */
+
+/* Rest-space voxelisation: nv^3 lattice over [-1,1]^3, voxel (ix,iy,iz) has
+ * id = ix + nv*(iy + nv*iz) and is occupied iff occupancy[id] != 0. */
+typedef struct {
+    int32_t nv;                   /* 2 <= nv <= 512 */
+    const uint8_t* occupancy;     /* DEVICE, nv^3 bytes */
+} nif_voxel_set;
+
+/* Parameterised deformation (formulas B:7-11, R7): twist about +y by
+ * twist_theta_max*(y+1)/2, then bend about z with curvature bend_k (|k| < 1e-6 = no bend).
+ * (0, 0) is the identity pose. */
+typedef struct {
+    float twist_theta_max;
+    float bend_k;
+} nif_deform_params;
+
+/* Encoding + MLP shape (B:7-11).  D_in = 2 * (1 + 2*pe_bands) * levels * feat. */
+typedef struct {
+    int32_t pe_bands;             /* B: sinusoidal bands (the paper's "F"), 0..8          */
+    int32_t levels;               /* L: hash-grid levels, 1..16                                 */
+    int32_t log2_T;               /* table entries per level = 2^log2_T, 4..24                  */
+    int32_t feat;                 /* F: features per entry: 1, 2 or 4 (NIF_F16: 2 or 4)         */
+    const int32_t* level_res;     /* HOST, `levels` entries: grid resolution N_l of each level  */
+    int32_t hidden_layers;        /* H: 1..8                                                    */
+    int32_t width;                /* W: 16..128, multiple of 16                                 */
+    int32_t dtype;                /* NIF_F32: table/weights float; NIF_F16: table/weights __half */
+} nif_net_desc;
+
+typedef struct {
+    int64_t n;                    /* rays in the batch, >= 0 */
+    const float* origin;          /* n*3 */
+    const float* dir;             /* n*3, unit length */
+} nif_ray_batch;
+
+/* Outputs, all DEVICE, struct-of-arrays.  voxel_id/t_in/t_out are always written.
+ * Miss ray: voxel_id = -1, t_in = t_out = +inf, every head output 0 (R18).
+ * Head pointers may be NULL only with NIF_TRAVERSE_ONLY; with NIF_OCCLUSION_ONLY only
+ * `occlusion` is required.  raw_logits is optional (NULL to skip). */
+typedef struct {
+    int32_t* voxel_id;            /* n   rest-space linear id of the nearest deformed voxel        */
+    float* t_in;                  /* n   entry parameter along the ray (deformed space, unit dir)  */
+    float* t_out;                 /* n   exit parameter                                            */
+    float* occlusion;             /* n   sigmoid(z0)                                               */
+    float* distance;              /* n   sigmoid(z1) * (t_out - t_in)                     */
+    float* dist_total;            /* n   D = t_in + distance            (k = 0)              */
+    float* normal;                /* 3n  z2..4 normalised                                          */
+    float* albedo;                /* 3n  sigmoid(z5..7)                                            */
+    float* material_logits;       /* 4n  z8..11                                                    */
+    float* raw_logits;            /* 12n optional                                                  */
+} nif_query_out;
+
+typedef struct {
+    int32_t nv;
+    int32_t n_occupied;           /* occupied voxels                                   */
+    int32_t n_nodes;              /* BVH nodes                                         */
+    int32_t depth;                /* levels of the hierarchy (root = depth-1)          */
+    float lo[3], hi[3];           /* bounding box of the posed object (root box)       */
+    float theta_max, bend_k;
+} nif_bvh_info;
+
+/* -------- step (a0): per-pose build ("For each deformation pose, we build a simple BVH
+ * over the deformed voxels") ------------------------------------------------------------- */
+
+/* Bytes of workspace nif_build_deformed_bvh needs for an nv^3 grid with at most
+ * `max_occupied` occupied voxels (pass nv^3 if unknown).  Host-only, no CUDA call. */
+int nif_bvh_workspace_bytes(int32_t nv, int64_t max_occupied, size_t* bytes);
+
+/* Deforms the (nv+1)^3 corner lattice (fp64 evaluation, one rounding to fp32), computes the
+ * exact AABB of every occupied deformed voxel and builds the 8-wide hierarchy over them.
+ * `workspace`: DEVICE, 256-byte aligned, at least nif_bvh_workspace_bytes; it holds the BVH
+ * for the lifetime of *out and must not be touched by the caller.  SYNCHRONISES `stream`
+ * (it reads back counts and the fold-over check).  Errors: NIF_ERR_DEFORM_SINGULAR,
+ * NIF_ERR_WORKSPACE (also when the grid holds more than the max_occupied the workspace was
+ * sized for), NIF_ERR_INVALID_ARG, NIF_ERR_CUDA. */
+int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_deform_params* pose,
+                           void* workspace, size_t workspace_bytes, void* stream, nif_bvh** out);
+
+int nif_bvh_get_info(const nif_bvh* bvh, nif_bvh_info* info);      /* host-only */
+
+/* DEVICE pointer to the deformed corner lattice: (nv+1)^3 float4 (x,y,z,0), lattice point
+ * (i,j,k) at index i + (nv+1)*(j + (nv+1)*k).  Valid while the BVH lives.  For parity tests. */
+int nif_bvh_get_lattice(const nif_bvh* bvh, const float** lattice_xyzw);
+
+void nif_bvh_destroy(nif_bvh* bvh);                                /* frees the host object only */
+
+/* -------- network ------------------------------------------------------------------------ */
+
+/* `table`: DEVICE, layout table[l][index][f], every level 2^log2_T entries, float (NIF_F32) or
+ * __half (NIF_F16); borrowed for the lifetime of the net (not copied).
+ * `weights`: HOST array of hidden_layers+1 DEVICE pointers; weights[i] is row-major
+ * (fan_out, fan_in): (W, D_in), (W, W)..., (12, W); same element type as the table.  Copied and
+ * repacked on `stream` (tensor-core operand images, zero-padded output layer).  SYNCHRONISES. */
+int nif_net_create(const nif_net_desc* desc, const void* table, const void* const* weights,
+                   void* stream, nif_net** out);
+void nif_net_destroy(nif_net* net);
+
+/* -------- steps (a1)-(a5): the query ------------------------------------------------------ */
+
+/* Scratch bytes nif_query needs for a batch of n rays.  Host-only. */
+int nif_query_workspace_bytes(int64_t n, size_t* bytes);
+
+/* Enqueues the whole hot path on `stream` and returns without synchronising.
+ * `workspace`: DEVICE, 256-byte aligned, >= nif_query_workspace_bytes(rays->n); contents are
+ * scratch (hit-ray compaction list and counters) and may be reused by the next call on the
+ * same stream.  Several poses (B:9) = one nif_bvh and one nif_query per pose sharing one net. */
+int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+              const nif_query_out* out, void* workspace, size_t workspace_bytes,
+              unsigned flags, void* stream);
+
+/* -------- end-to-end with HOST buffers ---------------------------------------------------- */
+
+/* Staging for nif_query_host: device buffers for `chunk_rays` rays x 2 (double buffer), three
+ * streams.  chunk_rays >= 1. */
+int nif_stage_create(int64_t chunk_rays, nif_stage** out);
+void nif_stage_destroy(nif_stage* stage);
+
+/* Same query with HOST pointers in `rays` and `out` (pinned memory recommended; pageable
+ * works but copies synchronously).  Splits the batch into chunks, overlapping the host->device
+ * copy of chunk i+1, the kernels of chunk i and the device->host copy of chunk i-1.
+ * SYNCHRONISES: on return every output is in host memory. */
+int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
+                   const nif_ray_batch* rays_host, const nif_query_out* out_host, unsigned flags);
+
+/* -------- diagnostics --------------------------------------------------------------------- */
+
+/* Counters of the last nif_query on this thread's workspace: hit rays found by the traversal.
+ * Reads 8 bytes back from the workspace; SYNCHRONISES `stream`. */
+int nif_query_last_hit_count(const void* workspace, void* stream, int64_t* n_hit);
+
+/* Kernels launched by the library since load (every nif_* call adds its launches). */
+int64_t nif_kernel_launch_count(void);
+
+const char* nif_error_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NIF_H_ */

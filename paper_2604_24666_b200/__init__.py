@@ -1,0 +1,9 @@
+"""B200-native batched inference of the voxel-deformation-aware neural intersection query
+(arxiv 2604.24666).  The product is libnif.so (CUDA, sm_100a; C ABI in include/nif.h); this
+package is the thin binding over it.  See DESIGN.md."""
+from .binding import (  # noqa: F401
+    NIF_F16, NIF_F32, NIF_N_OUT, NIF_OCCLUSION_ONLY, NIF_ENGINE_FFMA, NIF_TRAVERSE_ONLY,
+    Bvh, Net, NifError, Stage, alloc_outputs, lib,
+    nif_build_deformed_bvh, nif_bvh_workspace_bytes, nif_kernel_launch_count, nif_net_create,
+    nif_query, nif_query_host, nif_query_last_hit_count, nif_query_workspace_bytes,
+)

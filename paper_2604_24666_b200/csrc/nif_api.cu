@@ -1,0 +1,264 @@
+// nif_api.cu -- C ABI glue of libnif.so (include/nif.h): argument validation, network object,
+// nif_query (enqueue only), the host-buffer end-to-end entry and diagnostics.
+#include "nif_common.cuh"
+
+#include <atomic>
+#include <new>
+#include <string.h>
+
+extern "C" int nif_device_supported(void);
+
+namespace {
+std::atomic<long long> g_launches{0};
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline size_t elem_bytes(int dtype) { return dtype == NIF_F16 ? 2 : 4; }
+}  // namespace
+
+extern "C" void nif_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+extern "C" int64_t nif_kernel_launch_count(void) { return (int64_t)g_launches.load(); }
+
+extern "C" const char* nif_error_string(int status)
+{
+    switch (status) {
+        case NIF_OK: return "ok";
+        case NIF_ERR_INVALID_ARG: return "invalid argument";
+        case NIF_ERR_UNSUPPORTED: return "unsupported shape, dtype or device (needs sm_100)";
+        case NIF_ERR_DEFORM_SINGULAR: return "deformation folds over (bend k*y >= 1)";
+        case NIF_ERR_WORKSPACE: return "workspace too small or misaligned";
+        case NIF_ERR_CUDA: return "CUDA runtime error";
+        default: return "unknown status";
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// network
+// ---------------------------------------------------------------------------------------------
+static int validate_desc(const nif_net_desc* d)
+{
+    if (!d || !d->level_res) return NIF_ERR_INVALID_ARG;
+    if (d->pe_bands < 0 || d->pe_bands > NIF_MAX_BANDS) return NIF_ERR_INVALID_ARG;
+    if (d->levels < 1 || d->levels > NIF_MAX_LEVELS) return NIF_ERR_INVALID_ARG;
+    if (d->log2_T < 4 || d->log2_T > 24) return NIF_ERR_INVALID_ARG;
+    if (d->hidden_layers < 1 || d->hidden_layers > NIF_MAX_LAYERS - 1) return NIF_ERR_INVALID_ARG;
+    if (d->dtype != NIF_F32 && d->dtype != NIF_F16) return NIF_ERR_INVALID_ARG;
+    for (int l = 0; l < d->levels; ++l)
+        if (d->level_res[l] < 1 || d->level_res[l] > (1 << 20)) return NIF_ERR_INVALID_ARG;
+    if (d->feat != 1 && d->feat != 2 && d->feat != 4) return NIF_ERR_UNSUPPORTED;
+    if (d->width < 16 || d->width > 128 || (d->width % 16) != 0) return NIF_ERR_UNSUPPORTED;
+    return NIF_OK;
+}
+
+extern "C" int nif_net_create(const nif_net_desc* desc, const void* table, const void* const* weights,
+                              void* stream_, nif_net** out)
+{
+    int rc = validate_desc(desc);
+    if (rc != NIF_OK) return rc;
+    if (!table || !weights || !out) return NIF_ERR_INVALID_ARG;
+    for (int i = 0; i <= desc->hidden_layers; ++i)
+        if (!weights[i]) return NIF_ERR_INVALID_ARG;
+    if (!nif_device_supported()) return NIF_ERR_UNSUPPORTED;
+    cudaStream_t stream = (cudaStream_t)stream_;
+
+    nif_net* net = new (std::nothrow) nif_net();
+    if (!net) return NIF_ERR_CUDA;
+    memset(net, 0, sizeof(*net));
+    net->desc = *desc;
+    net->desc.level_res = nullptr;                 // host pointer is not kept
+    net->enc.bands = desc->pe_bands; net->enc.levels = desc->levels;
+    net->enc.log2_T = desc->log2_T; net->enc.feat = desc->feat;
+    net->enc.dense_mask = 0;
+    const unsigned long long T = 1ull << desc->log2_T;
+    for (int l = 0; l < desc->levels; ++l) {
+        net->enc.res[l] = desc->level_res[l];
+        const unsigned long long np1 = (unsigned long long)desc->level_res[l] + 1ull;   // 64-bit compare (R6)
+        if (np1 * np1 * np1 <= T) net->enc.dense_mask |= 1u << l;
+    }
+    net->d_in = 2 * (1 + 2 * desc->pe_bands) * desc->levels * desc->feat;
+    net->table = table;
+    const size_t eb = elem_bytes(desc->dtype);
+    for (int i = 0; i <= desc->hidden_layers; ++i) {
+        const size_t fan_out = i == desc->hidden_layers ? NIF_N_OUT : (size_t)desc->width;
+        const size_t fan_in = i == 0 ? (size_t)net->d_in : (size_t)desc->width;
+        const size_t bytes = fan_out * fan_in * eb;
+        cudaError_t e = cudaMalloc(&net->w_plain[i], bytes);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(net->w_plain[i], weights[i], bytes, cudaMemcpyDeviceToDevice, stream);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); nif_net_destroy(net); return NIF_ERR_CUDA; }
+    }
+    net->tc_supported = nif_tc_supported(desc);
+    if (net->tc_supported) {
+        rc = nif_tc_pack_weights(net, stream);
+        if (rc != NIF_OK) { nif_net_destroy(net); return rc; }
+    }
+    if (cudaStreamSynchronize(stream) != cudaSuccess) { (void)cudaGetLastError(); nif_net_destroy(net); return NIF_ERR_CUDA; }
+    *out = net;
+    return NIF_OK;
+}
+
+extern "C" void nif_net_destroy(nif_net* net)
+{
+    if (!net) return;
+    for (int i = 0; i < NIF_MAX_LAYERS; ++i)
+        if (net->w_plain[i]) cudaFree(net->w_plain[i]);
+    if (net->w_tc) cudaFree(net->w_tc);
+    delete net;
+}
+
+// ---------------------------------------------------------------------------------------------
+// query
+// ---------------------------------------------------------------------------------------------
+extern "C" int nif_query_workspace_bytes(int64_t n, size_t* bytes)
+{
+    if (!bytes || n < 0 || n > 0x7fffffffLL) return NIF_ERR_INVALID_ARG;
+    *bytes = align_up(sizeof(NifQueryScratch) + (size_t)n * sizeof(int32_t), 256) + 256;
+    return NIF_OK;
+}
+
+static int validate_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                          const nif_query_out* out, unsigned flags)
+{
+    if (!bvh || !rays || !out) return NIF_ERR_INVALID_ARG;
+    if (rays->n < 0 || rays->n > 0x7fffffffLL) return NIF_ERR_INVALID_ARG;
+    if (rays->n == 0) return NIF_OK;
+    if (!rays->origin || !rays->dir) return NIF_ERR_INVALID_ARG;
+    if (!out->voxel_id || !out->t_in || !out->t_out) return NIF_ERR_INVALID_ARG;
+    if (flags & NIF_TRAVERSE_ONLY) return NIF_OK;
+    if (!net || !out->occlusion) return NIF_ERR_INVALID_ARG;
+    if (!(flags & NIF_OCCLUSION_ONLY) &&
+        (!out->distance || !out->dist_total || !out->normal || !out->albedo || !out->material_logits))
+        return NIF_ERR_INVALID_ARG;
+    return NIF_OK;
+}
+
+extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                         const nif_query_out* out, void* workspace, size_t workspace_bytes,
+                         unsigned flags, void* stream_)
+{
+    int rc = validate_query(bvh, net, rays, out, flags);
+    if (rc != NIF_OK) return rc;
+    if (rays->n == 0) return NIF_OK;
+    size_t need = 0;
+    nif_query_workspace_bytes(rays->n, &need);
+    if (!workspace || ((uintptr_t)workspace & 255u) != 0 || workspace_bytes < need - 256) return NIF_ERR_WORKSPACE;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    NifQueryScratch* scratch = (NifQueryScratch*)workspace;
+    int32_t* hit_list = (int32_t*)((char*)workspace + sizeof(NifQueryScratch));
+    NIF_CUDA_TRY(cudaMemsetAsync(scratch, 0, sizeof(NifQueryScratch), stream));
+    rc = nif_launch_traverse(bvh, rays, out, scratch, hit_list, flags, stream);
+    if (rc != NIF_OK || (flags & NIF_TRAVERSE_ONLY)) return rc;
+    const bool use_tc = net->desc.dtype == NIF_F16 && net->tc_supported && !(flags & NIF_ENGINE_FFMA);
+    if (use_tc) return nif_launch_fused_tc(bvh, net, rays, out, scratch, hit_list, flags, stream);
+    return nif_launch_ffma(bvh, net, rays, out, scratch, hit_list, flags, stream);
+}
+
+extern "C" int nif_query_last_hit_count(const void* workspace, void* stream_, int64_t* n_hit)
+{
+    if (!workspace || !n_hit) return NIF_ERR_INVALID_ARG;
+    unsigned long long v = 0;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    NIF_CUDA_TRY(cudaMemcpyAsync(&v, workspace, sizeof(v), cudaMemcpyDeviceToHost, stream));
+    NIF_CUDA_TRY(cudaStreamSynchronize(stream));
+    *n_hit = (int64_t)v;
+    return NIF_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// end-to-end with HOST buffers: chunked, NSLOT slots each on its own stream, so the H2D copy of
+// chunk i+1, the kernels of chunk i and the D2H copy of chunk i-1 overlap (two copy engines).
+// ---------------------------------------------------------------------------------------------
+namespace { constexpr int NSLOT = 3; }
+
+struct nif_stage {
+    int64_t chunk;
+    cudaStream_t stream[NSLOT];
+    char* dev[NSLOT];            // one allocation per slot
+    size_t slot_bytes, ws_bytes;
+    // offsets inside a slot
+    size_t o_origin, o_dir, o_vid, o_tin, o_tout, o_occ, o_dist, o_dtot, o_nrm, o_alb, o_mat, o_raw, o_ws;
+};
+
+extern "C" int nif_stage_create(int64_t chunk_rays, nif_stage** out)
+{
+    if (!out || chunk_rays < 1 || chunk_rays > 0x7fffffffLL) return NIF_ERR_INVALID_ARG;
+    if (!nif_device_supported()) return NIF_ERR_UNSUPPORTED;
+    nif_stage* s = new (std::nothrow) nif_stage();
+    if (!s) return NIF_ERR_CUDA;
+    memset(s, 0, sizeof(*s));
+    s->chunk = chunk_rays;
+    const size_t n = (size_t)chunk_rays;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    s->o_origin = take(n * 12); s->o_dir = take(n * 12);
+    s->o_vid = take(n * 4); s->o_tin = take(n * 4); s->o_tout = take(n * 4);
+    s->o_occ = take(n * 4); s->o_dist = take(n * 4); s->o_dtot = take(n * 4);
+    s->o_nrm = take(n * 12); s->o_alb = take(n * 12); s->o_mat = take(n * 16); s->o_raw = take(n * 48);
+    nif_query_workspace_bytes(chunk_rays, &s->ws_bytes);
+    s->o_ws = take(s->ws_bytes);
+    s->slot_bytes = off;
+    for (int i = 0; i < NSLOT; ++i) {
+        if (cudaStreamCreateWithFlags(&s->stream[i], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaMalloc((void**)&s->dev[i], s->slot_bytes) != cudaSuccess) {
+            (void)cudaGetLastError();
+            nif_stage_destroy(s);
+            return NIF_ERR_CUDA;
+        }
+    }
+    *out = s;
+    return NIF_OK;
+}
+
+extern "C" void nif_stage_destroy(nif_stage* s)
+{
+    if (!s) return;
+    for (int i = 0; i < NSLOT; ++i) {
+        if (s->dev[i]) cudaFree(s->dev[i]);
+        if (s->stream[i]) cudaStreamDestroy(s->stream[i]);
+    }
+    delete s;
+}
+
+extern "C" int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* st,
+                              const nif_ray_batch* rays, const nif_query_out* out, unsigned flags)
+{
+    if (!st) return NIF_ERR_INVALID_ARG;
+    int rc = validate_query(bvh, net, rays, out, flags);
+    if (rc != NIF_OK) return rc;
+    const bool heads = !(flags & NIF_TRAVERSE_ONLY);
+    const bool full = heads && !(flags & NIF_OCCLUSION_ONLY);
+    int chunk_idx = 0;
+    for (int64_t begin = 0; begin < rays->n; begin += st->chunk, ++chunk_idx) {
+        const int64_t m = (rays->n - begin < st->chunk) ? rays->n - begin : st->chunk;
+        const int slot = chunk_idx % NSLOT;
+        cudaStream_t stream = st->stream[slot];
+        char* d = st->dev[slot];
+        NIF_CUDA_TRY(cudaMemcpyAsync(d + st->o_origin, rays->origin + 3 * begin, (size_t)m * 12, cudaMemcpyHostToDevice, stream));
+        NIF_CUDA_TRY(cudaMemcpyAsync(d + st->o_dir, rays->dir + 3 * begin, (size_t)m * 12, cudaMemcpyHostToDevice, stream));
+        nif_ray_batch rb; rb.n = m; rb.origin = (const float*)(d + st->o_origin); rb.dir = (const float*)(d + st->o_dir);
+        nif_query_out qo;
+        qo.voxel_id = (int32_t*)(d + st->o_vid); qo.t_in = (float*)(d + st->o_tin); qo.t_out = (float*)(d + st->o_tout);
+        qo.occlusion = (float*)(d + st->o_occ); qo.distance = (float*)(d + st->o_dist);
+        qo.dist_total = (float*)(d + st->o_dtot); qo.normal = (float*)(d + st->o_nrm);
+        qo.albedo = (float*)(d + st->o_alb); qo.material_logits = (float*)(d + st->o_mat);
+        qo.raw_logits = (heads && out->raw_logits) ? (float*)(d + st->o_raw) : nullptr;
+        rc = nif_query(bvh, net, &rb, &qo, d + st->o_ws, st->ws_bytes, flags, stream);
+        if (rc != NIF_OK) return rc;
+        auto back = [&](void* host, size_t host_off, size_t dev_off, size_t bytes) -> cudaError_t {
+            return cudaMemcpyAsync((char*)host + host_off, d + dev_off, bytes, cudaMemcpyDeviceToHost, stream);
+        };
+        const size_t b = (size_t)begin, mm = (size_t)m;
+        NIF_CUDA_TRY(back(out->voxel_id, b * 4, st->o_vid, mm * 4));
+        NIF_CUDA_TRY(back(out->t_in, b * 4, st->o_tin, mm * 4));
+        NIF_CUDA_TRY(back(out->t_out, b * 4, st->o_tout, mm * 4));
+        if (heads) NIF_CUDA_TRY(back(out->occlusion, b * 4, st->o_occ, mm * 4));
+        if (full) {
+            NIF_CUDA_TRY(back(out->distance, b * 4, st->o_dist, mm * 4));
+            NIF_CUDA_TRY(back(out->dist_total, b * 4, st->o_dtot, mm * 4));
+            NIF_CUDA_TRY(back(out->normal, b * 12, st->o_nrm, mm * 12));
+            NIF_CUDA_TRY(back(out->albedo, b * 12, st->o_alb, mm * 12));
+            NIF_CUDA_TRY(back(out->material_logits, b * 16, st->o_mat, mm * 16));
+        }
+        if (heads && out->raw_logits) NIF_CUDA_TRY(back(out->raw_logits, b * 48, st->o_raw, mm * 48));
+    }
+    for (int i = 0; i < NSLOT; ++i) NIF_CUDA_TRY(cudaStreamSynchronize(st->stream[i]));
+    return NIF_OK;
+}

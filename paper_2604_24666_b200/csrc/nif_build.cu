@@ -1,0 +1,450 @@
+// nif_build.cu -- step (a0): per-pose build.  PAPER.md:41 "We voxelize the geometry in the rest
+// space and apply parameterized deformation to obtain deformed voxels. For each deformation
+// pose, we build a simple BVH over the deformed voxels".
+//
+// B200 design: the deformation keeps the rest lattice's topology, so
+// the hierarchy is the sparse octree of the REST lattice (8-wide nodes, Morton order, children
+// of a node contiguous one level down) and only the boxes depend on the pose.  Every step is a
+// flat data-parallel kernel: deform (nv+1)^3 corners, per-brick occupancy masks, one exclusive
+// scan per level, one node-write pass per level, bottom-up.
+#include "nif_common.cuh"
+
+#include <new>
+
+namespace {
+
+__host__ __device__ inline uint32_t spread3(uint32_t x)      // 10 bits -> every third bit
+{
+    x &= 0x3ffu;
+    x = (x | (x << 16)) & 0x030000ffu;
+    x = (x | (x << 8)) & 0x0300f00fu;
+    x = (x | (x << 4)) & 0x030c30c3u;
+    x = (x | (x << 2)) & 0x09249249u;
+    return x;
+}
+__host__ __device__ inline uint32_t compact3(uint32_t x)
+{
+    x &= 0x09249249u;
+    x = (x | (x >> 2)) & 0x030c30c3u;
+    x = (x | (x >> 4)) & 0x0300f00fu;
+    x = (x | (x >> 8)) & 0x030000ffu;
+    x = (x | (x >> 16)) & 0x3ffu;
+    return x;
+}
+
+// ---- O1/O2: rest lattice -> deformed lattice, fp64, one rounding to fp32 (R7) -------
+// Explicit _rn intrinsics: no fma contraction, so the operation sequence is the one DESIGN.md
+// states (twist about +y by theta_max (y+1)/2, then circular-arc bend about z).
+__global__ void k_deform_lattice(int nv, double theta_max, double k, float4* __restrict__ lat)
+{
+    const size_t np1 = (size_t)nv + 1;
+    const size_t total = np1 * np1 * np1;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (size_t)gridDim.x * blockDim.x) {
+        int i = (int)(idx % np1), j = (int)((idx / np1) % np1), kk = (int)(idx / (np1 * np1));
+        double x = __ddiv_rn(__dsub_rn(__dmul_rn(2.0, (double)i), (double)nv), (double)nv);
+        double y = __ddiv_rn(__dsub_rn(__dmul_rn(2.0, (double)j), (double)nv), (double)nv);
+        double z = __ddiv_rn(__dsub_rn(__dmul_rn(2.0, (double)kk), (double)nv), (double)nv);
+        double a = __ddiv_rn(__dmul_rn(theta_max, __dadd_rn(y, 1.0)), 2.0);
+        double sa, ca;
+        sincos(a, &sa, &ca);
+        double tx = __dadd_rn(__dmul_rn(x, ca), __dmul_rn(z, sa));
+        double ty = y;
+        double tz = __dadd_rn(__dmul_rn(-x, sa), __dmul_rn(z, ca));
+        double X = tx, Y = ty, Z = tz;
+        if (fabs(k) >= 1e-6) {
+            double al = __dmul_rn(k, tx);
+            double sal, cal;
+            sincos(al, &sal, &cal);
+            double sh = sin(__ddiv_rn(al, 2.0));
+            X = __ddiv_rn(__dmul_rn(__dsub_rn(1.0, __dmul_rn(k, ty)), sal), k);
+            Y = __dadd_rn(__dmul_rn(ty, cal), __ddiv_rn(__dmul_rn(__dmul_rn(2.0, sh), sh), k));
+        }
+        lat[idx] = make_float4((float)X, (float)Y, (float)Z, 0.0f);
+    }
+}
+
+// ---- occupancy masks ------------------------------------------------------------------------
+// level 1: one Morton-indexed brick of 2x2x2 voxels; bit c = octant (c&1, (c>>1)&1, c>>2).
+// counters[0] += occupied voxels; counters[1] = max (iy+1) over occupied voxels.
+__global__ void k_brick_mask(int nv, const uint8_t* __restrict__ occ, uint32_t n_bricks,
+                             uint8_t* __restrict__ mask, uint32_t* __restrict__ counters)
+{
+    uint32_t m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n_bricks) return;
+    uint32_t bx = compact3(m), by = compact3(m >> 1), bz = compact3(m >> 2);
+    uint32_t bits = 0; int top = 0;
+    for (int c = 0; c < 8; ++c) {
+        int ix = 2 * bx + (c & 1), iy = 2 * by + ((c >> 1) & 1), iz = 2 * bz + (c >> 2);
+        if (ix < nv && iy < nv && iz < nv && occ[(size_t)ix + (size_t)nv * ((size_t)iy + (size_t)nv * iz)]) {
+            bits |= 1u << c;
+            top = max(top, iy + 1);
+        }
+    }
+    mask[m] = (uint8_t)bits;
+    if (bits) {
+        atomicAdd(&counters[0], (uint32_t)__popc(bits));
+        atomicMax(&counters[1], (uint32_t)top);
+    }
+}
+
+__global__ void k_upper_mask(const uint8_t* __restrict__ lower, uint32_t n_cells,
+                             uint8_t* __restrict__ mask)
+{
+    uint32_t m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n_cells) return;
+    const uint2 v = *reinterpret_cast<const uint2*>(lower + 8 * (size_t)m);   // 8 child masks
+    uint32_t bits = 0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        if ((v.x >> (8 * c)) & 0xffu) bits |= 1u << c;
+        if ((v.y >> (8 * c)) & 0xffu) bits |= 1u << (4 + c);
+    }
+    mask[m] = (uint8_t)bits;
+}
+
+// ---- exclusive scan of (mask != 0): three passes, 2048 elements per block -------------------
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_PER_THREAD = 8;
+constexpr int SCAN_BLOCK = SCAN_THREADS * SCAN_PER_THREAD;
+
+__device__ inline uint32_t block_exclusive_scan(uint32_t v, uint32_t* total)
+{
+    __shared__ uint32_t warp_sums[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) warp_sums[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        uint32_t s = lane < SCAN_THREADS / 32 ? warp_sums[lane] : 0;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, s, d);
+            if (lane >= d) s += t;
+        }
+        if (lane < SCAN_THREADS / 32) warp_sums[lane] = s;        // inclusive over warps
+    }
+    __syncthreads();
+    uint32_t warp_off = wid ? warp_sums[wid - 1] : 0;
+    *total = warp_sums[SCAN_THREADS / 32 - 1];
+    __syncthreads();
+    return warp_off + inc - v;
+}
+
+__global__ void k_scan_count(const uint8_t* __restrict__ mask, uint32_t n, uint32_t* __restrict__ sums)
+{
+    uint32_t base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_PER_THREAD;
+    uint32_t c = 0;
+    for (int i = 0; i < SCAN_PER_THREAD; ++i)
+        if (base + i < n && mask[base + i]) ++c;
+    uint32_t total;
+    block_exclusive_scan(c, &total);
+    if (threadIdx.x == 0) sums[blockIdx.x] = total;
+}
+
+__global__ void k_scan_sums(uint32_t* __restrict__ sums, uint32_t nb, uint32_t* __restrict__ total_out)
+{
+    __shared__ uint32_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (uint32_t start = 0; start < nb; start += SCAN_THREADS) {
+        uint32_t i = start + threadIdx.x;
+        uint32_t v = i < nb ? sums[i] : 0;
+        uint32_t total;
+        uint32_t ex = block_exclusive_scan(v, &total);
+        uint32_t c = carry;
+        if (i < nb) sums[i] = c + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) carry = c + total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *total_out = carry;
+}
+
+__global__ void k_scan_write(const uint8_t* __restrict__ mask, uint32_t n,
+                             const uint32_t* __restrict__ sums, uint32_t* __restrict__ offs)
+{
+    uint32_t base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_PER_THREAD;
+    uint32_t f[SCAN_PER_THREAD]; uint32_t c = 0;
+    for (int i = 0; i < SCAN_PER_THREAD; ++i) {
+        f[i] = (base + i < n && mask[base + i]) ? 1u : 0u;
+        c += f[i];
+    }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan(c, &total) + sums[blockIdx.x];
+    for (int i = 0; i < SCAN_PER_THREAD; ++i) {
+        if (base + i < n) offs[base + i] = ex;
+        ex += f[i];
+    }
+}
+
+// ---- node writes, bottom-up -----------------------------------------------------------------
+__device__ inline void store_node(NifNode* dst, const NifNode& nd)
+{
+    const float4* s = reinterpret_cast<const float4*>(&nd);
+    float4* d = reinterpret_cast<float4*>(dst);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) d[i] = s[i];
+}
+
+__global__ void k_write_bricks(int nv, uint32_t n_bricks, const uint8_t* __restrict__ mask,
+                               const uint32_t* __restrict__ offs, uint32_t node_base,
+                               const float4* __restrict__ lat, NifNode* __restrict__ nodes,
+                               float4* __restrict__ boxes)
+{
+    uint32_t m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n_bricks) return;
+    uint32_t bits = mask[m];
+    if (!bits) return;
+    uint32_t bx = compact3(m), by = compact3(m >> 1), bz = compact3(m >> 2);
+    const size_t np1 = (size_t)nv + 1;
+    NifNode nd;
+    float blo[3] = {INFINITY, INFINITY, INFINITY}, bhi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int c = 0; c < 8; ++c) {
+        float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+        uint32_t id = 0xffffffffu;
+        if (bits & (1u << c)) {
+            int ix = 2 * bx + (c & 1), iy = 2 * by + ((c >> 1) & 1), iz = 2 * bz + (c >> 2);
+            id = (uint32_t)ix + (uint32_t)nv * ((uint32_t)iy + (uint32_t)nv * (uint32_t)iz);
+            for (int q = 0; q < 8; ++q) {     // exact AABB of the 8 deformed corners (min/max: no rounding)
+                float4 p = lat[(size_t)(ix + (q & 1)) + np1 * ((size_t)(iy + ((q >> 1) & 1)) + np1 * (size_t)(iz + (q >> 2)))];
+                lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+                lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+                lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+            }
+            for (int a = 0; a < 3; ++a) { blo[a] = fminf(blo[a], lo[a]); bhi[a] = fmaxf(bhi[a], hi[a]); }
+        }
+        for (int a = 0; a < 3; ++a) { nd.lo[a][c] = lo[a]; nd.hi[a][c] = hi[a]; }
+        nd.child[c] = id;
+    }
+    nd.mask = bits; nd.is_brick = 1;
+    for (int i = 0; i < 6; ++i) nd.pad[i] = 0;
+    uint32_t idx = node_base + offs[m];
+    store_node(nodes + idx, nd);
+    boxes[2 * (size_t)idx] = make_float4(blo[0], blo[1], blo[2], 0.f);
+    boxes[2 * (size_t)idx + 1] = make_float4(bhi[0], bhi[1], bhi[2], 0.f);
+}
+
+__global__ void k_write_level(uint32_t n_cells, const uint8_t* __restrict__ mask,
+                              const uint32_t* __restrict__ offs, uint32_t node_base,
+                              const uint8_t* __restrict__ child_mask,
+                              const uint32_t* __restrict__ child_offs, uint32_t child_base,
+                              NifNode* __restrict__ nodes, float4* __restrict__ boxes)
+{
+    uint32_t m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n_cells) return;
+    uint32_t bits = mask[m];
+    if (!bits) return;
+    NifNode nd;
+    float blo[3] = {INFINITY, INFINITY, INFINITY}, bhi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int c = 0; c < 8; ++c) {
+        float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+        uint32_t id = 0xffffffffu;
+        if (bits & (1u << c)) {
+            id = child_base + child_offs[8 * (size_t)m + c];
+            float4 l = boxes[2 * (size_t)id], h = boxes[2 * (size_t)id + 1];
+            lo[0] = l.x; lo[1] = l.y; lo[2] = l.z; hi[0] = h.x; hi[1] = h.y; hi[2] = h.z;
+            for (int a = 0; a < 3; ++a) { blo[a] = fminf(blo[a], lo[a]); bhi[a] = fmaxf(bhi[a], hi[a]); }
+        }
+        for (int a = 0; a < 3; ++a) { nd.lo[a][c] = lo[a]; nd.hi[a][c] = hi[a]; }
+        nd.child[c] = id;
+    }
+    (void)child_mask;
+    nd.mask = bits; nd.is_brick = 0;
+    for (int i = 0; i < 6; ++i) nd.pad[i] = 0;
+    uint32_t idx = node_base + offs[m];
+    store_node(nodes + idx, nd);
+    boxes[2 * (size_t)idx] = make_float4(blo[0], blo[1], blo[2], 0.f);
+    boxes[2 * (size_t)idx + 1] = make_float4(bhi[0], bhi[1], bhi[2], 0.f);
+}
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct BuildLayout {
+    int P, levels;                       // padded pow2 resolution, hierarchy levels (1..levels)
+    size_t cells[12];                    // cells[l], l = 1..levels
+    size_t off_lattice, off_counters, off_sums, off_mask[12], off_offs[12], off_nodes;
+    size_t fixed_bytes;
+};
+
+BuildLayout make_layout(int nv)
+{
+    BuildLayout L{};
+    int P = 2;
+    while (P < nv) P <<= 1;
+    L.P = P;
+    int levels = 0;
+    for (int p = P; p > 1; p >>= 1) ++levels;
+    L.levels = levels;
+    size_t off = 0;
+    const size_t np1 = (size_t)nv + 1;
+    L.off_lattice = off; off = align_up(off + np1 * np1 * np1 * sizeof(float4), 256);
+    L.off_counters = off; off = align_up(off + 64 * sizeof(uint32_t), 256);
+    size_t c1 = (size_t)(P / 2) * (P / 2) * (P / 2);
+    L.off_sums = off; off = align_up(off + (c1 / SCAN_BLOCK + 2) * sizeof(uint32_t), 256);
+    for (int l = 1; l <= levels; ++l) {
+        size_t c = (size_t)(P >> l) * (P >> l) * (P >> l);
+        L.cells[l] = c;
+        L.off_mask[l] = off; off = align_up(off + align_up(c, 8), 256);
+        L.off_offs[l] = off; off = align_up(off + c * sizeof(uint32_t), 256);
+    }
+    L.off_nodes = off;
+    L.fixed_bytes = off;
+    return L;
+}
+
+size_t max_nodes_for(const BuildLayout& L, int64_t max_occ)
+{
+    size_t total = 0;
+    for (int l = 1; l <= L.levels; ++l)
+        total += (size_t)((int64_t)L.cells[l] < max_occ ? (int64_t)L.cells[l] : max_occ);
+    return total ? total : 1;
+}
+
+constexpr size_t NODE_BYTES = sizeof(NifNode) + 2 * sizeof(float4);
+
+int device_is_sm100()
+{
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return 0; }
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        (void)cudaGetLastError(); return 0;
+    }
+    return major == 10;
+}
+
+}  // namespace
+
+extern "C" int nif_device_supported(void) { return device_is_sm100(); }
+
+extern "C" int nif_bvh_workspace_bytes(int32_t nv, int64_t max_occupied, size_t* bytes)
+{
+    if (!bytes || nv < 2 || nv > 512 || max_occupied < 0) return NIF_ERR_INVALID_ARG;
+    int64_t all = (int64_t)nv * nv * nv;
+    if (max_occupied > all) max_occupied = all;
+    BuildLayout L = make_layout(nv);
+    *bytes = L.fixed_bytes + align_up(max_nodes_for(L, max_occupied) * NODE_BYTES, 256) + 256;
+    return NIF_OK;
+}
+
+extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_deform_params* pose,
+                                      void* workspace, size_t workspace_bytes, void* stream_,
+                                      nif_bvh** out)
+{
+    if (!voxels || !pose || !workspace || !out || !voxels->occupancy) return NIF_ERR_INVALID_ARG;
+    const int nv = voxels->nv;
+    if (nv < 2 || nv > 512) return NIF_ERR_INVALID_ARG;
+    if (!isfinite(pose->twist_theta_max) || !isfinite(pose->bend_k)) return NIF_ERR_INVALID_ARG;
+    if (((uintptr_t)workspace & 255u) != 0) return NIF_ERR_WORKSPACE;
+    if (!device_is_sm100()) return NIF_ERR_UNSUPPORTED;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const BuildLayout L = make_layout(nv);
+    if (workspace_bytes < L.fixed_bytes + NODE_BYTES) return NIF_ERR_WORKSPACE;
+    char* ws = (char*)workspace;
+    float4* lattice = (float4*)(ws + L.off_lattice);
+    uint32_t* counters = (uint32_t*)(ws + L.off_counters);
+    uint32_t* sums = (uint32_t*)(ws + L.off_sums);
+    const size_t node_capacity = (workspace_bytes - L.off_nodes) / NODE_BYTES;
+
+    NIF_CUDA_TRY(cudaMemsetAsync(counters, 0, 64 * sizeof(uint32_t), stream));
+    {
+        const size_t np1 = (size_t)nv + 1, total = np1 * np1 * np1;
+        int blocks = (int)((total + 255) / 256);
+        if (blocks > 148 * 32) blocks = 148 * 32;
+        k_deform_lattice<<<blocks, 256, 0, stream>>>(nv, (double)pose->twist_theta_max,
+                                                     (double)pose->bend_k, lattice);
+        nif_count_launch(1);
+    }
+    for (int l = 1; l <= L.levels; ++l) {
+        const uint32_t c = (uint32_t)L.cells[l];
+        uint8_t* mask = (uint8_t*)(ws + L.off_mask[l]);
+        uint32_t* offs = (uint32_t*)(ws + L.off_offs[l]);
+        if (l == 1)
+            k_brick_mask<<<(c + 255) / 256, 256, 0, stream>>>(nv, voxels->occupancy, c, mask, counters);
+        else
+            k_upper_mask<<<(c + 255) / 256, 256, 0, stream>>>((const uint8_t*)(ws + L.off_mask[l - 1]), c, mask);
+        const uint32_t nb = (c + SCAN_BLOCK - 1) / SCAN_BLOCK;
+        k_scan_count<<<nb, SCAN_THREADS, 0, stream>>>(mask, c, sums);
+        k_scan_sums<<<1, SCAN_THREADS, 0, stream>>>(sums, nb, counters + 2 + l);
+        k_scan_write<<<nb, SCAN_THREADS, 0, stream>>>(mask, c, sums, offs);
+        nif_count_launch(4);
+    }
+    uint32_t h_counters[64];
+    NIF_CUDA_TRY(cudaMemcpyAsync(h_counters, counters, sizeof(h_counters), cudaMemcpyDeviceToHost, stream));
+    NIF_CUDA_TRY(cudaStreamSynchronize(stream));
+    NIF_CUDA_TRY(cudaGetLastError());
+
+    const uint32_t n_occ = h_counters[0];
+    // fold-over check (R7): the twist keeps y, so the largest k*y over occupied corners
+    // is k * rest-y of the highest occupied corner.
+    if (n_occ && fabsf(pose->bend_k) >= 1e-6f) {
+        double ytop = (2.0 * (double)h_counters[1] - nv) / nv;
+        double ybot = -1.0;                       // k < 0 folds at the bottom; be conservative
+        double worst = pose->bend_k > 0 ? (double)pose->bend_k * ytop : (double)pose->bend_k * ybot;
+        if (worst >= 1.0 - 1e-3) return NIF_ERR_DEFORM_SINGULAR;
+    }
+    uint32_t base[12] = {0};
+    size_t n_nodes = 0;
+    for (int l = 1; l <= L.levels; ++l) { base[l] = (uint32_t)n_nodes; n_nodes += h_counters[2 + l]; }
+    if (n_nodes > node_capacity) return NIF_ERR_WORKSPACE;
+    NifNode* nodes = (NifNode*)(ws + L.off_nodes);
+    float4* boxes = (float4*)(ws + L.off_nodes + align_up(node_capacity * sizeof(NifNode), 256));
+    // boxes region must fit too: node_capacity was computed with NODE_BYTES per node, minus alignment slack
+    if ((char*)(boxes + 2 * n_nodes) > ws + workspace_bytes) return NIF_ERR_WORKSPACE;
+
+    nif_bvh* b = new (std::nothrow) nif_bvh();
+    if (!b) return NIF_ERR_CUDA;
+    b->nv = nv; b->n_occupied = (int32_t)n_occ; b->n_nodes = (int32_t)n_nodes; b->depth = L.levels;
+    b->root = -1;
+    b->theta_max = pose->twist_theta_max; b->bend_k = pose->bend_k;
+    b->lattice = lattice; b->nodes = nodes;
+    for (int a = 0; a < 3; ++a) { b->lo[a] = 0.f; b->hi[a] = 0.f; }
+    if (n_occ) {
+        for (int l = 1; l <= L.levels; ++l) {
+            const uint32_t c = (uint32_t)L.cells[l];
+            const uint8_t* mask = (const uint8_t*)(ws + L.off_mask[l]);
+            const uint32_t* offs = (const uint32_t*)(ws + L.off_offs[l]);
+            if (l == 1)
+                k_write_bricks<<<(c + 127) / 128, 128, 0, stream>>>(nv, c, mask, offs, base[1], lattice, nodes, boxes);
+            else
+                k_write_level<<<(c + 127) / 128, 128, 0, stream>>>(
+                    c, mask, offs, base[l], (const uint8_t*)(ws + L.off_mask[l - 1]),
+                    (const uint32_t*)(ws + L.off_offs[l - 1]), base[l - 1], nodes, boxes);
+            nif_count_launch(1);
+        }
+        b->root = (int32_t)base[L.levels];
+        float4 rb[2];
+        cudaError_t e = cudaMemcpyAsync(rb, boxes + 2 * (size_t)b->root, sizeof(rb), cudaMemcpyDeviceToHost, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) { (void)cudaGetLastError(); delete b; return NIF_ERR_CUDA; }
+        b->lo[0] = rb[0].x; b->lo[1] = rb[0].y; b->lo[2] = rb[0].z;
+        b->hi[0] = rb[1].x; b->hi[1] = rb[1].y; b->hi[2] = rb[1].z;
+    }
+    *out = b;
+    return NIF_OK;
+}
+
+extern "C" int nif_bvh_get_info(const nif_bvh* b, nif_bvh_info* info)
+{
+    if (!b || !info) return NIF_ERR_INVALID_ARG;
+    info->nv = b->nv; info->n_occupied = b->n_occupied; info->n_nodes = b->n_nodes;
+    info->depth = b->depth;
+    for (int a = 0; a < 3; ++a) { info->lo[a] = b->lo[a]; info->hi[a] = b->hi[a]; }
+    info->theta_max = b->theta_max; info->bend_k = b->bend_k;
+    return NIF_OK;
+}
+
+extern "C" int nif_bvh_get_lattice(const nif_bvh* b, const float** lattice_xyzw)
+{
+    if (!b || !lattice_xyzw) return NIF_ERR_INVALID_ARG;
+    *lattice_xyzw = reinterpret_cast<const float*>(b->lattice);
+    return NIF_OK;
+}
+
+extern "C" void nif_bvh_destroy(nif_bvh* b) { delete b; }

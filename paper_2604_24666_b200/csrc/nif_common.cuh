@@ -1,0 +1,91 @@
+// nif_common.cuh -- internal types shared by the CUDA translation units of libnif.so.
+// Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+#include <math.h>
+
+#include "nif.h"
+
+#define NIF_MAX_LEVELS 16
+#define NIF_MAX_LAYERS 9      // hidden_layers (<= 8) + output layer
+#define NIF_MAX_BANDS 8
+
+// One node of the 8-wide hierarchy over deformed voxels.
+// Children are the non-empty octants of an octree cell of the REST lattice; the boxes are the
+// exact fp32 min/max of the DEFORMED voxels below them, so boxes nest exactly and culling is
+// bit-exactly conservative (R10).  256 bytes = two 128 B lines.
+struct __align__(16) NifNode {
+    float lo[3][8];        // [axis][child]
+    float hi[3][8];
+    uint32_t child[8];     // is_brick ? rest-space voxel id : node index
+    uint32_t mask;         // bit c set <=> child c exists
+    uint32_t is_brick;     // children are voxels (lowest level)
+    uint32_t pad[6];
+};
+static_assert(sizeof(NifNode) == 256, "NifNode must be 256 bytes");
+
+struct nif_bvh {
+    int32_t nv;
+    int32_t n_occupied;
+    int32_t n_nodes;
+    int32_t depth;
+    int32_t root;          // node index, -1 if the grid is empty
+    float lo[3], hi[3];
+    float theta_max, bend_k;
+    const float4* lattice; // device, (nv+1)^3
+    const NifNode* nodes;  // device
+};
+
+// Encoding geometry handed to kernels by value.
+struct NifEnc {
+    int32_t bands, levels, log2_T, feat;
+    int32_t res[NIF_MAX_LEVELS];
+    uint32_t dense_mask;   // bit l set <=> level l is dense ((N+1)^3 <= T)
+};
+
+struct nif_net {
+    nif_net_desc desc;
+    NifEnc enc;
+    int32_t d_in;
+    const void* table;                 // borrowed device pointer
+    void* w_plain[NIF_MAX_LAYERS];     // device copies, row-major (fan_out, fan_in), net dtype
+    void* w_tc;                        // device: tensor-core operand images (NIF_F16 only)
+    size_t w_tc_bytes;
+    size_t w_tc_layer_off[NIF_MAX_LAYERS];
+    int tc_supported;
+};
+
+// per-query scratch layout (device)
+struct NifQueryScratch {
+    unsigned long long n_hit;          // hit rays appended by the traversal
+    unsigned int tile_counter;         // dynamic tile scheduler of the fused kernel
+    unsigned int pad[13];
+    // followed by int32 hit_list[n]
+};
+static_assert(sizeof(NifQueryScratch) == 64, "scratch header is 64 bytes");
+
+extern "C" void nif_count_launch(int n);
+
+#define NIF_CUDA_TRY(expr)                                   \
+    do {                                                     \
+        cudaError_t _e = (expr);                             \
+        if (_e != cudaSuccess) { (void)cudaGetLastError(); return NIF_ERR_CUDA; } \
+    } while (0)
+
+// launchers implemented in the individual .cu files
+int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
+                        NifQueryScratch* scratch, int32_t* hit_list, unsigned flags,
+                        cudaStream_t stream);
+int nif_launch_ffma(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                    const nif_query_out* out, const NifQueryScratch* scratch,
+                    const int32_t* hit_list, unsigned flags, cudaStream_t stream);
+int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                        const nif_query_out* out, NifQueryScratch* scratch,
+                        const int32_t* hit_list, unsigned flags, cudaStream_t stream);
+int nif_tc_pack_weights(nif_net* net, cudaStream_t stream);
+int nif_tc_supported(const nif_net_desc* d);
+
+extern "C" int nif_device_supported(void);

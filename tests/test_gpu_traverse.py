@@ -1,0 +1,168 @@
+"""`-m gpu` parity: steps (a0) build and (a1) traversal of the CUDA path against the oracle,
+through the C ABI.  Ids and hit flags bit-exact, t within 1e-5 relative (BASELINE.json:5)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import nif_inputs as I
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def H():
+    import harness
+    return harness
+
+
+@pytest.fixture(scope="module")
+def P():
+    import parity
+    return parity
+
+
+def _trav(H, case):
+    import paper_2604_24666_b200 as nif
+    return H.run_gpu(case, flags=nif.NIF_TRAVERSE_ONLY, raw_logits=False)
+
+
+@pytest.mark.parametrize("cfg_id,pose_index", [(0, 0), (1, 0), (2, 3), (4, 0)])
+def test_deformed_lattice_matches_oracle(oracle, H, cfg_id, pose_index):
+    # both sides evaluate O2 in fp64 with their own libm and round once; a last-bit fp64
+    # difference can flip an fp32 rounding with probability ~1e-8 per value (R7)
+    case = H.make_case(cfg_id, n_rays=16, pose_index=pose_index, with_net=False)
+    got = case.bvh.lattice().cpu().numpy()
+    want = oracle.deform_lattice(case.cfg.nv, float(case.pose[0]), float(case.pose[1]))
+    diff = got.view(np.int32) != want.view(np.int32)
+    n_bad = int(diff.sum())
+    assert n_bad <= max(1, int(2e-7 * want.size)), n_bad
+    if n_bad:
+        assert np.abs(got.view(np.int32)[diff] - want.view(np.int32)[diff]).max() <= 1
+    info = case.bvh.info()
+    assert info["n_occupied"] == int(case.occ.sum())
+    if n_bad == 0:
+        obvh = oracle.bvh_build(case.cfg.nv, case.occ, want)
+        lo, hi = obvh.bounds()
+        assert np.array_equal(lo, info["lo"]) and np.array_equal(hi, info["hi"])
+
+
+def test_identity_pose_lattice_is_rest_lattice(H):
+    cfg = I.get_config(0)
+    case = H.make_case(0, n_rays=16, with_net=False, pose=[0.0, 0.0])
+    nv = cfg.nv
+    lat = case.bvh.lattice().cpu().numpy().reshape(nv + 1, nv + 1, nv + 1, 3)
+    c = ((2.0 * np.arange(nv + 1) - nv) / nv).astype(np.float32)
+    assert np.array_equal(lat[..., 0], np.broadcast_to(c[None, None, :], lat.shape[:3]))
+    assert np.array_equal(lat[..., 1], np.broadcast_to(c[None, :, None], lat.shape[:3]))
+    assert np.array_equal(lat[..., 2], np.broadcast_to(c[:, None, None], lat.shape[:3]))
+
+
+def test_traversal_config0_all_rays_vs_brute_force_definition(oracle, H, P):
+    case = H.make_case(0, with_net=False)
+    gpu = _trav(H, case)
+    lat = oracle.deform_lattice(case.cfg.nv, *map(float, case.pose))
+    vid, ti, to = oracle.traverse_brute(case.cfg.nv, case.occ, lat, case.origin, case.direction)
+    m = P.compare_traversal(gpu, {"voxel_id": vid, "t_in": ti, "t_out": to})
+    P.assert_traversal(m)
+    assert m["t_in_bit_mismatch"] == 0 and m["t_out_bit_mismatch"] == 0, m
+    assert gpu["n_hit_counter"] == 0        # TRAVERSE_ONLY does not compact
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_traversal_random_grids_vs_brute_force(oracle, H, P, seed):
+    rng = np.random.default_rng(200 + seed)
+    nv = [8, 8, 6, 12][seed]                      # includes non-power-of-two lattices
+    occ = I.random_occupancy(nv, float(rng.uniform(0.05, 0.6)), seed)
+    pose = [float(rng.uniform(0, math.pi / 2)), float(rng.uniform(0, 0.9))]
+    cfg = I.scaled(I.get_config(0), nv=nv)
+    case = H.make_case(0, n_rays=16, with_net=False, cfg=cfg, occ=occ, pose=pose)
+    lo, hi = case.bvh.info()["lo"], case.bvh.info()["hi"]
+    n = 3000
+    o1 = rng.standard_normal((n, 3)); o1 *= 3.0 / np.linalg.norm(o1, axis=1, keepdims=True)
+    d1 = rng.uniform(lo, hi, (n, 3)) - o1
+    o2 = rng.uniform(lo, hi, (n, 3)); d2 = rng.standard_normal((n, 3))
+    o3 = rng.uniform(lo, hi, (333, 3)); d3 = np.eye(3)[rng.integers(0, 3, 333)] * rng.choice([-1, 1], (333, 1))
+    o = np.concatenate([o1, o2, o3]); d = np.concatenate([d1, d2, d3])
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    case.origin = o.astype(np.float32); case.direction = d.astype(np.float32)
+    case.origin_d = torch.from_numpy(case.origin).cuda(); case.direction_d = torch.from_numpy(case.direction).cuda()
+    gpu = _trav(H, case)
+    lat = oracle.deform_lattice(nv, *pose)
+    vid, ti, to = oracle.traverse_brute(nv, occ, lat, case.origin, case.direction)
+    m = P.compare_traversal(gpu, {"voxel_id": vid, "t_in": ti, "t_out": to})
+    P.assert_traversal(m)
+    assert m["t_in_bit_mismatch"] == 0 and m["t_out_bit_mismatch"] == 0, m
+    assert m["n_hit"] > 500
+
+
+def test_tie_lowest_id_and_face_plane_ray(oracle, H):
+    # same construction as tests/test_oracle_traverse.py: the ray lies in a lattice plane
+    nv = 4
+    cfg = I.scaled(I.get_config(0), nv=nv)
+    case = H.make_case(0, n_rays=16, with_net=False, cfg=cfg, occ=np.ones(nv ** 3, np.uint8), pose=[0.0, 0.0])
+    case.origin = np.array([[-3.0, 0.0, 0.25]], np.float32); case.direction = np.array([[1.0, 0.0, 0.0]], np.float32)
+    case.origin_d = torch.from_numpy(case.origin).cuda(); case.direction_d = torch.from_numpy(case.direction).cuda()
+    gpu = _trav(H, case)
+    assert gpu["voxel_id"][0] == 0 + nv * (1 + nv * 2) and gpu["t_in"][0] == 2.0 and gpu["t_out"][0] == 2.5
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 129, 1000])
+def test_ragged_and_empty_batches(oracle, H, P, n):
+    case = H.make_case(0, n_rays=max(n, 1), with_net=False)
+    case.origin = case.origin[:n]; case.direction = case.direction[:n]
+    case.origin_d = case.origin_d[:n].contiguous(); case.direction_d = case.direction_d[:n].contiguous()
+    gpu = _trav(H, case)
+    if n == 0:
+        assert gpu["voxel_id"].shape == (0,)
+        return
+    ref = H.OracleSide(oracle, case).query(traverse_only=True)
+    P.assert_traversal(P.compare_traversal(gpu, ref))
+
+
+def test_empty_grid_everything_misses(H):
+    cfg = I.scaled(I.get_config(0), nv=8)
+    case = H.make_case(0, n_rays=500, with_net=False, cfg=cfg, occ=np.zeros(512, np.uint8))
+    assert case.bvh.info()["n_occupied"] == 0 and case.bvh.info()["n_nodes"] == 0
+    gpu = _trav(H, case)
+    assert (gpu["voxel_id"] == -1).all() and np.isinf(gpu["t_in"]).all() and np.isinf(gpu["t_out"]).all()
+
+
+def test_single_voxel_and_full_grid(oracle, H, P):
+    for occ in (np.eye(1, 64, 21, dtype=np.uint8)[0], np.ones(64, np.uint8)):
+        cfg = I.scaled(I.get_config(0), nv=4)
+        case = H.make_case(0, n_rays=2000, with_net=False, cfg=cfg, occ=occ, pose=[0.8, 0.5])
+        gpu = _trav(H, case)
+        lat = oracle.deform_lattice(4, 0.8, 0.5)
+        vid, ti, to = oracle.traverse_brute(4, occ, lat, case.origin, case.direction)
+        P.assert_traversal(P.compare_traversal(gpu, {"voxel_id": vid, "t_in": ti, "t_out": to}))
+
+
+def test_fold_over_pose_is_rejected(H):
+    import paper_2604_24666_b200 as nif
+    cfg = I.scaled(I.get_config(0), nv=8)
+    with pytest.raises(nif.NifError) as e:
+        H.make_case(0, n_rays=16, with_net=False, cfg=cfg, occ=np.ones(512, np.uint8), pose=[0.0, 1.2])
+    assert e.value.status == -3          # NIF_ERR_DEFORM_SINGULAR
+
+
+def test_workspace_too_small_is_rejected(H):
+    import paper_2604_24666_b200 as nif
+    cfg = I.get_config(0)
+    occ = torch.from_numpy(I.occupancy(cfg)).cuda()
+    with pytest.raises(nif.NifError) as e:
+        nif.nif_build_deformed_bvh(cfg.nv, occ, 1.0, 0.0, max_occupied=1)
+    assert e.value.status == -4          # NIF_ERR_WORKSPACE
+
+
+@pytest.mark.parametrize("cfg_id,n,pose_index", [(1, 40_000, 0), (2, 30_000, 0), (2, 30_000, 4), (3, 30_000, 2)])
+def test_traversal_reduced_configs_all_rays(oracle, H, P, cfg_id, n, pose_index):
+    # configs 1-3 at a size the oracle traverses completely in seconds (its own BVH, which
+    # tests/test_oracle_traverse.py pins bit-exactly to the brute-force definition)
+    case = H.make_case(cfg_id, n_rays=n, pose_index=pose_index, with_net=False)
+    gpu = _trav(H, case)
+    ref = H.OracleSide(oracle, case).query(traverse_only=True)
+    m = P.compare_traversal(gpu, ref)
+    P.assert_traversal(m)
+    assert m["n_hit"] > 1000, m
