@@ -153,6 +153,11 @@ int nif_net_create(const nif_net_desc* desc, const void* table, const void* cons
                    void* stream, nif_net** out);
 void nif_net_destroy(nif_net* net);
 
+/* 1 if nif_query runs this net on the tcgen05 fused encode+MLP kernel, 0 if on the scalar-FMA
+ * kernel (NIF_F32 nets, shapes the tensor-core kernel does not cover), negative on error.
+ * Host-only. */
+int nif_net_uses_tensor_cores(const nif_net* net);
+
 /* -------- steps (a1)-(a5): the query ------------------------------------------------------ */
 
 /* Scratch bytes nif_query needs for a batch of n rays.  Host-only. */
@@ -185,6 +190,22 @@ int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
 /* Counters of the last nif_query on this thread's workspace: hit rays found by the traversal.
  * Reads 8 bytes back from the workspace; SYNCHRONISES `stream`. */
 int nif_query_last_hit_count(const void* workspace, void* stream, int64_t* n_hit);
+
+/* Per-kernel timing of nif_query (bench.py's roofline figure is taken from it).  After
+ * nif_profile_enable(1) every nif_query records CUDA events on its stream before the traversal
+ * kernel, between it and the encode+MLP kernel, and after; up to 512 queries are remembered.
+ * nif_profile_read SYNCHRONISES on those events, returns the summed kernel milliseconds of the
+ * remembered queries and forgets them.  nif_profile_enable(0) switches the events off again. */
+int nif_profile_enable(int on);
+int nif_profile_read(double* traverse_ms, double* network_ms, int64_t* n_queries);
+
+/* Random-sector gather probe: the denominator of the gather roofline.
+ * All SMs issue independent 4-byte loads at pseudo-random 32-byte sectors of the DEVICE buffer
+ * `buf` (`bytes` rounded down to a power-of-two number of sectors); `iters` batches of 8 loads
+ * per thread, 4 x 512 threads per SM.  Returns the best of 3 timed launches as 32-byte sectors
+ * per second (and its milliseconds in *ms, optional).  SYNCHRONISES. */
+int nif_probe_gather(const void* buf, size_t bytes, int iters, void* stream,
+                     double* sectors_per_s, double* ms);
 
 /* Kernels launched by the library since load (every nif_* call adds its launches). */
 int64_t nif_kernel_launch_count(void);

@@ -83,6 +83,7 @@ def lib() -> C.CDLL:
                                      C.POINTER(C.c_void_p)]
         L.nif_net_destroy.argtypes = [C.c_void_p]
         L.nif_net_destroy.restype = None
+        L.nif_net_uses_tensor_cores.argtypes = [C.c_void_p]
         L.nif_query_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_query.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut),
                                 C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
@@ -92,6 +93,10 @@ def lib() -> C.CDLL:
         L.nif_query_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(_RayBatch),
                                      C.POINTER(_QueryOut), C.c_uint]
         L.nif_query_last_hit_count.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+        L.nif_profile_enable.argtypes = [C.c_int]
+        L.nif_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.nif_probe_gather.argtypes = [C.c_void_p, C.c_size_t, C.c_int, C.c_void_p, C.POINTER(C.c_double),
+                                       C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -201,6 +206,12 @@ def nif_net_create(shape, level_res, table: torch.Tensor, weights: list, stream=
     return Net(h, (table, list(weights)))
 
 
+def nif_net_uses_tensor_cores(net: Net) -> bool:
+    r = lib().nif_net_uses_tensor_cores(net.handle)
+    _check(min(r, 0), "nif_net_uses_tensor_cores")
+    return bool(r)
+
+
 def nif_query_workspace_bytes(n: int) -> int:
     b = C.c_size_t()
     _check(lib().nif_query_workspace_bytes(n, C.byref(b)), "nif_query_workspace_bytes")
@@ -250,6 +261,26 @@ def nif_query_last_hit_count(workspace: torch.Tensor, stream=None) -> int:
     _check(lib().nif_query_last_hit_count(workspace.data_ptr(), _stream_ptr(stream), C.byref(v)),
            "nif_query_last_hit_count")
     return v.value
+
+
+def nif_profile_enable(on: bool):
+    _check(lib().nif_profile_enable(1 if on else 0), "nif_profile_enable")
+
+
+def nif_profile_read() -> dict:
+    """Summed per-kernel milliseconds of the queries issued since the last read (synchronises)."""
+    t, m, n = C.c_double(), C.c_double(), C.c_int64()
+    _check(lib().nif_profile_read(C.byref(t), C.byref(m), C.byref(n)), "nif_profile_read")
+    return {"traverse_ms": t.value, "network_ms": m.value, "n_queries": n.value}
+
+
+def nif_probe_gather(buf: torch.Tensor, iters: int = 64, stream=None) -> dict:
+    """Random 32-byte-sector gather rate over `buf` (CUDA tensor); see include/nif.h."""
+    assert buf.is_cuda and buf.is_contiguous()
+    r, ms = C.c_double(), C.c_double()
+    _check(lib().nif_probe_gather(buf.data_ptr(), buf.numel() * buf.element_size(), iters,
+                                  _stream_ptr(stream), C.byref(r), C.byref(ms)), "nif_probe_gather")
+    return {"sectors_per_s": r.value, "gbps": r.value * 32 / 1e9, "ms": ms.value}
 
 
 class Stage:

@@ -14,7 +14,7 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 INCLUDE = HERE.parent / "include"
 LIB = HERE / "libnif.so"
-SOURCES = ["nif_api.cu", "nif_build.cu", "nif_traverse.cu", "nif_mlp_ffma.cu", "nif_fused_tc.cu"]
+SOURCES = ["nif_api.cu", "nif_build.cu", "nif_traverse.cu", "nif_mlp_ffma.cu", "nif_fused_tc.cu", "nif_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
@@ -56,8 +56,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         raise RuntimeError("nvcc failed")
     if procs or not LIB.exists():
         tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
-        subprocess.check_call([_nvcc(), "-shared", "-o", str(tmp), *map(str, objs), "-Xcompiler", "-fPIC",
-                               "-cudart", "static"])
+        subprocess.check_call([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(tmp),
+                               *map(str, objs), "-Xcompiler", "-fPIC", "-cudart", "static"])
         os.replace(tmp, LIB)
     return LIB
 

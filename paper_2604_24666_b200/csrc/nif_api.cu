@@ -104,6 +104,12 @@ extern "C" void nif_net_destroy(nif_net* net)
     delete net;
 }
 
+extern "C" int nif_net_uses_tensor_cores(const nif_net* net)
+{
+    if (!net) return NIF_ERR_INVALID_ARG;
+    return net->desc.dtype == NIF_F16 && net->tc_supported ? 1 : 0;
+}
+
 // ---------------------------------------------------------------------------------------------
 // query
 // ---------------------------------------------------------------------------------------------
@@ -144,11 +150,15 @@ extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_b
     NifQueryScratch* scratch = (NifQueryScratch*)workspace;
     int32_t* hit_list = (int32_t*)((char*)workspace + sizeof(NifQueryScratch));
     NIF_CUDA_TRY(cudaMemsetAsync(scratch, 0, sizeof(NifQueryScratch), stream));
+    const int prof = nif_prof_begin(stream);                 // -1 unless nif_profile_enable(1)
     rc = nif_launch_traverse(bvh, rays, out, scratch, hit_list, flags, stream);
+    nif_prof_mark(prof, 1, stream);
     if (rc != NIF_OK || (flags & NIF_TRAVERSE_ONLY)) return rc;
     const bool use_tc = net->desc.dtype == NIF_F16 && net->tc_supported && !(flags & NIF_ENGINE_FFMA);
-    if (use_tc) return nif_launch_fused_tc(bvh, net, rays, out, scratch, hit_list, flags, stream);
-    return nif_launch_ffma(bvh, net, rays, out, scratch, hit_list, flags, stream);
+    if (use_tc) rc = nif_launch_fused_tc(bvh, net, rays, out, scratch, hit_list, flags, stream);
+    else rc = nif_launch_ffma(bvh, net, rays, out, scratch, hit_list, flags, stream);
+    nif_prof_mark(prof, 2, stream);
+    return rc;
 }
 
 extern "C" int nif_query_last_hit_count(const void* workspace, void* stream_, int64_t* n_hit)

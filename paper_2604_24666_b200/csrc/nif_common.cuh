@@ -89,3 +89,7 @@ int nif_tc_pack_weights(nif_net* net, cudaStream_t stream);
 int nif_tc_supported(const nif_net_desc* d);
 
 extern "C" int nif_device_supported(void);
+
+// per-kernel event timing hooks (nif_probe.cu); slot < 0 = profiling off
+int nif_prof_begin(cudaStream_t stream);
+void nif_prof_mark(int slot, int which, cudaStream_t stream);
