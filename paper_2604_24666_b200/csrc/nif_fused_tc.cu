@@ -1,6 +1,629 @@
-// nif_fused_tc.cu -- placeholder until the tcgen05 fused encode+MLP kernel lands (next commit).
-#include "nif_common.cuh"
-int nif_tc_supported(const nif_net_desc*) { return 0; }
-int nif_tc_pack_weights(nif_net*, cudaStream_t) { return NIF_ERR_UNSUPPORTED; }
-int nif_launch_fused_tc(const nif_bvh*, const nif_net*, const nif_ray_batch*, const nif_query_out*,
-                        NifQueryScratch*, const int32_t*, unsigned, cudaStream_t) { return NIF_ERR_UNSUPPORTED; }
+// nif_fused_tc.cu -- steps (a2)-(a5) for NIF_F16 networks as ONE persistent sm_100a kernel:
+// inverse deformation -> composite encoding psi = phi o gamma (Eq. 1) -> MLP on
+// tcgen05 tensor cores -> head decode, per tile of 128 hit rays, with no
+// intermediate HBM round trip.
+//
+// Warp roles (one CTA per SM, TC_THREADS threads):
+//   warps 0-3   "row" warps: thread r owns ray r of the tile.  They prepare the NEXT tile's rest-space
+//               endpoints (a2), then drain the layer-1 accumulator from TMEM (tcgen05.ld), run the
+//               hidden and output layers (ReLU -> fp16 -> swizzled smem A operand -> tcgen05.mma,
+//               issued by thread 0) and decode/store the heads (a5).
+//   warp 4      allocates TMEM; one lane issues the layer-1 MMAs chunk by chunk as the gather warps
+//               fill the A-operand ring (full/empty mbarriers), commits to the accumulator barrier.
+//   warps 5..   gather warps: lane = ray, one work item = (32-ray group, endpoint, PE sample); the
+//               L levels of that sample are interpolated (8 table gathers each, fp32) and written as
+//               fp16 into the canonical K-major SWIZZLE_128B A tile, 16 bytes per store.
+// Weights sit in shared memory for the whole kernel as pre-swizzled B-operand images, loaded once
+// with cp.async.bulk.  The layer-1 accumulator is double-buffered in TMEM so the gathers of tile
+// t+1 overlap the MLP tail of tile t.
+#include "nif_encode.cuh"
+
+namespace {
+
+constexpr int TC_TILE = 128;                 // rays per tile = UMMA M
+constexpr int TC_ROW_WARPS = 4;
+constexpr int TC_GATHER_WARPS = 16;
+constexpr int TC_MMA_WARP = TC_ROW_WARPS;    // warp index 4
+constexpr int TC_THREADS = 32 * (TC_ROW_WARPS + 1 + TC_GATHER_WARPS);
+constexpr int TC_STAGES = 4;                 // A-operand ring depth (K chunks of 64 columns)
+constexpr int TC_A_CHUNK_BYTES = TC_TILE * 128;
+constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded to the UMMA minimum)
+
+// ---- PTX wrappers -----------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+
+// D[tmem] (+)= A[smem] * B[smem]^T, fp16 operands, fp32 accumulate, M = 128
+__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// all previously issued MMAs of this thread arrive on `bar` when they complete (implies fence::before_thread_sync)
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// K-major SWIZZLE_128B shared-memory matrix descriptor: rows of 128 bytes, 8-row groups 1024 bytes
+// apart (SBO), LBO unused (1), descriptor version 1 (sm_100), layout type 2 (cute::UMMA::SWIZZLE_128B)
+__device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t addr)
+{
+    return (uint64_t)((addr & 0x3ffffu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
+           ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+// instruction descriptor, kind::f16: D fp32 (bit 4), A/B fp16 (0), both K-major, N>>3 at bit 17, M>>4 at bit 24
+__host__ __device__ constexpr uint32_t idesc_f16(int M, int N)
+{
+    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+// TMEM -> registers: this warp's 32 lanes x 32 consecutive fp32 columns (thread = lane = row)
+__device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t* v)
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t* v)
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void row_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
+__device__ __forceinline__ uint32_t pack_half2(float a, float b)
+{
+    __half2 h = __floats2half2_rn(a, b);
+    return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// byte offset of the 16-byte unit `unit` (0..7) of row `row` inside a [rows x 128 B] SWIZZLE_128B chunk
+__host__ __device__ __forceinline__ uint32_t sw128_off(uint32_t row, uint32_t unit)
+{
+    return row * 128u + ((unit ^ (row & 7u)) << 4);
+}
+
+// ---- kernel parameters -------------------------------------------------------------------------
+struct TcParams {
+    NifEnc enc;
+    int hidden_layers;            // H
+    int n_chunks;                 // layer-1 K chunks of 64 columns = ceil(2 S L F / 64)
+    int es_per_chunk;             // (endpoint, sample) pairs per chunk = 64 / (L F)
+    int n_es;                     // 2 S
+    const __half* table;
+    const uint8_t* w_img;         // B-operand images: W1 chunks | hidden layers 2..H | output layer
+    uint32_t w_bytes;
+    float theta_max, bend_k;
+    const float* origin;
+    const float* dir;
+    nif_query_out out;
+    const NifQueryScratch* scratch;
+    const int32_t* hit_list;
+    unsigned flags;
+};
+
+struct TcSmemLayout {
+    uint32_t w_img, a_ring, act, ray_buf, bars, total;
+};
+__host__ __device__ inline TcSmemLayout tc_smem_layout(uint32_t w_bytes, int W)
+{
+    TcSmemLayout L;
+    uint32_t off = 0;
+    L.w_img = off;   off += (w_bytes + 1023u) & ~1023u;
+    L.a_ring = off;  off += TC_STAGES * TC_A_CHUNK_BYTES;
+    L.act = off;     off += (uint32_t)((W + 63) / 64) * TC_A_CHUNK_BYTES;
+    L.ray_buf = off; off += 2u * TC_TILE * 8u * sizeof(float);
+    L.bars = off;    off += 512;
+    L.total = off + 1024;                       // slack for the manual 1024-byte alignment
+    return L;
+}
+
+enum { BAR_FULL = 0, BAR_EMPTY = TC_STAGES, BAR_ACC_FULL = 2 * TC_STAGES, BAR_ACC_EMPTY = BAR_ACC_FULL + 2,
+       BAR_RAY_FULL = BAR_ACC_EMPTY + 2, BAR_RAY_EMPTY = BAR_RAY_FULL + 2, BAR_HID = BAR_RAY_EMPTY + 2,
+       BAR_W = BAR_HID + 1, BAR_COUNT = BAR_W + 1 };
+
+// ---- (a3) one group of levels of one sample: LG * F = 8 features = 16 bytes of the A row ----------
+// Index rule and corner order as nif_level_features (R6); all LG*8 gathers are issued
+// before any is consumed.
+template <int F>
+__device__ __forceinline__ void gather_group(const __half* __restrict__ table, const int* __restrict__ s_res,
+                                             uint32_t dense_mask, int log2_T, int l0,
+                                             float px, float py, float pz, uint32_t packed[4])
+{
+    constexpr int LG = 8 / F;                                 // levels per 16-byte unit
+    const uint32_t t_mask = (1u << log2_T) - 1u;
+    uint32_t idx[LG][8];
+    float wx[LG], wy[LG], wz[LG];
+#pragma unroll
+    for (int li = 0; li < LG; ++li) {
+        const int l = l0 + li;
+        const int N = s_res[l];
+        const float fn = (float)N, top = (float)(N - 1);
+        const float posx = px * fn, posy = py * fn, posz = pz * fn;
+        const float flx = fmaxf(fminf(floorf(posx), top), 0.0f);
+        const float fly = fmaxf(fminf(floorf(posy), top), 0.0f);
+        const float flz = fmaxf(fminf(floorf(posz), top), 0.0f);
+        wx[li] = posx - flx; wy[li] = posy - fly; wz[li] = posz - flz;
+        const uint32_t cx = (uint32_t)flx, cy = (uint32_t)fly, cz = (uint32_t)flz;
+        if ((dense_mask >> l) & 1u) {
+            const uint32_t np1 = (uint32_t)N + 1u;
+            const uint32_t b = cx + np1 * (cy + np1 * cz);
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                idx[li][c] = b + (uint32_t)(c & 1) + np1 * ((uint32_t)((c >> 1) & 1) + np1 * (uint32_t)(c >> 2));
+        } else {
+            const uint32_t hy0 = cy * 2654435761u, hy1 = hy0 + 2654435761u;
+            const uint32_t hz0 = cz * 805459861u, hz1 = hz0 + 805459861u;
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                idx[li][c] = ((cx + (uint32_t)(c & 1)) ^ (((c >> 1) & 1) ? hy1 : hy0) ^ ((c >> 2) ? hz1 : hz0)) & t_mask;
+        }
+    }
+    float feat[LG][F];
+    if constexpr (F == 2) {
+        uint32_t raw[LG][8];
+#pragma unroll
+        for (int li = 0; li < LG; ++li) {
+            const uint32_t* lvl = reinterpret_cast<const uint32_t*>(table) + ((size_t)(l0 + li) << log2_T);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(lvl + idx[li][c]);
+        }
+#pragma unroll
+        for (int li = 0; li < LG; ++li) {
+            float f0 = 0.0f, f1 = 0.0f;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const float w = (((c & 1) ? wx[li] : 1.0f - wx[li]) * (((c >> 1) & 1) ? wy[li] : 1.0f - wy[li])) *
+                                ((c >> 2) ? wz[li] : 1.0f - wz[li]);
+                const float2 v = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c]));
+                f0 = fmaf(w, v.x, f0); f1 = fmaf(w, v.y, f1);
+            }
+            feat[li][0] = f0; feat[li][1] = f1;
+        }
+    } else {
+        uint2 raw[LG][8];
+#pragma unroll
+        for (int li = 0; li < LG; ++li) {
+            const uint2* lvl = reinterpret_cast<const uint2*>(table) + ((size_t)(l0 + li) << log2_T);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(lvl + idx[li][c]);
+        }
+#pragma unroll
+        for (int li = 0; li < LG; ++li) {
+            float f0 = 0.0f, f1 = 0.0f, f2 = 0.0f, f3 = 0.0f;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const float w = (((c & 1) ? wx[li] : 1.0f - wx[li]) * (((c >> 1) & 1) ? wy[li] : 1.0f - wy[li])) *
+                                ((c >> 2) ? wz[li] : 1.0f - wz[li]);
+                const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c].x));
+                const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c].y));
+                f0 = fmaf(w, a.x, f0); f1 = fmaf(w, a.y, f1); f2 = fmaf(w, b.x, f2); f3 = fmaf(w, b.y, f3);
+            }
+            feat[li][0] = f0; feat[li][1] = f1; feat[li][2] = f2; feat[li][3] = f3;
+        }
+    }
+    const float* ff = &feat[0][0];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) packed[i] = pack_half2(ff[2 * i], ff[2 * i + 1]);
+}
+
+// drains W fp32 accumulator columns of this thread's row from TMEM, applies ReLU, rounds to fp16
+// and writes them as the next layer's A operand (K-major SWIZZLE_128B, chunks of 64 columns)
+template <int W>
+__device__ __forceinline__ void drain_relu_to_act(uint32_t taddr_row, uint32_t act_base, uint32_t row)
+{
+    __syncwarp();                                          // tcgen05.ld is .sync.aligned
+#pragma unroll
+    for (int cg = 0; cg < W / 32; ++cg) {
+        uint32_t v[32];
+        tmem_ld_32x32(taddr_row + (uint32_t)(cg * 32), v);
+        tmem_ld_wait();
+        const uint32_t chunk = act_base + (uint32_t)((cg * 32) / 64) * TC_A_CHUNK_BYTES;
+        const uint32_t unit0 = (uint32_t)(((cg * 32) % 64) / 8);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            uint32_t h[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                h[i] = pack_half2(fmaxf(__uint_as_float(v[8 * u + 2 * i]), 0.0f),
+                                  fmaxf(__uint_as_float(v[8 * u + 2 * i + 1]), 0.0f));
+            st_shared_v4(chunk + sw128_off(row, unit0 + (uint32_t)u), h[0], h[1], h[2], h[3]);
+        }
+    }
+}
+
+// issues D[128 x N] = act[128 x W] * Wimg[N x W]^T (one thread)
+template <int W>
+__device__ __forceinline__ void issue_layer(uint32_t d_tmem, uint32_t act_base, uint32_t w_base, int N)
+{
+    constexpr int KC = (W + 63) / 64;                      // 64-column chunks
+    constexpr int K16 = (W < 64 ? W : 64) / 16;            // UMMA K steps per chunk
+    const uint32_t idesc = idesc_f16(TC_TILE, N);
+#pragma unroll
+    for (int kc = 0; kc < KC; ++kc)
+#pragma unroll
+        for (int k = 0; k < K16; ++k)
+            umma_f16(d_tmem, smem_desc_sw128(act_base + (uint32_t)kc * TC_A_CHUNK_BYTES + (uint32_t)k * 32u),
+                     smem_desc_sw128(w_base + (uint32_t)kc * (uint32_t)(N * 128) + (uint32_t)k * 32u), idesc,
+                     (uint32_t)((kc | k) != 0));
+}
+
+template <int W, int F>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_fused_encode_mlp(const TcParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+    const TcSmemLayout SL = tc_smem_layout(p.w_bytes, W);
+    const uint32_t s_w = smem_base + SL.w_img, s_a = smem_base + SL.a_ring, s_act = smem_base + SL.act;
+    float* ray_buf = reinterpret_cast<float*>(smem_gen + SL.ray_buf);          // [2][128][8]
+    const uint32_t s_bar = smem_base + SL.bars;
+    uint32_t* s_tmem_ptr = reinterpret_cast<uint32_t*>(smem_gen + SL.bars + 8 * BAR_COUNT);
+    int* s_res = reinterpret_cast<int*>(smem_gen + SL.bars + 8 * BAR_COUNT + 16);
+    auto bar = [&](int i) { return s_bar + 8u * (uint32_t)i; };
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int L = p.enc.levels, S = 1 + 2 * p.enc.bands;
+    const int epc = p.es_per_chunk, n_chunks = p.n_chunks;
+    constexpr uint32_t TMEM_COLS = (3 * W + 32) <= 256 ? 256 : 512;
+    constexpr int KC = (W + 63) / 64;
+
+    // ---- one-time setup ------------------------------------------------------------------------
+    if (tid == 0) {
+        for (int i = 0; i < TC_STAGES; ++i) { mbar_init(bar(BAR_FULL + i), 4u * (uint32_t)epc); mbar_init(bar(BAR_EMPTY + i), 1); }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(bar(BAR_ACC_FULL + i), 1); mbar_init(bar(BAR_ACC_EMPTY + i), TC_TILE);
+            mbar_init(bar(BAR_RAY_FULL + i), TC_TILE); mbar_init(bar(BAR_RAY_EMPTY + i), TC_GATHER_WARPS);
+        }
+        mbar_init(bar(BAR_HID), 1); mbar_init(bar(BAR_W), 1);
+        fence_barrier_init();
+    }
+    if (tid < NIF_MAX_LEVELS) s_res[tid] = tid < L ? p.enc.res[tid] : 1;
+    if (warp == TC_MMA_WARP) tmem_alloc(smem_u32(s_tmem_ptr), TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *s_tmem_ptr;
+    const uint32_t tm_acc1 = tmem_base, tm_hid = tmem_base + 2u * W, tm_out = tmem_base + 3u * W;
+
+    const long long n_hit = (long long)p.scratch->n_hit;
+    const long long n_tiles = (n_hit + TC_TILE - 1) / TC_TILE;
+    const int n_my = (int)((n_tiles > (long long)blockIdx.x) ? (n_tiles - 1 - blockIdx.x) / gridDim.x + 1 : 0);
+
+    // weight images -> shared memory, once (TMA bulk copies, completion on BAR_W)
+    if (warp == TC_MMA_WARP && lane == 0 && n_my > 0) {
+        mbar_expect_tx(bar(BAR_W), p.w_bytes);
+        for (uint32_t off = 0; off < p.w_bytes; off += 16384u) {
+            const uint32_t n = p.w_bytes - off < 16384u ? p.w_bytes - off : 16384u;
+            bulk_g2s(s_w + off, p.w_img + off, n, bar(BAR_W));
+        }
+    }
+    const uint32_t s_w1 = s_w;
+    const uint32_t s_wh = s_w + (uint32_t)n_chunks * (uint32_t)(W * 128);
+    const uint32_t s_wo = s_wh + (uint32_t)(p.hidden_layers - 1) * (uint32_t)(KC * W * 128);
+
+    if (warp < TC_ROW_WARPS) {
+        // ======================= row warps: (a2) for the next tile, MLP tail + (a5) ==============
+        const int r = tid;
+        long long cur_ray = -1, nxt_ray = -1;
+        float cur_ti = 0.f, cur_to = 0.f, nxt_ti = 0.f, nxt_to = 0.f;
+        uint32_t hid_phase = 0;
+        auto prepare = [&](int j) {                       // rest-space endpoints of tile j -> ray_buf[j&1]
+            const int b = j & 1;
+            mbar_wait(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
+            const long long tile = (long long)blockIdx.x + (long long)j * gridDim.x;
+            const long long h = tile * TC_TILE + r;
+            float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f;
+            nxt_ray = -1; nxt_ti = 0.f; nxt_to = 0.f;
+            if (h < n_hit) {
+                nxt_ray = p.hit_list[h];
+                nxt_ti = p.out.t_in[nxt_ray]; nxt_to = p.out.t_out[nxt_ray];
+                const float ox = p.origin[3 * nxt_ray], oy = p.origin[3 * nxt_ray + 1], oz = p.origin[3 * nxt_ray + 2];
+                const float dx = p.dir[3 * nxt_ray], dy = p.dir[3 * nxt_ray + 1], dz = p.dir[3 * nxt_ray + 2];
+                nif_inverse_deform(p.theta_max, p.bend_k, fmaf(nxt_ti, dx, ox), fmaf(nxt_ti, dy, oy), fmaf(nxt_ti, dz, oz), xi, yi, zi);
+                nif_inverse_deform(p.theta_max, p.bend_k, fmaf(nxt_to, dx, ox), fmaf(nxt_to, dy, oy), fmaf(nxt_to, dz, oz), xo, yo, zo);
+            }
+            float* rb = ray_buf + ((size_t)b * TC_TILE + r) * 8;
+            rb[0] = nif_normalise(xi); rb[1] = nif_normalise(yi); rb[2] = nif_normalise(zi);
+            rb[3] = nif_normalise(xo); rb[4] = nif_normalise(yo); rb[5] = nif_normalise(zo);
+            mbar_arrive(bar(BAR_RAY_FULL + b));
+        };
+        if (n_my > 0) { prepare(0); mbar_wait(bar(BAR_W), 0); }
+        const uint32_t t_row = (uint32_t)(warp * 32) << 16;          // this warp's TMEM lane quarter
+        for (int j = 0; j < n_my; ++j) {
+            cur_ray = nxt_ray; cur_ti = nxt_ti; cur_to = nxt_to;
+            if (j + 1 < n_my) prepare(j + 1);
+            const int b = j & 1;
+            // layer 1 accumulator of tile j
+            mbar_wait(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1));
+            tc_fence_after();
+            drain_relu_to_act<W>(tm_acc1 + (uint32_t)(b * W) + t_row, s_act, (uint32_t)r);
+            tc_fence_before();
+            mbar_arrive(bar(BAR_ACC_EMPTY + b));
+            fence_proxy_async();
+            row_bar_sync();
+            // hidden layers 2..H
+            for (int hl = 1; hl < p.hidden_layers; ++hl) {
+                if (tid == 0) {
+                    tc_fence_after();
+                    issue_layer<W>(tm_hid, s_act, s_wh + (uint32_t)(hl - 1) * (uint32_t)(KC * W * 128), W);
+                    umma_commit(bar(BAR_HID));
+                }
+                mbar_wait(bar(BAR_HID), hid_phase); hid_phase ^= 1u;
+                tc_fence_after();
+                drain_relu_to_act<W>(tm_hid + t_row, s_act, (uint32_t)r);
+                tc_fence_before();
+                fence_proxy_async();
+                row_bar_sync();
+            }
+            // output layer (12 heads padded to N = 16) and (a5) decode
+            if (tid == 0) {
+                tc_fence_after();
+                issue_layer<W>(tm_out, s_act, s_wo, TC_NOUT_PAD);
+                umma_commit(bar(BAR_HID));
+            }
+            mbar_wait(bar(BAR_HID), hid_phase); hid_phase ^= 1u;
+            tc_fence_after();
+            uint32_t zr[16];
+            __syncwarp();
+            tmem_ld_32x16(tm_out + t_row, zr);
+            tmem_ld_wait();
+            tc_fence_before();
+            if (cur_ray >= 0) {
+                float z[NIF_N_OUT];
+#pragma unroll
+                for (int a = 0; a < NIF_N_OUT; ++a) z[a] = __uint_as_float(zr[a]);
+                nif_decode_store(z, cur_ti, cur_to, cur_ray, p.out, p.flags);
+            }
+        }
+    } else if (warp == TC_MMA_WARP) {
+        // ======================= layer-1 MMA issuer =============================================
+        if (lane == 0 && n_my > 0) {
+            mbar_wait(bar(BAR_W), 0);
+            const uint32_t idesc = idesc_f16(TC_TILE, W);
+            uint32_t q = 0;
+            for (int j = 0; j < n_my; ++j) {
+                const int b = j & 1;
+                mbar_wait(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
+                tc_fence_after();
+                for (int c = 0; c < n_chunks; ++c, ++q) {
+                    const uint32_t stage = q % TC_STAGES;
+                    mbar_wait(bar(BAR_FULL + stage), (q / TC_STAGES) & 1u);
+                    tc_fence_after();
+                    const uint32_t a0 = s_a + stage * TC_A_CHUNK_BYTES, b0 = s_w1 + (uint32_t)c * (uint32_t)(W * 128);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k)
+                        umma_f16(tm_acc1 + (uint32_t)(b * W), smem_desc_sw128(a0 + (uint32_t)k * 32u),
+                                 smem_desc_sw128(b0 + (uint32_t)k * 32u), idesc, (uint32_t)((c | k) != 0));
+                    umma_commit(bar(BAR_EMPTY + stage));
+                }
+                umma_commit(bar(BAR_ACC_FULL + b));
+            }
+        }
+    } else {
+        // ======================= gather warps: (a3) encode into the A ring ======================
+        const int gw = warp - (TC_MMA_WARP + 1);
+        const int items_per_chunk = 4 * epc;
+        const int items_per_tile = items_per_chunk * n_chunks;
+        const int units_per_es = (L * F) / 8;                          // 16-byte units one sample fills
+        constexpr int LG = 8 / F;
+        for (int j = 0; j < n_my; ++j) {
+            const int b = j & 1;
+            mbar_wait(bar(BAR_RAY_FULL + b), (uint32_t)((j >> 1) & 1));
+            const long long gi0 = (long long)j * items_per_tile;
+            const int first = (int)(((long long)gw - gi0 % TC_GATHER_WARPS + TC_GATHER_WARPS) % TC_GATHER_WARPS);
+            for (int i = first; i < items_per_tile; i += TC_GATHER_WARPS) {
+                const int c = i / items_per_chunk, rem = i - c * items_per_chunk;
+                const int esl = rem >> 2, g = rem & 3;
+                const int es = c * epc + esl;
+                const uint32_t q = (uint32_t)j * (uint32_t)n_chunks + (uint32_t)c;
+                const uint32_t stage = q % TC_STAGES;
+                mbar_wait(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u);
+                const uint32_t row = (uint32_t)(g * 32 + lane);
+                const uint32_t a_stage = s_a + stage * TC_A_CHUNK_BYTES;
+                const uint32_t unit0 = (uint32_t)(esl * units_per_es);
+                if (es < p.n_es) {
+                    const int e = es >= S ? 1 : 0, s = es - e * S;
+                    const float* rb = ray_buf + ((size_t)b * TC_TILE + row) * 8 + 3 * e;
+                    const float px = nif_pe_sample(rb[0], s), py = nif_pe_sample(rb[1], s), pz = nif_pe_sample(rb[2], s);
+                    for (int u = 0; u < units_per_es; ++u) {
+                        uint32_t pk[4];
+                        gather_group<F>(p.table, s_res, p.enc.dense_mask, p.enc.log2_T, u * LG, px, py, pz, pk);
+                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), pk[0], pk[1], pk[2], pk[3]);
+                    }
+                } else {
+                    for (int u = 0; u < units_per_es; ++u)
+                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), 0u, 0u, 0u, 0u);
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(BAR_FULL + stage));
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(BAR_RAY_EMPTY + b));
+        }
+    }
+
+    // ---- teardown --------------------------------------------------------------------------------
+    tc_fence_before();
+    __syncthreads();
+    if (warp == TC_MMA_WARP) { tc_fence_after(); tmem_dealloc(tmem_base, TMEM_COLS); }
+}
+
+// ---- weight repacking: row-major (fan_out, fan_in) fp16 -> K-major SWIZZLE_128B B-operand images ----
+// image of one layer = ceil(K/64) chunks of [n_rows x 128 B]; element (n, k) sits in chunk k/64 at
+// sw128_off(n, (k%64)/8) + (k%8)*2.  Rows/columns beyond the real matrix stay zero.
+__global__ void k_pack_weights(const __half* __restrict__ w, int fan_out, int fan_in, int n_rows,
+                               uint8_t* __restrict__ img)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= fan_out * fan_in) return;
+    const int n = i / fan_in, k = i - n * fan_in;
+    const uint32_t off = (uint32_t)(k / 64) * (uint32_t)(n_rows * 128) + sw128_off((uint32_t)n, (uint32_t)((k % 64) / 8)) +
+                         (uint32_t)(k % 8) * 2u;
+    *reinterpret_cast<__half*>(img + off) = w[i];
+}
+
+struct TcShape {
+    int S, n_es, lf, epc, n_chunks, KC;
+    uint32_t w1_bytes, wh_bytes, wo_bytes, w_bytes;
+};
+TcShape tc_shape(const nif_net_desc* d)
+{
+    TcShape s{};
+    s.S = 1 + 2 * d->pe_bands; s.n_es = 2 * s.S; s.lf = d->levels * d->feat;
+    s.epc = s.lf > 0 && s.lf <= 64 ? 64 / s.lf : 0;
+    s.n_chunks = s.epc ? (s.n_es + s.epc - 1) / s.epc : 0;
+    s.KC = (d->width + 63) / 64;
+    s.w1_bytes = (uint32_t)s.n_chunks * (uint32_t)d->width * 128u;
+    s.wh_bytes = (uint32_t)(d->hidden_layers - 1) * (uint32_t)s.KC * (uint32_t)d->width * 128u;
+    s.wo_bytes = (uint32_t)s.KC * TC_NOUT_PAD * 128u;
+    s.w_bytes = s.w1_bytes + s.wh_bytes + s.wo_bytes;
+    return s;
+}
+
+constexpr uint32_t TC_MAX_SMEM = 227u * 1024u;
+
+template <int W, int F>
+int launch_tc(const TcParams& p, uint32_t smem, int blocks, cudaStream_t stream)
+{
+    NIF_CUDA_TRY(cudaFuncSetAttribute(k_fused_encode_mlp<W, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_fused_encode_mlp<W, F><<<blocks, TC_THREADS, smem, stream>>>(p);
+    nif_count_launch(1);
+    NIF_CUDA_TRY(cudaGetLastError());
+    return NIF_OK;
+}
+
+}  // namespace
+
+int nif_tc_supported(const nif_net_desc* d)
+{
+    if (d->dtype != NIF_F16) return 0;
+    if (d->feat != 2 && d->feat != 4) return 0;
+    if (d->width != 32 && d->width != 64 && d->width != 128) return 0;
+    const int lf = d->levels * d->feat;
+    if (lf != 8 && lf != 16 && lf != 32 && lf != 64) return 0;
+    if (d->hidden_layers < 1) return 0;
+    const TcShape s = tc_shape(d);
+    return tc_smem_layout(s.w_bytes, d->width).total <= TC_MAX_SMEM ? 1 : 0;
+}
+
+int nif_tc_pack_weights(nif_net* net, cudaStream_t stream)
+{
+    const nif_net_desc* d = &net->desc;
+    const TcShape s = tc_shape(d);
+    net->w_tc_bytes = s.w_bytes;
+    NIF_CUDA_TRY(cudaMalloc(&net->w_tc, s.w_bytes));
+    NIF_CUDA_TRY(cudaMemsetAsync(net->w_tc, 0, s.w_bytes, stream));
+    uint8_t* img = (uint8_t*)net->w_tc;
+    size_t off = 0;
+    for (int i = 0; i <= d->hidden_layers; ++i) {
+        const int fan_out = i == d->hidden_layers ? NIF_N_OUT : d->width;
+        const int fan_in = i == 0 ? net->d_in : d->width;
+        const int n_rows = i == d->hidden_layers ? TC_NOUT_PAD : d->width;
+        net->w_tc_layer_off[i] = off;
+        const int total = fan_out * fan_in;
+        k_pack_weights<<<(total + 255) / 256, 256, 0, stream>>>((const __half*)net->w_plain[i], fan_out, fan_in, n_rows, img + off);
+        nif_count_launch(1);
+        off += i == 0 ? s.w1_bytes : (size_t)s.KC * n_rows * 128;
+    }
+    NIF_CUDA_TRY(cudaGetLastError());
+    return NIF_OK;
+}
+
+int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays, const nif_query_out* out,
+                        NifQueryScratch* scratch, const int32_t* hit_list, unsigned flags, cudaStream_t stream)
+{
+    if (rays->n == 0) return NIF_OK;
+    const nif_net_desc* d = &net->desc;
+    const TcShape s = tc_shape(d);
+    TcParams p;
+    p.enc = net->enc;
+    p.hidden_layers = d->hidden_layers;
+    p.n_chunks = s.n_chunks; p.es_per_chunk = s.epc; p.n_es = s.n_es;
+    p.table = (const __half*)net->table;
+    p.w_img = (const uint8_t*)net->w_tc; p.w_bytes = s.w_bytes;
+    p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
+    p.origin = rays->origin; p.dir = rays->dir;
+    p.out = *out; p.scratch = scratch; p.hit_list = hit_list; p.flags = flags;
+    const uint32_t smem = tc_smem_layout(s.w_bytes, d->width).total;
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        NIF_CUDA_TRY(cudaGetDevice(&dev));
+        NIF_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    const long long max_tiles = (rays->n + TC_TILE - 1) / TC_TILE;
+    const int blocks = (int)(max_tiles < n_sm ? max_tiles : n_sm);
+#define NIF_TC_CASE(WW, FF) if (d->width == WW && d->feat == FF) return launch_tc<WW, FF>(p, smem, blocks, stream)
+    NIF_TC_CASE(32, 2); NIF_TC_CASE(64, 2); NIF_TC_CASE(128, 2);
+    NIF_TC_CASE(32, 4); NIF_TC_CASE(64, 4); NIF_TC_CASE(128, 4);
+#undef NIF_TC_CASE
+    return NIF_ERR_UNSUPPORTED;
+}
