@@ -42,7 +42,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         obj = objdir / (name + ".o")
         objs.append(obj)
         if force or _stale(obj, src):
-            cmd = [_nvcc(), *NVCC_FLAGS, "-I", str(INCLUDE), "-I", str(CSRC), "-c", str(src), "-o", str(obj)]
+            cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("NIF_NVCC_EXTRA", "").split(), "-I", str(INCLUDE), "-I", str(CSRC), "-c", str(src), "-o", str(obj)]
             if verbose:
                 cmd.insert(1, "-Xptxas=-v")
             procs.append((name, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))

@@ -18,11 +18,16 @@
 // t+1 overlap the MLP tail of tile t.
 #include "nif_encode.cuh"
 
+#include <type_traits>
+
 namespace {
 
 constexpr int TC_TILE = 128;                 // rays per tile = UMMA M
 constexpr int TC_ROW_WARPS = 4;
-constexpr int TC_GATHER_WARPS = 16;
+#ifndef NIF_TC_GATHER_WARPS
+#define NIF_TC_GATHER_WARPS 16
+#endif
+constexpr int TC_GATHER_WARPS = NIF_TC_GATHER_WARPS;
 constexpr int TC_MMA_WARP = TC_ROW_WARPS;    // warp index 4
 constexpr int TC_THREADS = 32 * (TC_ROW_WARPS + 1 + TC_GATHER_WARPS);
 constexpr int TC_STAGES = 4;                 // A-operand ring depth (K chunks of 64 columns)
@@ -187,90 +192,88 @@ enum { BAR_FULL = 0, BAR_EMPTY = TC_STAGES, BAR_ACC_FULL = 2 * TC_STAGES, BAR_AC
        BAR_RAY_FULL = BAR_ACC_EMPTY + 2, BAR_RAY_EMPTY = BAR_RAY_FULL + 2, BAR_HID = BAR_RAY_EMPTY + 2,
        BAR_W = BAR_HID + 1, BAR_COUNT = BAR_W + 1 };
 
-// ---- (a3) one group of levels of one sample: LG * F = 8 features = 16 bytes of the A row ----------
-// Index rule and corner order as nif_level_features (R6); all LG*8 gathers are issued
-// before any is consumed.
+// ---- (a3) gathers of one sample, software-pipelined in batches of 8/F levels (16 loads of 4 B for
+// F = 2, 8 loads of 8 B for F = 4).  issue() computes the 8 table indices of each level of the batch
+// (index rule and corner order of nif_level_features, R6) and issues the loads; consume()
+// interpolates in fp32 and returns the batch's 4 features as two packed half2.  Two batches are in
+// flight per thread: the next batch's loads are issued before the current one is consumed.
+struct TcLevel {            // per-level constants, staged in shared memory (one LDS.128 per level)
+    float fn, top;          // N, N-1
+    uint32_t np1;           // N+1 for a dense level, 0 for a hashed one
+    uint32_t pad;
+};
+
 template <int F>
-__device__ __forceinline__ void gather_group(const __half* __restrict__ table, const int* __restrict__ s_res,
-                                             uint32_t dense_mask, int log2_T, int l0,
-                                             float px, float py, float pz, uint32_t packed[4])
-{
-    constexpr int LG = 8 / F;                                 // levels per 16-byte unit
-    const uint32_t t_mask = (1u << log2_T) - 1u;
-    uint32_t idx[LG][8];
-    float wx[LG], wy[LG], wz[LG];
+struct GatherBatch {
+    static constexpr int NL = 4 / F;                          // levels per batch
+    typedef typename std::conditional<F == 2, uint32_t, uint2>::type raw_t;
+    raw_t raw[NL][8];
+    float wx[NL], wy[NL], wz[NL];
+
+    __device__ __forceinline__ void issue(const __half* __restrict__ table, const TcLevel* __restrict__ s_lvl,
+                                          int log2_T, int l0, float px, float py, float pz)
+    {
+        const uint32_t t_mask = (1u << log2_T) - 1u;
 #pragma unroll
-    for (int li = 0; li < LG; ++li) {
-        const int l = l0 + li;
-        const int N = s_res[l];
-        const float fn = (float)N, top = (float)(N - 1);
-        const float posx = px * fn, posy = py * fn, posz = pz * fn;
-        const float flx = fmaxf(fminf(floorf(posx), top), 0.0f);
-        const float fly = fmaxf(fminf(floorf(posy), top), 0.0f);
-        const float flz = fmaxf(fminf(floorf(posz), top), 0.0f);
-        wx[li] = posx - flx; wy[li] = posy - fly; wz[li] = posz - flz;
-        const uint32_t cx = (uint32_t)flx, cy = (uint32_t)fly, cz = (uint32_t)flz;
-        if ((dense_mask >> l) & 1u) {
-            const uint32_t np1 = (uint32_t)N + 1u;
-            const uint32_t b = cx + np1 * (cy + np1 * cz);
+        for (int li = 0; li < NL; ++li) {
+            const int l = l0 + li;
+            const float4 lv = *reinterpret_cast<const float4*>(s_lvl + l);
+            const uint32_t np1 = __float_as_uint(lv.z);
+            const float posx = px * lv.x, posy = py * lv.x, posz = pz * lv.x;     // p in [0,1]: floor >= 0
+            const float flx = fminf(floorf(posx), lv.y), fly = fminf(floorf(posy), lv.y), flz = fminf(floorf(posz), lv.y);
+            wx[li] = posx - flx; wy[li] = posy - fly; wz[li] = posz - flz;
+            const uint32_t cx = (uint32_t)flx, cy = (uint32_t)fly, cz = (uint32_t)flz;
+            uint32_t idx[8];
+            if (np1) {
+                const uint32_t o2 = np1 * np1;
+                const uint32_t b = cx + np1 * cy + o2 * cz;
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
-                idx[li][c] = b + (uint32_t)(c & 1) + np1 * ((uint32_t)((c >> 1) & 1) + np1 * (uint32_t)(c >> 2));
-        } else {
-            const uint32_t hy0 = cy * 2654435761u, hy1 = hy0 + 2654435761u;
-            const uint32_t hz0 = cz * 805459861u, hz1 = hz0 + 805459861u;
+                for (int c = 0; c < 8; ++c)
+                    idx[c] = b + (uint32_t)(c & 1) + (((c >> 1) & 1) ? np1 : 0u) + ((c >> 2) ? o2 : 0u);
+            } else {
+                const uint32_t hy0 = cy * 2654435761u, hy1 = hy0 + 2654435761u;
+                const uint32_t hz0 = cz * 805459861u, hz1 = hz0 + 805459861u;
+                const uint32_t hyz[4] = {hy0 ^ hz0, hy1 ^ hz0, hy0 ^ hz1, hy1 ^ hz1};
+                const uint32_t cx1 = cx + 1u;
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
-                idx[li][c] = ((cx + (uint32_t)(c & 1)) ^ (((c >> 1) & 1) ? hy1 : hy0) ^ ((c >> 2) ? hz1 : hz0)) & t_mask;
+                for (int c = 0; c < 8; ++c) idx[c] = (((c & 1) ? cx1 : cx) ^ hyz[c >> 1]) & t_mask;
+            }
+            const raw_t* lvl = reinterpret_cast<const raw_t*>(table) + ((size_t)l << log2_T);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(lvl + idx[c]);
         }
     }
-    float feat[LG][F];
-    if constexpr (F == 2) {
-        uint32_t raw[LG][8];
+
+    __device__ __forceinline__ void consume(uint32_t& p0, uint32_t& p1) const
+    {
+        float f[4];
 #pragma unroll
-        for (int li = 0; li < LG; ++li) {
-            const uint32_t* lvl = reinterpret_cast<const uint32_t*>(table) + ((size_t)(l0 + li) << log2_T);
+        for (int li = 0; li < NL; ++li) {
+            const float x1 = wx[li], x0 = 1.0f - x1, y1 = wy[li], y0 = 1.0f - y1, z1 = wz[li], z0 = 1.0f - z1;
+            const float xy[4] = {x0 * y0, x1 * y0, x0 * y1, x1 * y1};
+            float acc[F];
 #pragma unroll
-            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(lvl + idx[li][c]);
-        }
-#pragma unroll
-        for (int li = 0; li < LG; ++li) {
-            float f0 = 0.0f, f1 = 0.0f;
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const float w = (((c & 1) ? wx[li] : 1.0f - wx[li]) * (((c >> 1) & 1) ? wy[li] : 1.0f - wy[li])) *
-                                ((c >> 2) ? wz[li] : 1.0f - wz[li]);
-                const float2 v = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c]));
-                f0 = fmaf(w, v.x, f0); f1 = fmaf(w, v.y, f1);
-            }
-            feat[li][0] = f0; feat[li][1] = f1;
-        }
-    } else {
-        uint2 raw[LG][8];
-#pragma unroll
-        for (int li = 0; li < LG; ++li) {
-            const uint2* lvl = reinterpret_cast<const uint2*>(table) + ((size_t)(l0 + li) << log2_T);
-#pragma unroll
-            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(lvl + idx[li][c]);
-        }
-#pragma unroll
-        for (int li = 0; li < LG; ++li) {
-            float f0 = 0.0f, f1 = 0.0f, f2 = 0.0f, f3 = 0.0f;
+            for (int k = 0; k < F; ++k) acc[k] = 0.0f;
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
-                const float w = (((c & 1) ? wx[li] : 1.0f - wx[li]) * (((c >> 1) & 1) ? wy[li] : 1.0f - wy[li])) *
-                                ((c >> 2) ? wz[li] : 1.0f - wz[li]);
-                const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c].x));
-                const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c].y));
-                f0 = fmaf(w, a.x, f0); f1 = fmaf(w, a.y, f1); f2 = fmaf(w, b.x, f2); f3 = fmaf(w, b.y, f3);
+                const float w = xy[c & 3] * ((c >> 2) ? z1 : z0);
+                if constexpr (F == 2) {
+                    const float2 v = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c]));
+                    acc[0] = fmaf(w, v.x, acc[0]); acc[1] = fmaf(w, v.y, acc[1]);
+                } else {
+                    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c].x));
+                    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&raw[li][c].y));
+                    acc[0] = fmaf(w, a.x, acc[0]); acc[1] = fmaf(w, a.y, acc[1]);
+                    acc[2] = fmaf(w, b.x, acc[2]); acc[3] = fmaf(w, b.y, acc[3]);
+                }
             }
-            feat[li][0] = f0; feat[li][1] = f1; feat[li][2] = f2; feat[li][3] = f3;
+#pragma unroll
+            for (int k = 0; k < F; ++k) f[li * F + k] = acc[k];
         }
+        p0 = pack_half2(f[0], f[1]);
+        p1 = pack_half2(f[2], f[3]);
     }
-    const float* ff = &feat[0][0];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) packed[i] = pack_half2(ff[2 * i], ff[2 * i + 1]);
-}
+};
 
 // drains W fp32 accumulator columns of this thread's row from TMEM, applies ReLU, rounds to fp16
 // and writes them as the next layer's A operand (K-major SWIZZLE_128B, chunks of 64 columns)
@@ -325,7 +328,7 @@ k_fused_encode_mlp(const TcParams p)
     float* ray_buf = reinterpret_cast<float*>(smem_gen + SL.ray_buf);          // [2][128][8]
     const uint32_t s_bar = smem_base + SL.bars;
     uint32_t* s_tmem_ptr = reinterpret_cast<uint32_t*>(smem_gen + SL.bars + 8 * BAR_COUNT);
-    int* s_res = reinterpret_cast<int*>(smem_gen + SL.bars + 8 * BAR_COUNT + 16);
+    TcLevel* s_lvl = reinterpret_cast<TcLevel*>(smem_gen + SL.bars + 8 * BAR_COUNT + 16);
     auto bar = [&](int i) { return s_bar + 8u * (uint32_t)i; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -344,7 +347,13 @@ k_fused_encode_mlp(const TcParams p)
         mbar_init(bar(BAR_HID), 1); mbar_init(bar(BAR_W), 1);
         fence_barrier_init();
     }
-    if (tid < NIF_MAX_LEVELS) s_res[tid] = tid < L ? p.enc.res[tid] : 1;
+    if (tid < NIF_MAX_LEVELS) {
+        const int N = tid < L ? p.enc.res[tid] : 1;
+        TcLevel lv;
+        lv.fn = (float)N; lv.top = (float)(N - 1);
+        lv.np1 = ((p.enc.dense_mask >> tid) & 1u) ? (uint32_t)N + 1u : 0u; lv.pad = 0u;
+        s_lvl[tid] = lv;
+    }
     if (warp == TC_MMA_WARP) tmem_alloc(smem_u32(s_tmem_ptr), TMEM_COLS);
     tc_fence_before();
     __syncthreads();
@@ -472,7 +481,6 @@ k_fused_encode_mlp(const TcParams p)
         const int items_per_chunk = 4 * epc;
         const int items_per_tile = items_per_chunk * n_chunks;
         const int units_per_es = (L * F) / 8;                          // 16-byte units one sample fills
-        constexpr int LG = 8 / F;
         for (int j = 0; j < n_my; ++j) {
             const int b = j & 1;
             mbar_wait(bar(BAR_RAY_FULL + b), (uint32_t)((j >> 1) & 1));
@@ -492,9 +500,15 @@ k_fused_encode_mlp(const TcParams p)
                     const int e = es >= S ? 1 : 0, s = es - e * S;
                     const float* rb = ray_buf + ((size_t)b * TC_TILE + row) * 8 + 3 * e;
                     const float px = nif_pe_sample(rb[0], s), py = nif_pe_sample(rb[1], s), pz = nif_pe_sample(rb[2], s);
+                    GatherBatch<F> ba, bb;                                     // two batches in flight
+                    constexpr int NL = GatherBatch<F>::NL;
+                    ba.issue(p.table, s_lvl, p.enc.log2_T, 0, px, py, pz);
                     for (int u = 0; u < units_per_es; ++u) {
                         uint32_t pk[4];
-                        gather_group<F>(p.table, s_res, p.enc.dense_mask, p.enc.log2_T, u * LG, px, py, pz, pk);
+                        bb.issue(p.table, s_lvl, p.enc.log2_T, (2 * u + 1) * NL, px, py, pz);
+                        ba.consume(pk[0], pk[1]);
+                        if (u + 1 < units_per_es) ba.issue(p.table, s_lvl, p.enc.log2_T, (2 * u + 2) * NL, px, py, pz);
+                        bb.consume(pk[2], pk[3]);
                         st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), pk[0], pk[1], pk[2], pk[3]);
                     }
                 } else {
