@@ -202,9 +202,11 @@ int nif_profile_read(double* traverse_ms, double* network_ms, int64_t* n_queries
 /* Random-sector gather probe: the denominator of the gather roofline.
  * All SMs issue independent 4-byte loads at pseudo-random 32-byte sectors of the DEVICE buffer
  * `buf` (`bytes` rounded down to a power-of-two number of sectors); `iters` batches of 8 loads
- * per thread, 4 x 512 threads per SM.  Returns the best of 3 timed launches as 32-byte sectors
+ * per thread, 512-thread blocks.  `smem_bytes` of (untouched) dynamic shared memory per block
+ * shrink the L1 data cache to what a kernel with that footprint is left with (4 blocks per SM, 2
+ * above 56 KiB, 1 above 113 KiB).  Returns the best of 3 timed launches as 32-byte sectors
  * per second (and its milliseconds in *ms, optional).  SYNCHRONISES. */
-int nif_probe_gather(const void* buf, size_t bytes, int iters, void* stream,
+int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t smem_bytes, void* stream,
                      double* sectors_per_s, double* ms);
 
 /* Kernels launched by the library since load (every nif_* call adds its launches). */

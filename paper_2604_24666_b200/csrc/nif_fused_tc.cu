@@ -29,8 +29,12 @@ constexpr int TC_ROW_WARPS = 4;
 #endif
 constexpr int TC_GATHER_WARPS = NIF_TC_GATHER_WARPS;
 constexpr int TC_MMA_WARP = TC_ROW_WARPS;    // warp index 4
-constexpr int TC_THREADS = 32 * (TC_ROW_WARPS + 1 + TC_GATHER_WARPS);
-constexpr int TC_STAGES = 4;                 // A-operand ring depth (K chunks of 64 columns)
+constexpr int TC_TMA_WARP = TC_ROW_WARPS + 1;  // warp index 5: streams the layer-1 weight chunks
+constexpr int TC_THREADS = 32 * (TC_ROW_WARPS + 2 + TC_GATHER_WARPS);
+#ifndef NIF_TC_STAGES
+#define NIF_TC_STAGES 4
+#endif
+constexpr int TC_STAGES = NIF_TC_STAGES;     // ring depth; one stage = A chunk (128 x 64) + W1 chunk (W x 64)
 constexpr int TC_A_CHUNK_BYTES = TC_TILE * 128;
 constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded to the UMMA minimum)
 
@@ -162,7 +166,7 @@ struct TcParams {
     int n_es;                     // 2 S
     const __half* table;
     const uint8_t* w_img;         // B-operand images: W1 chunks | hidden layers 2..H | output layer
-    uint32_t w_bytes;
+    uint32_t w_bytes, w1_bytes;
     float theta_max, bend_k;
     const float* origin;
     const float* dir;
@@ -175,12 +179,12 @@ struct TcParams {
 struct TcSmemLayout {
     uint32_t w_img, a_ring, act, ray_buf, bars, total;
 };
-__host__ __device__ inline TcSmemLayout tc_smem_layout(uint32_t w_bytes, int W)
+__host__ __device__ inline TcSmemLayout tc_smem_layout(uint32_t w_res_bytes, int W)
 {
     TcSmemLayout L;
     uint32_t off = 0;
-    L.w_img = off;   off += (w_bytes + 1023u) & ~1023u;
-    L.a_ring = off;  off += TC_STAGES * TC_A_CHUNK_BYTES;
+    L.w_img = off;   off += (w_res_bytes + 1023u) & ~1023u;          // resident: hidden + output layers
+    L.a_ring = off;  off += TC_STAGES * (TC_A_CHUNK_BYTES + (uint32_t)W * 128u);   // stage = A chunk | W1 chunk
     L.act = off;     off += (uint32_t)((W + 63) / 64) * TC_A_CHUNK_BYTES;
     L.ray_buf = off; off += 2u * TC_TILE * 8u * sizeof(float);
     L.bars = off;    off += 512;
@@ -323,7 +327,8 @@ k_fused_encode_mlp(const TcParams p)
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    const TcSmemLayout SL = tc_smem_layout(p.w_bytes, W);
+    const TcSmemLayout SL = tc_smem_layout(p.w_bytes - p.w1_bytes, W);
+    constexpr uint32_t STAGE_BYTES = TC_A_CHUNK_BYTES + (uint32_t)W * 128u;
     const uint32_t s_w = smem_base + SL.w_img, s_a = smem_base + SL.a_ring, s_act = smem_base + SL.act;
     float* ray_buf = reinterpret_cast<float*>(smem_gen + SL.ray_buf);          // [2][128][8]
     const uint32_t s_bar = smem_base + SL.bars;
@@ -339,7 +344,7 @@ k_fused_encode_mlp(const TcParams p)
 
     // ---- one-time setup ------------------------------------------------------------------------
     if (tid == 0) {
-        for (int i = 0; i < TC_STAGES; ++i) { mbar_init(bar(BAR_FULL + i), 4u * (uint32_t)epc); mbar_init(bar(BAR_EMPTY + i), 1); }
+        for (int i = 0; i < TC_STAGES; ++i) { mbar_init(bar(BAR_FULL + i), 4u * (uint32_t)epc + 1u); mbar_init(bar(BAR_EMPTY + i), 1); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar(BAR_ACC_FULL + i), 1); mbar_init(bar(BAR_ACC_EMPTY + i), TC_TILE);
             mbar_init(bar(BAR_RAY_FULL + i), TC_TILE); mbar_init(bar(BAR_RAY_EMPTY + i), TC_GATHER_WARPS);
@@ -367,14 +372,14 @@ k_fused_encode_mlp(const TcParams p)
 
     // weight images -> shared memory, once (TMA bulk copies, completion on BAR_W)
     if (warp == TC_MMA_WARP && lane == 0 && n_my > 0) {
-        mbar_expect_tx(bar(BAR_W), p.w_bytes);
-        for (uint32_t off = 0; off < p.w_bytes; off += 16384u) {
-            const uint32_t n = p.w_bytes - off < 16384u ? p.w_bytes - off : 16384u;
-            bulk_g2s(s_w + off, p.w_img + off, n, bar(BAR_W));
+        const uint32_t res_bytes = p.w_bytes - p.w1_bytes;
+        mbar_expect_tx(bar(BAR_W), res_bytes);
+        for (uint32_t off = 0; off < res_bytes; off += 16384u) {
+            const uint32_t n = res_bytes - off < 16384u ? res_bytes - off : 16384u;
+            bulk_g2s(s_w + off, p.w_img + p.w1_bytes + off, n, bar(BAR_W));
         }
     }
-    const uint32_t s_w1 = s_w;
-    const uint32_t s_wh = s_w + (uint32_t)n_chunks * (uint32_t)(W * 128);
+    const uint32_t s_wh = s_w;
     const uint32_t s_wo = s_wh + (uint32_t)(p.hidden_layers - 1) * (uint32_t)(KC * W * 128);
 
     if (warp < TC_ROW_WARPS) {
@@ -465,7 +470,7 @@ k_fused_encode_mlp(const TcParams p)
                     const uint32_t stage = q % TC_STAGES;
                     mbar_wait(bar(BAR_FULL + stage), (q / TC_STAGES) & 1u);
                     tc_fence_after();
-                    const uint32_t a0 = s_a + stage * TC_A_CHUNK_BYTES, b0 = s_w1 + (uint32_t)c * (uint32_t)(W * 128);
+                    const uint32_t a0 = s_a + stage * STAGE_BYTES, b0 = a0 + TC_A_CHUNK_BYTES;
 #pragma unroll
                     for (int k = 0; k < 4; ++k)
                         umma_f16(tm_acc1 + (uint32_t)(b * W), smem_desc_sw128(a0 + (uint32_t)k * 32u),
@@ -475,9 +480,25 @@ k_fused_encode_mlp(const TcParams p)
                 umma_commit(bar(BAR_ACC_FULL + b));
             }
         }
+    } else if (warp == TC_TMA_WARP) {
+        // ======================= layer-1 weight chunks: L2 -> ring stage (cp.async.bulk) ========
+        // W1 (D_in x W fp16) does not stay in shared memory: a small footprint leaves the L1 data
+        // cache large enough to keep the gathers' misses in flight.
+        if (lane == 0) {
+            constexpr uint32_t W1_CHUNK = (uint32_t)W * 128u;
+            uint32_t q = 0;
+            for (int j = 0; j < n_my; ++j)
+                for (int c = 0; c < n_chunks; ++c, ++q) {
+                    const uint32_t stage = q % TC_STAGES;
+                    mbar_wait(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u);
+                    mbar_expect_tx(bar(BAR_FULL + stage), W1_CHUNK);
+                    bulk_g2s(s_a + stage * STAGE_BYTES + TC_A_CHUNK_BYTES, p.w_img + (size_t)c * W1_CHUNK, W1_CHUNK,
+                             bar(BAR_FULL + stage));
+                }
+        }
     } else {
         // ======================= gather warps: (a3) encode into the A ring ======================
-        const int gw = warp - (TC_MMA_WARP + 1);
+        const int gw = warp - (TC_TMA_WARP + 1);
         const int items_per_chunk = 4 * epc;
         const int items_per_tile = items_per_chunk * n_chunks;
         const int units_per_es = (L * F) / 8;                          // 16-byte units one sample fills
@@ -494,7 +515,7 @@ k_fused_encode_mlp(const TcParams p)
                 const uint32_t stage = q % TC_STAGES;
                 mbar_wait(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u);
                 const uint32_t row = (uint32_t)(g * 32 + lane);
-                const uint32_t a_stage = s_a + stage * TC_A_CHUNK_BYTES;
+                const uint32_t a_stage = s_a + stage * STAGE_BYTES;
                 const uint32_t unit0 = (uint32_t)(esl * units_per_es);
                 if (es < p.n_es) {
                     const int e = es >= S ? 1 : 0, s = es - e * S;
@@ -585,7 +606,7 @@ int nif_tc_supported(const nif_net_desc* d)
     if (lf != 8 && lf != 16 && lf != 32 && lf != 64) return 0;
     if (d->hidden_layers < 1) return 0;
     const TcShape s = tc_shape(d);
-    return tc_smem_layout(s.w_bytes, d->width).total <= TC_MAX_SMEM ? 1 : 0;
+    return tc_smem_layout(s.w_bytes - s.w1_bytes, d->width).total <= TC_MAX_SMEM ? 1 : 0;
 }
 
 int nif_tc_pack_weights(nif_net* net, cudaStream_t stream)
@@ -622,11 +643,11 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     p.hidden_layers = d->hidden_layers;
     p.n_chunks = s.n_chunks; p.es_per_chunk = s.epc; p.n_es = s.n_es;
     p.table = (const __half*)net->table;
-    p.w_img = (const uint8_t*)net->w_tc; p.w_bytes = s.w_bytes;
+    p.w_img = (const uint8_t*)net->w_tc; p.w_bytes = s.w_bytes; p.w1_bytes = s.w1_bytes;
     p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
     p.origin = rays->origin; p.dir = rays->dir;
     p.out = *out; p.scratch = scratch; p.hit_list = hit_list; p.flags = flags;
-    const uint32_t smem = tc_smem_layout(s.w_bytes, d->width).total;
+    const uint32_t smem = tc_smem_layout(s.w_bytes - s.w1_bytes, d->width).total;
     static int n_sm = 0;
     if (!n_sm) {
         int dev = 0;

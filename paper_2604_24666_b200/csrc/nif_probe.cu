@@ -114,9 +114,10 @@ k_probe_gather(const uint32_t* __restrict__ buf, uint32_t sector_mask, int iters
 
 }  // namespace
 
-extern "C" int nif_probe_gather(const void* buf, size_t bytes, int iters, void* stream_,
+extern "C" int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t smem_bytes, void* stream_,
                                 double* sectors_per_s, double* ms)
 {
+    if (smem_bytes > 227u * 1024u) return NIF_ERR_INVALID_ARG;
     if (!buf || !sectors_per_s || iters < 1 || bytes < 4096) return NIF_ERR_INVALID_ARG;
     if (!nif_device_supported()) return NIF_ERR_UNSUPPORTED;
     cudaStream_t stream = (cudaStream_t)stream_;
@@ -129,11 +130,15 @@ extern "C" int nif_probe_gather(const void* buf, size_t bytes, int iters, void* 
     NIF_CUDA_TRY(cudaEventCreate(&e1));
     int sms = 148;
     (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
-    const int blocks = sms * 4, threads = 512;
+    // dynamic shared memory the probe does not touch: it only shrinks the L1 data cache to what a
+    // kernel with that much shared memory is left with (one block per SM above ~113 KB)
+    NIF_CUDA_TRY(cudaFuncSetAttribute(k_probe_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+    const int per_sm = smem_bytes > 113u * 1024u ? 1 : (smem_bytes > 56u * 1024u ? 2 : 4);
+    const int blocks = sms * per_sm, threads = 512;
     double best = 1e30;
     for (int rep = 0; rep < 4; ++rep) {                            // rep 0 warms L2 with the buffer
         NIF_CUDA_TRY(cudaEventRecord(e0, stream));
-        k_probe_gather<<<blocks, threads, 0, stream>>>((const uint32_t*)buf, (uint32_t)(n_sectors - 1), iters, sink);
+        k_probe_gather<<<blocks, threads, smem_bytes, stream>>>((const uint32_t*)buf, (uint32_t)(n_sectors - 1), iters, sink);
         NIF_CUDA_TRY(cudaEventRecord(e1, stream));
         NIF_CUDA_TRY(cudaEventSynchronize(e1));
         nif_count_launch(1);
