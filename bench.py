@@ -337,6 +337,8 @@ def run_ours(args) -> None:
                 "peak_source": "measured live: nif_probe_gather, random 32 B sectors over a 32 MiB buffer, all SMs",
                 "algorithmic": f"{work['gathers_per_hit_ray']} gathers x 32 B sector per hit ray x "
                                f"{hits_per_launch:.0f} hit rays per launch",
+                "frac_note": "per-lane gathers counted as one 32 B sector each (SURVEY 8(d).2 worst case); coherent "
+                             "rays share sectors and lines, so frac can exceed 1 -- see profiles/ for the sectors ncu counted",
                 "avg_launch_ms": net_ms, "share_of_step": net_ms * cfg.n_poses / ms_per_step,
                 "tensor": {"bound": "tensor", "achieved": tensor_tfs, "peak": peaks["tf_sustained"],
                            "unit": "TFLOP/s", "frac": tensor_tfs / peaks["tf_sustained"],
