@@ -1,0 +1,77 @@
+"""Host logic of the N>1 path on CPU (gloo, world_size 2): rays are independent, so ranks take
+disjoint contiguous ray ranges (nif_inputs.shard_range) with no data-path collective; only the
+timing reduction (max over ranks) and an optional gather of per-rank results go through
+torch.distributed.  The per-rank "query" here is the CPU oracle's traversal -- this test checks
+the sharding arithmetic and the rendezvous/reduction code, not a kernel."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+import nif_inputs as I
+
+
+def test_shard_range_partitions_exactly():
+    for n in (0, 1, 7, 128, 1000, 2_073_600):
+        for world in (1, 2, 3, 8):
+            spans = [I.shard_range(n, r, world) for r in range(world)]
+            assert spans[0][0] == 0 and spans[-1][1] == n
+            for (a0, a1), (b0, b1) in zip(spans, spans[1:]):
+                assert a1 == b0 and a0 <= a1
+            sizes = [b - a for a, b in spans]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank: int, world: int, port: int, n: int, out_dir: str):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle import Oracle
+        cfg = I.get_config(0)
+        orc = Oracle()
+        occ = I.occupancy(cfg)
+        pose = I.poses(cfg)[0]
+        lat = orc.deform_lattice(cfg.nv, float(pose[0]), float(pose[1]))
+        bvh = orc.bvh_build(cfg.nv, occ, lat)
+        o, d = I.rays(cfg, 0, n=n)
+        b, e = I.shard_range(n, rank, world)
+        vid, ti, to = bvh.traverse(o[b:e], d[b:e])
+        # what bench.py does with its device time: max over ranks
+        t = torch.tensor([float(rank + 1)], dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        hits = torch.tensor([int((vid >= 0).sum())], dtype=torch.int64)
+        dist.all_reduce(hits, op=dist.ReduceOp.SUM)
+        gathered = [None] * world
+        dist.all_gather_object(gathered, (b, e, vid))
+        if rank == 0:
+            full = np.concatenate([g[2] for g in sorted(gathered, key=lambda g: g[0])])
+            np.save(os.path.join(out_dir, "vid.npy"), full)
+            np.save(os.path.join(out_dir, "meta.npy"), np.array([t.item(), hits.item()]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+def test_two_ranks_shard_rays_without_exchange(tmp_path, oracle):
+    n, world = 1001, 2                                   # odd count: ragged shards
+    mp.spawn(_worker, args=(world, _free_port(), n, str(tmp_path)), nprocs=world, join=True)
+    cfg = I.get_config(0)
+    occ = I.occupancy(cfg)
+    pose = I.poses(cfg)[0]
+    lat = oracle.deform_lattice(cfg.nv, float(pose[0]), float(pose[1]))
+    o, d = I.rays(cfg, 0, n=n)
+    vid, _, _ = oracle.bvh_build(cfg.nv, occ, lat).traverse(o, d)
+    got = np.load(tmp_path / "vid.npy")
+    t_max, hits = np.load(tmp_path / "meta.npy")
+    assert np.array_equal(got, vid)                      # sharded == single rank, ray for ray
+    assert t_max == world and hits == int((vid >= 0).sum())
