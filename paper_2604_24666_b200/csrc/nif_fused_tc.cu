@@ -8,14 +8,18 @@
 //               endpoints (a2), then drain the layer-1 accumulator from TMEM (tcgen05.ld), run the
 //               hidden and output layers (ReLU -> fp16 -> swizzled smem A operand -> tcgen05.mma,
 //               issued by thread 0) and decode/store the heads (a5).
-//   warp 4      allocates TMEM; one lane issues the layer-1 MMAs chunk by chunk as the gather warps
-//               fill the A-operand ring (full/empty mbarriers), commits to the accumulator barrier.
-//   warps 5..   gather warps: lane = ray, one work item = (32-ray group, endpoint, PE sample); the
-//               L levels of that sample are interpolated (8 table gathers each, fp32) and written as
-//               fp16 into the canonical K-major SWIZZLE_128B A tile, 16 bytes per store.
-// Weights sit in shared memory for the whole kernel as pre-swizzled B-operand images, loaded once
-// with cp.async.bulk.  The layer-1 accumulator is double-buffered in TMEM so the gathers of tile
-// t+1 overlap the MLP tail of tile t.
+//   warp 4      allocates TMEM; one lane issues the layer-1 MMAs chunk by chunk as ring stages fill
+//               (full/empty mbarriers), commits to the accumulator barrier.
+//   warp 5      one lane streams the layer-1 weight chunk of every ring stage from L2 with
+//               cp.async.bulk (W1 is NOT kept resident: a small shared-memory footprint leaves the L1
+//               large enough to keep the gathers' misses in flight).
+//   warps 6..   gather warps: lane = ray, one work item = (32-ray group, endpoint, PE sample); the
+//               L levels of that sample are interpolated (8 table gathers each, fp32, two batches of
+//               loads in flight) and written as fp16 into the canonical K-major SWIZZLE_128B A chunk
+//               of the stage, 16 bytes per store.
+// Hidden/output weights sit in shared memory for the whole kernel as pre-swizzled B-operand images.
+// The layer-1 accumulator is double-buffered in TMEM so the gathers of tile t+1 overlap the MLP tail
+// of tile t.
 #include "nif_encode.cuh"
 
 #include <type_traits>
