@@ -35,10 +35,8 @@ constexpr int TC_GATHER_WARPS = NIF_TC_GATHER_WARPS;
 constexpr int TC_MMA_WARP = TC_ROW_WARPS;    // warp index 4
 constexpr int TC_TMA_WARP = TC_ROW_WARPS + 1;  // warp index 5: streams the layer-1 weight chunks
 constexpr int TC_THREADS = 32 * (TC_ROW_WARPS + 2 + TC_GATHER_WARPS);
-#ifndef NIF_TC_STAGES
-#define NIF_TC_STAGES 4
-#endif
-constexpr int TC_STAGES = NIF_TC_STAGES;     // ring depth; one stage = A chunk (128 x 64) + W1 chunk (W x 64)
+constexpr int TC_MAX_STAGES = 4;             // ring depth (runtime 2..4); one stage = A chunk (128 x 64) + W1 chunk (W x 64)
+constexpr int TC_HSLOTS = 2;                 // ring of hidden/output-layer weight chunks (W x 64 each)
 constexpr int TC_A_CHUNK_BYTES = TC_TILE * 128;
 constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded to the UMMA minimum)
 
@@ -171,6 +169,7 @@ struct TcParams {
     const __half* table;
     const uint8_t* w_img;         // B-operand images: W1 chunks | hidden layers 2..H | output layer
     uint32_t w_bytes, w1_bytes;
+    int stages;                   // ring depth, 2..TC_MAX_STAGES
     float theta_max, bend_k;
     const float* origin;
     const float* dir;
@@ -183,12 +182,12 @@ struct TcParams {
 struct TcSmemLayout {
     uint32_t w_img, a_ring, act, ray_buf, bars, total;
 };
-__host__ __device__ inline TcSmemLayout tc_smem_layout(uint32_t w_res_bytes, int W)
+__host__ __device__ inline TcSmemLayout tc_smem_layout(int stages, int W)
 {
     TcSmemLayout L;
     uint32_t off = 0;
-    L.w_img = off;   off += (w_res_bytes + 1023u) & ~1023u;          // resident: hidden + output layers
-    L.a_ring = off;  off += TC_STAGES * (TC_A_CHUNK_BYTES + (uint32_t)W * 128u);   // stage = A chunk | W1 chunk
+    L.w_img = off;   off += TC_HSLOTS * (uint32_t)W * 128u;          // hidden/output weight chunk ring
+    L.a_ring = off;  off += (uint32_t)stages * (TC_A_CHUNK_BYTES + (uint32_t)W * 128u);   // stage = A chunk | W1 chunk
     L.act = off;     off += (uint32_t)((W + 63) / 64) * TC_A_CHUNK_BYTES;
     L.ray_buf = off; off += 2u * TC_TILE * 8u * sizeof(float);
     L.bars = off;    off += 512;
@@ -196,9 +195,9 @@ __host__ __device__ inline TcSmemLayout tc_smem_layout(uint32_t w_res_bytes, int
     return L;
 }
 
-enum { BAR_FULL = 0, BAR_EMPTY = TC_STAGES, BAR_ACC_FULL = 2 * TC_STAGES, BAR_ACC_EMPTY = BAR_ACC_FULL + 2,
+enum { BAR_FULL = 0, BAR_EMPTY = TC_MAX_STAGES, BAR_ACC_FULL = 2 * TC_MAX_STAGES, BAR_ACC_EMPTY = BAR_ACC_FULL + 2,
        BAR_RAY_FULL = BAR_ACC_EMPTY + 2, BAR_RAY_EMPTY = BAR_RAY_FULL + 2, BAR_HID = BAR_RAY_EMPTY + 2,
-       BAR_W = BAR_HID + 1, BAR_COUNT = BAR_W + 1 };
+       BAR_HFULL = BAR_HID + 1, BAR_HEMPTY = BAR_HFULL + TC_HSLOTS, BAR_COUNT = BAR_HEMPTY + TC_HSLOTS };
 
 // ---- (a3) gathers of one sample, software-pipelined in batches of 8/F levels (16 loads of 4 B for
 // F = 2, 8 loads of 8 B for F = 4).  issue() computes the 8 table indices of each level of the batch
@@ -308,20 +307,16 @@ __device__ __forceinline__ void drain_relu_to_act(uint32_t taddr_row, uint32_t a
     }
 }
 
-// issues D[128 x N] = act[128 x W] * Wimg[N x W]^T (one thread)
+// issues D[128 x N] (+)= act[:, 64 kc .. 64 kc + 63] * Wchunk[N x 64]^T for one K chunk (one thread)
 template <int W>
-__device__ __forceinline__ void issue_layer(uint32_t d_tmem, uint32_t act_base, uint32_t w_base, int N)
+__device__ __forceinline__ void issue_layer_chunk(uint32_t d_tmem, uint32_t act_base, uint32_t w_chunk, int N, int kc)
 {
-    constexpr int KC = (W + 63) / 64;                      // 64-column chunks
     constexpr int K16 = (W < 64 ? W : 64) / 16;            // UMMA K steps per chunk
     const uint32_t idesc = idesc_f16(TC_TILE, N);
 #pragma unroll
-    for (int kc = 0; kc < KC; ++kc)
-#pragma unroll
-        for (int k = 0; k < K16; ++k)
-            umma_f16(d_tmem, smem_desc_sw128(act_base + (uint32_t)kc * TC_A_CHUNK_BYTES + (uint32_t)k * 32u),
-                     smem_desc_sw128(w_base + (uint32_t)kc * (uint32_t)(N * 128) + (uint32_t)k * 32u), idesc,
-                     (uint32_t)((kc | k) != 0));
+    for (int k = 0; k < K16; ++k)
+        umma_f16(d_tmem, smem_desc_sw128(act_base + (uint32_t)kc * TC_A_CHUNK_BYTES + (uint32_t)k * 32u),
+                 smem_desc_sw128(w_chunk + (uint32_t)k * 32u), idesc, (uint32_t)((kc | k) != 0));
 }
 
 template <int W, int F>
@@ -331,13 +326,16 @@ k_fused_encode_mlp(const TcParams p)
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    const TcSmemLayout SL = tc_smem_layout(p.w_bytes - p.w1_bytes, W);
+    const TcSmemLayout SL = tc_smem_layout(p.stages, W);
+    const uint32_t TC_STAGES = (uint32_t)p.stages;
+    constexpr uint32_t HCHUNK = (uint32_t)W * 128u;                            // hidden-layer weight chunk (W x 64 fp16)
     constexpr uint32_t STAGE_BYTES = TC_A_CHUNK_BYTES + (uint32_t)W * 128u;
     const uint32_t s_w = smem_base + SL.w_img, s_a = smem_base + SL.a_ring, s_act = smem_base + SL.act;
     float* ray_buf = reinterpret_cast<float*>(smem_gen + SL.ray_buf);          // [2][128][8]
     const uint32_t s_bar = smem_base + SL.bars;
-    uint32_t* s_tmem_ptr = reinterpret_cast<uint32_t*>(smem_gen + SL.bars + 8 * BAR_COUNT);
-    TcLevel* s_lvl = reinterpret_cast<TcLevel*>(smem_gen + SL.bars + 8 * BAR_COUNT + 16);
+    uint32_t* s_tmem_ptr = reinterpret_cast<uint32_t*>(smem_gen + SL.bars + 240);
+    TcLevel* s_lvl = reinterpret_cast<TcLevel*>(smem_gen + SL.bars + 256);      // 16 levels x 16 B, 16-byte aligned
+    static_assert(8 * BAR_COUNT <= 240, "barrier block overlaps the TMEM pointer slot");
     auto bar = [&](int i) { return s_bar + 8u * (uint32_t)i; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -348,12 +346,13 @@ k_fused_encode_mlp(const TcParams p)
 
     // ---- one-time setup ------------------------------------------------------------------------
     if (tid == 0) {
-        for (int i = 0; i < TC_STAGES; ++i) { mbar_init(bar(BAR_FULL + i), 4u * (uint32_t)epc + 1u); mbar_init(bar(BAR_EMPTY + i), 1); }
+        for (int i = 0; i < TC_MAX_STAGES; ++i) { mbar_init(bar(BAR_FULL + i), 4u * (uint32_t)epc + 1u); mbar_init(bar(BAR_EMPTY + i), 1); }
+        for (int i = 0; i < TC_HSLOTS; ++i) { mbar_init(bar(BAR_HFULL + i), 1); mbar_init(bar(BAR_HEMPTY + i), 1); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar(BAR_ACC_FULL + i), 1); mbar_init(bar(BAR_ACC_EMPTY + i), TC_TILE);
             mbar_init(bar(BAR_RAY_FULL + i), TC_TILE); mbar_init(bar(BAR_RAY_EMPTY + i), TC_GATHER_WARPS);
         }
-        mbar_init(bar(BAR_HID), 1); mbar_init(bar(BAR_W), 1);
+        mbar_init(bar(BAR_HID), 1);
         fence_barrier_init();
     }
     if (tid < NIF_MAX_LEVELS) {
@@ -374,24 +373,23 @@ k_fused_encode_mlp(const TcParams p)
     const long long n_tiles = (n_hit + TC_TILE - 1) / TC_TILE;
     const int n_my = (int)((n_tiles > (long long)blockIdx.x) ? (n_tiles - 1 - blockIdx.x) / gridDim.x + 1 : 0);
 
-    // weight images -> shared memory, once (TMA bulk copies, completion on BAR_W)
-    if (warp == TC_MMA_WARP && lane == 0 && n_my > 0) {
-        const uint32_t res_bytes = p.w_bytes - p.w1_bytes;
-        mbar_expect_tx(bar(BAR_W), res_bytes);
-        for (uint32_t off = 0; off < res_bytes; off += 16384u) {
-            const uint32_t n = res_bytes - off < 16384u ? res_bytes - off : 16384u;
-            bulk_g2s(s_w + off, p.w_img + p.w1_bytes + off, n, bar(BAR_W));
-        }
-    }
-    const uint32_t s_wh = s_w;
-    const uint32_t s_wo = s_wh + (uint32_t)(p.hidden_layers - 1) * (uint32_t)(KC * W * 128);
-
     if (warp < TC_ROW_WARPS) {
         // ======================= row warps: (a2) for the next tile, MLP tail + (a5) ==============
         const int r = tid;
         long long cur_ray = -1, nxt_ray = -1;
         float cur_ti = 0.f, cur_to = 0.f, nxt_ti = 0.f, nxt_to = 0.f;
-        uint32_t hid_phase = 0;
+        uint32_t hid_phase = 0, hq = 0;                   // hq: hidden/output weight chunks consumed so far
+        auto run_layer = [&](uint32_t d_tmem, int N) {   // thread 0: one layer, chunks arrive through the H ring
+            tc_fence_after();
+            for (int kc = 0; kc < KC; ++kc, ++hq) {
+                const uint32_t slot = hq % TC_HSLOTS;
+                mbar_wait(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u);
+                tc_fence_after();
+                issue_layer_chunk<W>(d_tmem, s_act, s_w + slot * HCHUNK, N, kc);
+                umma_commit(bar(BAR_HEMPTY + slot));
+            }
+            umma_commit(bar(BAR_HID));
+        };
         auto prepare = [&](int j) {                       // rest-space endpoints of tile j -> ray_buf[j&1]
             const int b = j & 1;
             mbar_wait(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
@@ -412,7 +410,7 @@ k_fused_encode_mlp(const TcParams p)
             rb[3] = nif_normalise(xo); rb[4] = nif_normalise(yo); rb[5] = nif_normalise(zo);
             mbar_arrive(bar(BAR_RAY_FULL + b));
         };
-        if (n_my > 0) { prepare(0); mbar_wait(bar(BAR_W), 0); }
+        if (n_my > 0) prepare(0);
         const uint32_t t_row = (uint32_t)(warp * 32) << 16;          // this warp's TMEM lane quarter
         for (int j = 0; j < n_my; ++j) {
             cur_ray = nxt_ray; cur_ti = nxt_ti; cur_to = nxt_to;
@@ -428,11 +426,7 @@ k_fused_encode_mlp(const TcParams p)
             row_bar_sync();
             // hidden layers 2..H
             for (int hl = 1; hl < p.hidden_layers; ++hl) {
-                if (tid == 0) {
-                    tc_fence_after();
-                    issue_layer<W>(tm_hid, s_act, s_wh + (uint32_t)(hl - 1) * (uint32_t)(KC * W * 128), W);
-                    umma_commit(bar(BAR_HID));
-                }
+                if (tid == 0) run_layer(tm_hid, W);
                 mbar_wait(bar(BAR_HID), hid_phase); hid_phase ^= 1u;
                 tc_fence_after();
                 drain_relu_to_act<W>(tm_hid + t_row, s_act, (uint32_t)r);
@@ -441,11 +435,7 @@ k_fused_encode_mlp(const TcParams p)
                 row_bar_sync();
             }
             // output layer (12 heads padded to N = 16) and (a5) decode
-            if (tid == 0) {
-                tc_fence_after();
-                issue_layer<W>(tm_out, s_act, s_wo, TC_NOUT_PAD);
-                umma_commit(bar(BAR_HID));
-            }
+            if (tid == 0) run_layer(tm_out, TC_NOUT_PAD);
             mbar_wait(bar(BAR_HID), hid_phase); hid_phase ^= 1u;
             tc_fence_after();
             uint32_t zr[16];
@@ -463,7 +453,6 @@ k_fused_encode_mlp(const TcParams p)
     } else if (warp == TC_MMA_WARP) {
         // ======================= layer-1 MMA issuer =============================================
         if (lane == 0 && n_my > 0) {
-            mbar_wait(bar(BAR_W), 0);
             const uint32_t idesc = idesc_f16(TC_TILE, W);
             uint32_t q = 0;
             for (int j = 0; j < n_my; ++j) {
@@ -498,6 +487,24 @@ k_fused_encode_mlp(const TcParams p)
                     mbar_expect_tx(bar(BAR_FULL + stage), W1_CHUNK);
                     bulk_g2s(s_a + stage * STAGE_BYTES + TC_A_CHUNK_BYTES, p.w_img + (size_t)c * W1_CHUNK, W1_CHUNK,
                              bar(BAR_FULL + stage));
+                }
+        } else if (lane == 1) {
+            // hidden layers 2..H and the output layer: KC chunks each, per tile, in the order the row
+            // warps consume them (they are small, so they share one 2-slot ring instead of living in smem)
+            const uint8_t* wh = p.w_img + p.w1_bytes;
+            const uint32_t out_chunk = TC_NOUT_PAD * 128u;
+            uint32_t hq = 0;
+            for (int j = 0; j < n_my; ++j)
+                for (int l = 1; l <= p.hidden_layers; ++l) {
+                    const bool is_out = l == p.hidden_layers;
+                    const uint32_t bytes = is_out ? out_chunk : HCHUNK;
+                    const uint8_t* src = wh + (size_t)(l - 1) * (size_t)(KC * HCHUNK);
+                    for (int kc = 0; kc < KC; ++kc, ++hq) {
+                        const uint32_t slot = hq % TC_HSLOTS;
+                        mbar_wait(bar(BAR_HEMPTY + slot), ((hq / TC_HSLOTS) & 1u) ^ 1u);
+                        mbar_expect_tx(bar(BAR_HFULL + slot), bytes);
+                        bulk_g2s(s_w + slot * HCHUNK, src + (size_t)kc * bytes, bytes, bar(BAR_HFULL + slot));
+                    }
                 }
         }
     } else {
@@ -588,6 +595,17 @@ TcShape tc_shape(const nif_net_desc* d)
 }
 
 constexpr uint32_t TC_MAX_SMEM = 227u * 1024u;
+constexpr uint32_t TC_L1_FRIENDLY_SMEM = 164u * 1024u;    // above this carve-out the L1 is too small for the gathers
+
+// ring depth: the deepest that keeps the footprint L1-friendly, else the deepest that fits at all
+int tc_pick_stages(int W)
+{
+    for (int st = TC_MAX_STAGES; st >= 3; --st)
+        if (tc_smem_layout(st, W).total <= TC_L1_FRIENDLY_SMEM) return st;
+    for (int st = TC_MAX_STAGES; st >= 2; --st)
+        if (tc_smem_layout(st, W).total <= TC_MAX_SMEM) return st;
+    return 0;
+}
 
 template <int W, int F>
 int launch_tc(const TcParams& p, uint32_t smem, int blocks, cudaStream_t stream)
@@ -610,7 +628,8 @@ int nif_tc_supported(const nif_net_desc* d)
     if (lf != 8 && lf != 16 && lf != 32 && lf != 64) return 0;
     if (d->hidden_layers < 1) return 0;
     const TcShape s = tc_shape(d);
-    return tc_smem_layout(s.w_bytes - s.w1_bytes, d->width).total <= TC_MAX_SMEM ? 1 : 0;
+    (void)s;
+    return tc_pick_stages(d->width) >= 2 ? 1 : 0;
 }
 
 int nif_tc_pack_weights(nif_net* net, cudaStream_t stream)
@@ -651,7 +670,8 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
     p.origin = rays->origin; p.dir = rays->dir;
     p.out = *out; p.scratch = scratch; p.hit_list = hit_list; p.flags = flags;
-    const uint32_t smem = tc_smem_layout(s.w_bytes - s.w1_bytes, d->width).total;
+    p.stages = tc_pick_stages(d->width);
+    const uint32_t smem = tc_smem_layout(p.stages, d->width).total;
     static int n_sm = 0;
     if (!n_sm) {
         int dev = 0;
