@@ -67,6 +67,22 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
             "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
     } while (!done);
 }
+// wait for the role warps whose waits are long (a whole tile of gathers): poll, then sleep between polls
+// so that the spin loop does not take issue slots from the gather warps
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, unsigned ns)
+{
+    for (;;) {
+        uint32_t done;
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(ns);
+    }
+}
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -230,24 +246,28 @@ struct GatherBatch {
             const float flx = fminf(floorf(posx), lv.y), fly = fminf(floorf(posy), lv.y), flz = fminf(floorf(posz), lv.y);
             wx[li] = posx - flx; wy[li] = posy - fly; wz[li] = posz - flz;
             const uint32_t cx = (uint32_t)flx, cy = (uint32_t)fly, cz = (uint32_t)flz;
-            uint32_t idx[8];
+            // byte offsets (32-bit) from the level's base: entry index << log2(entry bytes), folded into
+            // the index arithmetic so that each gather is one LDG [uniform base + 32-bit offset]
+            constexpr uint32_t SH = (F == 2) ? 2u : 3u;
+            uint32_t off[8];
             if (np1) {
-                const uint32_t o2 = np1 * np1;
-                const uint32_t b = cx + np1 * cy + o2 * cz;
+                const uint32_t o1 = np1 << SH, o2 = (np1 * np1) << SH;
+                const uint32_t b = (cx + np1 * cy + np1 * np1 * cz) << SH;
 #pragma unroll
                 for (int c = 0; c < 8; ++c)
-                    idx[c] = b + (uint32_t)(c & 1) + (((c >> 1) & 1) ? np1 : 0u) + ((c >> 2) ? o2 : 0u);
+                    off[c] = b + ((c & 1) ? (1u << SH) : 0u) + (((c >> 1) & 1) ? o1 : 0u) + ((c >> 2) ? o2 : 0u);
             } else {
+                const uint32_t m = t_mask << SH;
                 const uint32_t hy0 = cy * 2654435761u, hy1 = hy0 + 2654435761u;
                 const uint32_t hz0 = cz * 805459861u, hz1 = hz0 + 805459861u;
-                const uint32_t hyz[4] = {hy0 ^ hz0, hy1 ^ hz0, hy0 ^ hz1, hy1 ^ hz1};
-                const uint32_t cx1 = cx + 1u;
+                const uint32_t hyz[4] = {(hy0 ^ hz0) << SH, (hy1 ^ hz0) << SH, (hy0 ^ hz1) << SH, (hy1 ^ hz1) << SH};
+                const uint32_t x0 = cx << SH, x1 = (cx + 1u) << SH;
 #pragma unroll
-                for (int c = 0; c < 8; ++c) idx[c] = (((c & 1) ? cx1 : cx) ^ hyz[c >> 1]) & t_mask;
+                for (int c = 0; c < 8; ++c) off[c] = (((c & 1) ? x1 : x0) ^ hyz[c >> 1]) & m;
             }
-            const raw_t* lvl = reinterpret_cast<const raw_t*>(table) + ((size_t)l << log2_T);
+            const char* lvl = reinterpret_cast<const char*>(table) + ((size_t)l << (log2_T + SH));
 #pragma unroll
-            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(lvl + idx[c]);
+            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(reinterpret_cast<const raw_t*>(lvl + off[c]));
         }
     }
 
@@ -383,7 +403,7 @@ k_fused_encode_mlp(const TcParams p)
             tc_fence_after();
             for (int kc = 0; kc < KC; ++kc, ++hq) {
                 const uint32_t slot = hq % TC_HSLOTS;
-                mbar_wait(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u);
+                mbar_wait_sleep(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u, 32);
                 tc_fence_after();
                 issue_layer_chunk<W>(d_tmem, s_act, s_w + slot * HCHUNK, N, kc);
                 umma_commit(bar(BAR_HEMPTY + slot));
@@ -392,7 +412,7 @@ k_fused_encode_mlp(const TcParams p)
         };
         auto prepare = [&](int j) {                       // rest-space endpoints of tile j -> ray_buf[j&1]
             const int b = j & 1;
-            mbar_wait(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
+            mbar_wait_sleep(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 128);
             const long long tile = (long long)blockIdx.x + (long long)j * gridDim.x;
             const long long h = tile * TC_TILE + r;
             float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f;
@@ -417,7 +437,7 @@ k_fused_encode_mlp(const TcParams p)
             if (j + 1 < n_my) prepare(j + 1);
             const int b = j & 1;
             // layer 1 accumulator of tile j
-            mbar_wait(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1));
+            mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1), 256);
             tc_fence_after();
             drain_relu_to_act<W>(tm_acc1 + (uint32_t)(b * W) + t_row, s_act, (uint32_t)r);
             tc_fence_before();
@@ -427,7 +447,7 @@ k_fused_encode_mlp(const TcParams p)
             // hidden layers 2..H
             for (int hl = 1; hl < p.hidden_layers; ++hl) {
                 if (tid == 0) run_layer(tm_hid, W);
-                mbar_wait(bar(BAR_HID), hid_phase); hid_phase ^= 1u;
+                mbar_wait_sleep(bar(BAR_HID), hid_phase, 32); hid_phase ^= 1u;
                 tc_fence_after();
                 drain_relu_to_act<W>(tm_hid + t_row, s_act, (uint32_t)r);
                 tc_fence_before();
@@ -436,7 +456,7 @@ k_fused_encode_mlp(const TcParams p)
             }
             // output layer (12 heads padded to N = 16) and (a5) decode
             if (tid == 0) run_layer(tm_out, TC_NOUT_PAD);
-            mbar_wait(bar(BAR_HID), hid_phase); hid_phase ^= 1u;
+            mbar_wait_sleep(bar(BAR_HID), hid_phase, 32); hid_phase ^= 1u;
             tc_fence_after();
             uint32_t zr[16];
             __syncwarp();
@@ -457,11 +477,11 @@ k_fused_encode_mlp(const TcParams p)
             uint32_t q = 0;
             for (int j = 0; j < n_my; ++j) {
                 const int b = j & 1;
-                mbar_wait(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
+                mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 64);
                 tc_fence_after();
                 for (int c = 0; c < n_chunks; ++c, ++q) {
                     const uint32_t stage = q % TC_STAGES;
-                    mbar_wait(bar(BAR_FULL + stage), (q / TC_STAGES) & 1u);
+                    mbar_wait_sleep(bar(BAR_FULL + stage), (q / TC_STAGES) & 1u, 64);
                     tc_fence_after();
                     const uint32_t a0 = s_a + stage * STAGE_BYTES, b0 = a0 + TC_A_CHUNK_BYTES;
 #pragma unroll
@@ -483,7 +503,7 @@ k_fused_encode_mlp(const TcParams p)
             for (int j = 0; j < n_my; ++j)
                 for (int c = 0; c < n_chunks; ++c, ++q) {
                     const uint32_t stage = q % TC_STAGES;
-                    mbar_wait(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u);
+                    mbar_wait_sleep(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u, 128);
                     mbar_expect_tx(bar(BAR_FULL + stage), W1_CHUNK);
                     bulk_g2s(s_a + stage * STAGE_BYTES + TC_A_CHUNK_BYTES, p.w_img + (size_t)c * W1_CHUNK, W1_CHUNK,
                              bar(BAR_FULL + stage));
@@ -501,7 +521,7 @@ k_fused_encode_mlp(const TcParams p)
                     const uint8_t* src = wh + (size_t)(l - 1) * (size_t)(KC * HCHUNK);
                     for (int kc = 0; kc < KC; ++kc, ++hq) {
                         const uint32_t slot = hq % TC_HSLOTS;
-                        mbar_wait(bar(BAR_HEMPTY + slot), ((hq / TC_HSLOTS) & 1u) ^ 1u);
+                        mbar_wait_sleep(bar(BAR_HEMPTY + slot), ((hq / TC_HSLOTS) & 1u) ^ 1u, 128);
                         mbar_expect_tx(bar(BAR_HFULL + slot), bytes);
                         bulk_g2s(s_w + slot * HCHUNK, src + (size_t)kc * bytes, bytes, bar(BAR_HFULL + slot));
                     }
