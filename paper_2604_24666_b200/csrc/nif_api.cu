@@ -116,7 +116,7 @@ extern "C" int nif_net_uses_tensor_cores(const nif_net* net)
 extern "C" int nif_query_workspace_bytes(int64_t n, size_t* bytes)
 {
     if (!bytes || n < 0 || n > 0x7fffffffLL) return NIF_ERR_INVALID_ARG;
-    *bytes = align_up(sizeof(NifQueryScratch) + (size_t)n * sizeof(int32_t), 256) + 256;
+    *bytes = align_up(sizeof(NifQueryScratch) + (size_t)NIF_MAX_BINS * 4 + (size_t)n * 8, 256) + 256;
     return NIF_OK;
 }
 
@@ -147,13 +147,27 @@ extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_b
     nif_query_workspace_bytes(rays->n, &need);
     if (!workspace || ((uintptr_t)workspace & 255u) != 0 || workspace_bytes < need - 256) return NIF_ERR_WORKSPACE;
     cudaStream_t stream = (cudaStream_t)stream_;
-    NifQueryScratch* scratch = (NifQueryScratch*)workspace;
-    int32_t* hit_list = (int32_t*)((char*)workspace + sizeof(NifQueryScratch));
-    NIF_CUDA_TRY(cudaMemsetAsync(scratch, 0, sizeof(NifQueryScratch), stream));
+    NifQueryWs ws;
+    ws.scratch = (NifQueryScratch*)workspace;
+    ws.bin_count = (uint32_t*)((char*)workspace + sizeof(NifQueryScratch));
+    ws.rank = ws.bin_count + NIF_MAX_BINS;
+    ws.hit_list = (int32_t*)(ws.rank + rays->n);
+    ws.bin_shift = 0;
+    for (;;) {                                               // bricks of 2^s voxels until the bins fit
+        ws.nvb = (bvh->nv + (1 << ws.bin_shift) - 1) >> ws.bin_shift;
+        if ((unsigned long long)ws.nvb * ws.nvb * ws.nvb <= NIF_MAX_BINS) break;
+        ++ws.bin_shift;
+    }
+    ws.n_bins = (uint32_t)(ws.nvb * ws.nvb * ws.nvb);
+    NifQueryScratch* scratch = ws.scratch;
+    int32_t* hit_list = ws.hit_list;
+    const bool traverse_only = (flags & NIF_TRAVERSE_ONLY) != 0;
+    NIF_CUDA_TRY(cudaMemsetAsync(workspace, 0, sizeof(NifQueryScratch) + (traverse_only ? 0 : (size_t)ws.n_bins * 4), stream));
     const int prof = nif_prof_begin(stream);                 // -1 unless nif_profile_enable(1)
-    rc = nif_launch_traverse(bvh, rays, out, scratch, hit_list, flags, stream);
+    rc = nif_launch_traverse(bvh, rays, out, &ws, flags, stream);
+    if (rc == NIF_OK && !traverse_only) rc = nif_launch_bin_hits(bvh, rays, out, &ws, stream);
     nif_prof_mark(prof, 1, stream);
-    if (rc != NIF_OK || (flags & NIF_TRAVERSE_ONLY)) return rc;
+    if (rc != NIF_OK || traverse_only) return rc;
     const bool use_tc = net->desc.dtype == NIF_F16 && net->tc_supported && !(flags & NIF_ENGINE_FFMA);
     if (use_tc) rc = nif_launch_fused_tc(bvh, net, rays, out, scratch, hit_list, flags, stream);
     else rc = nif_launch_ffma(bvh, net, rays, out, scratch, hit_list, flags, stream);

@@ -58,14 +58,26 @@ struct nif_net {
     int tc_supported;
 };
 
-// per-query scratch layout (device)
+// per-query scratch layout (device):
+//   [NifQueryScratch header][uint32 bin_count[NIF_MAX_BINS]][uint32 rank[n]][int32 hit_list[n]]
+// Hit rays are binned by the voxel they hit (bricks of voxels when nv^3 > NIF_MAX_BINS) so that the
+// 128-ray tiles of the encode kernel are spatially coherent in rest space.
+#define NIF_MAX_BINS (1u << 21)
 struct NifQueryScratch {
-    unsigned long long n_hit;          // hit rays appended by the traversal
-    unsigned int tile_counter;         // dynamic tile scheduler of the fused kernel
+    unsigned long long n_hit;          // cursor of the bin allocation = hit rays once k_bin_offsets has run
+    unsigned int tile_counter;         // (unused) dynamic tile scheduler of the fused kernel
     unsigned int pad[13];
-    // followed by int32 hit_list[n]
 };
 static_assert(sizeof(NifQueryScratch) == 64, "scratch header is 64 bytes");
+
+struct NifQueryWs {                    // pointers into the caller's workspace
+    NifQueryScratch* scratch;
+    uint32_t* bin_count;
+    uint32_t* rank;
+    int32_t* hit_list;
+    uint32_t n_bins;
+    int bin_shift, nvb;                // bin = (ix >> s) + nvb * ((iy >> s) + nvb * (iz >> s))
+};
 
 extern "C" void nif_count_launch(int n);
 
@@ -77,8 +89,9 @@ extern "C" void nif_count_launch(int n);
 
 // launchers implemented in the individual .cu files
 int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        NifQueryScratch* scratch, int32_t* hit_list, unsigned flags,
-                        cudaStream_t stream);
+                        const NifQueryWs* ws, unsigned flags, cudaStream_t stream);
+int nif_launch_bin_hits(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
+                        const NifQueryWs* ws, cudaStream_t stream);
 int nif_launch_ffma(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                     const nif_query_out* out, const NifQueryScratch* scratch,
                     const int32_t* hit_list, unsigned flags, cudaStream_t stream);

@@ -134,8 +134,8 @@ __global__ void __launch_bounds__(TRAV_BLOCK)
 k_traverse(const NifNode* __restrict__ nodes, const float4* __restrict__ lat, int nv, int root,
            float rlx, float rly, float rlz, float rhx, float rhy, float rhz,
            long long n, const float* __restrict__ origin, const float* __restrict__ dir,
-           nif_query_out out, NifQueryScratch* __restrict__ scratch, int32_t* __restrict__ hit_list,
-           unsigned flags)
+           nif_query_out out, uint32_t* __restrict__ bin_count, uint32_t* __restrict__ rank,
+           int bin_shift, int nvb, unsigned flags)
 {
     const long long ray = (long long)blockIdx.x * TRAV_BLOCK + threadIdx.x;
     const bool active = ray < n;
@@ -216,32 +216,88 @@ k_traverse(const NifNode* __restrict__ nodes, const float4* __restrict__ lat, in
             for (int a = 0; a < NIF_N_OUT; ++a) out.raw_logits[NIF_N_OUT * ray + a] = 0.0f;
         }
     }
-    // hit-ray compaction: warp-aggregated append keeps each warp's rays contiguous, so the
-    // encode kernel sees the traversal's coherence
-    const unsigned m = __ballot_sync(0xffffffffu, hit);
-    if (m) {
-        const int lane = threadIdx.x & 31;
-        const int leader = __ffs(m) - 1;
-        unsigned long long base = 0;
-        if (lane == leader) base = atomicAdd(&scratch->n_hit, (unsigned long long)__popc(m));
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (hit) hit_list[base + __popc(m & ((1u << lane) - 1u))] = (int32_t)ray;
+    // hit rays are counted into the bin of the voxel they hit; the returned count is the ray's rank
+    // inside its bin (k_bin_offsets / k_scatter_hits below turn ranks into positions in hit_list)
+    if (hit) {
+        const uint32_t unv = (uint32_t)nv, id = (uint32_t)best_id;
+        const uint32_t ix = id % unv, iy = (id / unv) % unv, iz = id / (unv * unv);
+        const uint32_t bin = (ix >> bin_shift) + (uint32_t)nvb * ((iy >> bin_shift) + (uint32_t)nvb * (iz >> bin_shift));
+        rank[ray] = atomicAdd(&bin_count[bin], 1u);
     }
+}
+
+// bin_count[b] -> start of bin b in hit_list.  Each block scans 1024 consecutive bins and takes one
+// contiguous range from the global cursor (scratch->n_hit): bins of a block stay in order, blocks
+// land in arrival order -- enough locality for the encode kernel's tiles, no multi-pass scan.
+__global__ void __launch_bounds__(1024)
+k_bin_offsets(uint32_t* __restrict__ bin_count, uint32_t n_bins, NifQueryScratch* __restrict__ scratch)
+{
+    __shared__ uint32_t warp_sum[32];
+    __shared__ unsigned long long block_base;
+    const uint32_t b = blockIdx.x * 1024u + threadIdx.x;
+    const uint32_t c = b < n_bins ? bin_count[b] : 0u;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t inc = c;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) warp_sum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        uint32_t v = warp_sum[lane];
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, v, d);
+            if (lane >= d) v += t;
+        }
+        warp_sum[lane] = v;                                             // inclusive over warps
+        if (lane == 31) block_base = v ? atomicAdd(&scratch->n_hit, (unsigned long long)v) : 0ull;
+    }
+    __syncthreads();
+    if (b < n_bins) bin_count[b] = (uint32_t)block_base + (wid ? warp_sum[wid - 1] : 0u) + inc - c;
+}
+
+__global__ void __launch_bounds__(256)
+k_scatter_hits(long long n, int nv, int bin_shift, int nvb, const int32_t* __restrict__ voxel_id,
+               const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ rank,
+               int32_t* __restrict__ hit_list)
+{
+    const long long ray = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (ray >= n) return;
+    const int32_t vid = voxel_id[ray];
+    if (vid < 0) return;
+    const uint32_t unv = (uint32_t)nv, id = (uint32_t)vid;
+    const uint32_t ix = id % unv, iy = (id / unv) % unv, iz = id / (unv * unv);
+    const uint32_t bin = (ix >> bin_shift) + (uint32_t)nvb * ((iy >> bin_shift) + (uint32_t)nvb * (iz >> bin_shift));
+    hit_list[bin_start[bin] + rank[ray]] = (int32_t)ray;
 }
 
 }  // namespace
 
 int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        NifQueryScratch* scratch, int32_t* hit_list, unsigned flags,
-                        cudaStream_t stream)
+                        const NifQueryWs* ws, unsigned flags, cudaStream_t stream)
 {
     if (rays->n == 0) return NIF_OK;
     const long long blocks = (rays->n + TRAV_BLOCK - 1) / TRAV_BLOCK;
     k_traverse<<<(unsigned)blocks, TRAV_BLOCK, 0, stream>>>(
         bvh->nodes, bvh->lattice, bvh->nv, bvh->root, bvh->lo[0], bvh->lo[1], bvh->lo[2],
         bvh->hi[0], bvh->hi[1], bvh->hi[2], (long long)rays->n, rays->origin, rays->dir, *out,
-        scratch, hit_list, flags);
+        ws->bin_count, ws->rank, ws->bin_shift, ws->nvb, flags);
     nif_count_launch(1);
+    NIF_CUDA_TRY(cudaGetLastError());
+    return NIF_OK;
+}
+
+int nif_launch_bin_hits(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
+                        const NifQueryWs* ws, cudaStream_t stream)
+{
+    if (rays->n == 0) return NIF_OK;
+    k_bin_offsets<<<(ws->n_bins + 1023u) / 1024u, 1024, 0, stream>>>(ws->bin_count, ws->n_bins, ws->scratch);
+    k_scatter_hits<<<(unsigned)((rays->n + 255) / 256), 256, 0, stream>>>(
+        (long long)rays->n, bvh->nv, ws->bin_shift, ws->nvb, out->voxel_id, ws->bin_count, ws->rank, ws->hit_list);
+    nif_count_launch(2);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;
 }
