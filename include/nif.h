@@ -49,7 +49,13 @@ enum { NIF_F32 = 0, NIF_F16 = 1 };            /* nif_net_desc.dtype */
 enum {
     NIF_OCCLUSION_ONLY = 1u,   /* decode only the occlusion head (B:10); other head outputs untouched */
     NIF_ENGINE_FFMA    = 2u,   /* force the scalar-FMA encode+MLP kernel even for NIF_F16 nets        */
-    NIF_TRAVERSE_ONLY  = 4u    /* step (1) only: voxel_id, t_in, t_out                                */
+    NIF_TRAVERSE_ONLY  = 4u,   /* step (1) only: voxel_id, t_in, t_out                                */
+    /* The traversal has two kernels: one thread per ray with static assignment (best for coherent
+     * batches such as camera rays) and persistent warps with dynamic ray fetch (best for incoherent
+     * batches).  By default a device-side vote over sampled ray groups picks one; these force it.
+     * Results are identical either way. */
+    NIF_TRAVERSE_COHERENT   = 8u,
+    NIF_TRAVERSE_INCOHERENT = 16u
 };
 
 #define NIF_N_OUT 12   /* logits per ray: occlusion 1, distance 1, normal 3, albedo 3, material 4 (B:7) */

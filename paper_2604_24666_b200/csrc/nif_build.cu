@@ -224,6 +224,7 @@ __global__ void k_write_bricks(int nv, uint32_t n_bricks, const uint8_t* __restr
     }
     nd.mask = bits; nd.is_brick = 1;
     for (int i = 0; i < 6; ++i) nd.pad[i] = 0;
+    nd.pad[0] = 2u * bx + (uint32_t)nv * (2u * by + (uint32_t)nv * 2u * bz);   // voxel id of octant 0
     uint32_t idx = node_base + offs[m];
     store_node(nodes + idx, nd);
     boxes[2 * (size_t)idx] = make_float4(blo[0], blo[1], blo[2], 0.f);
@@ -257,6 +258,8 @@ __global__ void k_write_level(uint32_t n_cells, const uint8_t* __restrict__ mask
     (void)child_mask;
     nd.mask = bits; nd.is_brick = 0;
     for (int i = 0; i < 6; ++i) nd.pad[i] = 0;
+    // existing children are consecutive nodes (exclusive scan over Morton-ordered cells): first one
+    nd.pad[0] = child_base + child_offs[8 * (size_t)m + (size_t)(__ffs((int)bits) - 1)];
     uint32_t idx = node_base + offs[m];
     store_node(nodes + idx, nd);
     boxes[2 * (size_t)idx] = make_float4(blo[0], blo[1], blo[2], 0.f);

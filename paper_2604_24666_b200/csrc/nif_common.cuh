@@ -23,7 +23,8 @@ struct __align__(16) NifNode {
     uint32_t child[8];     // is_brick ? rest-space voxel id : node index
     uint32_t mask;         // bit c set <=> child c exists
     uint32_t is_brick;     // children are voxels (lowest level)
-    uint32_t pad[6];
+    uint32_t pad[6];       // pad[0]: brick -> voxel id of octant 0; inner -> index of the first existing child
+                           // (children of a node are consecutive nodes), so child ids need no lookup
 };
 static_assert(sizeof(NifNode) == 256, "NifNode must be 256 bytes");
 
@@ -65,7 +66,7 @@ struct nif_net {
 #define NIF_MAX_BINS (1u << 21)
 struct NifQueryScratch {
     unsigned long long n_hit;          // cursor of the bin allocation = hit rays once k_bin_offsets has run
-    unsigned int tile_counter;         // (unused) dynamic tile scheduler of the fused kernel
+    unsigned int tile_counter;         // dynamic ray fetch counter of the traversal kernel
     unsigned int pad[13];
 };
 static_assert(sizeof(NifQueryScratch) == 64, "scratch header is 64 bytes");

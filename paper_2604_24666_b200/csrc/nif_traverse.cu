@@ -127,102 +127,301 @@ __device__ __forceinline__ bool voxel_hit(const float4* __restrict__ lat, int nv
 }
 
 constexpr int TRAV_BLOCK = 128;
+constexpr int TRAV_BLOCKS_PER_SM = 6;
 constexpr int STACK_MAX = 96;                 // 7 pushes per level net, <= 10 levels
 constexpr uint32_t LEAF_FLAG = 0x80000000u;
+#ifndef NIF_TRAV_REFILL
+#define NIF_TRAV_REFILL 12
+#endif
+constexpr int TRAV_REFILL = NIF_TRAV_REFILL;               // fetch new rays when at least this many lanes are idle
 
-__global__ void __launch_bounds__(TRAV_BLOCK)
-k_traverse(const NifNode* __restrict__ nodes, const float4* __restrict__ lat, int nv, int root,
-           float rlx, float rly, float rlz, float rhx, float rhy, float rhz,
-           long long n, const float* __restrict__ origin, const float* __restrict__ dir,
-           nif_query_out out, uint32_t* __restrict__ bin_count, uint32_t* __restrict__ rank,
-           int bin_shift, int nvb, unsigned flags)
+struct TravParams {
+    const NifNode* nodes;
+    const float4* lat;
+    int nv, root;
+    float rlx, rly, rlz, rhx, rhy, rhz;       // root box
+    long long n;
+    const float* origin;
+    const float* dir;
+    nif_query_out out;
+    unsigned int* ray_counter;                // dynamic ray fetch (scratch header)
+    const unsigned int* coherent_flag;        // written by k_ray_coherence: 1 -> simple kernel, 0 -> persistent
+    uint32_t* bin_count;
+    uint32_t* rank;
+    int bin_shift, nvb;
+    unsigned flags;
+};
+
+// results of one finished ray: ids/t always; zero heads for a miss (R18); bin count for a hit
+__device__ __forceinline__ void retire_ray(const TravParams& p, long long ray, int32_t best_id, float best_in, float best_out)
 {
-    const long long ray = (long long)blockIdx.x * TRAV_BLOCK + threadIdx.x;
-    const bool active = ray < n;
+    p.out.voxel_id[ray] = best_id;
+    p.out.t_in[ray] = best_in;
+    p.out.t_out[ray] = best_out;
+    if (p.flags & NIF_TRAVERSE_ONLY) return;
+    if (best_id < 0) {
+        p.out.occlusion[ray] = 0.0f;
+        if (!(p.flags & NIF_OCCLUSION_ONLY)) {
+            p.out.distance[ray] = 0.0f; p.out.dist_total[ray] = 0.0f;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { p.out.normal[3 * ray + a] = 0.0f; p.out.albedo[3 * ray + a] = 0.0f; }
+#pragma unroll
+            for (int a = 0; a < 4; ++a) p.out.material_logits[4 * ray + a] = 0.0f;
+        }
+        if (p.out.raw_logits) {
+#pragma unroll
+            for (int a = 0; a < NIF_N_OUT; ++a) p.out.raw_logits[NIF_N_OUT * ray + a] = 0.0f;
+        }
+    } else {
+        // counted into the bin of the voxel it hit; the returned count is the ray's rank inside its
+        // bin (k_bin_offsets / k_scatter_hits below turn ranks into positions in hit_list)
+        const uint32_t unv = (uint32_t)p.nv, id = (uint32_t)best_id;
+        const uint32_t ix = id % unv, iy = (id / unv) % unv, iz = id / (unv * unv);
+        const uint32_t bin = (ix >> p.bin_shift) + (uint32_t)p.nvb * ((iy >> p.bin_shift) + (uint32_t)p.nvb * (iz >> p.bin_shift));
+        p.rank[ray] = atomicAdd(&p.bin_count[bin], 1u);
+    }
+}
+
+// Persistent warps, one ray per lane, "while-while" traversal with dynamic ray fetch: lanes first
+// work through inner nodes until every live lane has a voxel on top of its stack (or is finished),
+// then all of them run the expensive 12-triangle voxel test together; finished lanes are refilled
+// from a global counter once enough of them are idle.  Incoherent rays (config 3) otherwise leave
+// 4 of 32 lanes active on average.
+__global__ void __launch_bounds__(TRAV_BLOCK, TRAV_BLOCKS_PER_SM)
+k_traverse_persistent(const TravParams p)
+{
+    if (*p.coherent_flag != 0u) return;                   // k_traverse_simple takes this batch
+    const int lane = threadIdx.x & 31;
+    const NifNode* __restrict__ nodes = p.nodes;
+    uint2 stack[STACK_MAX];
+    int sp = 0;
+    long long ray = -1;                                   // -1: lane has no ray
     Ray r;
     int32_t best_id = -1;
     float best_in = INFINITY, best_out = INFINITY;
-    if (active) {
-        r.ox = origin[3 * ray]; r.oy = origin[3 * ray + 1]; r.oz = origin[3 * ray + 2];
-        r.dx = dir[3 * ray]; r.dy = dir[3 * ray + 1]; r.dz = dir[3 * ray + 2];
-        r.ix = __fdiv_rn(1.0f, r.dx); r.iy = __fdiv_rn(1.0f, r.dy); r.iz = __fdiv_rn(1.0f, r.dz);
-        uint2 stack[STACK_MAX];
-        int sp = 0;
-        float bn, bf;
-        if (root >= 0 && slab(rlx, rly, rlz, rhx, rhy, rhz, r, bn, bf)) {
-            stack[sp++] = make_uint2((uint32_t)root, __float_as_uint(bn));
+    bool exhausted = false;                               // the global counter ran past n
+
+    for (;;) {
+        // ---- refill idle lanes from the global ray counter.  Rays that miss the root box retire on
+        // the spot, so the loop keeps fetching until enough lanes hold a live ray.
+        for (;;) {
+            const unsigned idle = __ballot_sync(0xffffffffu, ray < 0);
+            if (exhausted || (__popc(idle) < TRAV_REFILL && idle != 0xffffffffu)) break;
+            unsigned base = 0;
+            if (lane == 0) base = atomicAdd(p.ray_counter, (unsigned)__popc(idle));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if ((long long)base + __popc(idle) >= p.n) exhausted = true;
+            const long long cand = (long long)base + __popc(idle & ((1u << lane) - 1u));
+            if (ray < 0 && cand < p.n) {
+                ray = cand;
+                r.ox = p.origin[3 * ray]; r.oy = p.origin[3 * ray + 1]; r.oz = p.origin[3 * ray + 2];
+                r.dx = p.dir[3 * ray]; r.dy = p.dir[3 * ray + 1]; r.dz = p.dir[3 * ray + 2];
+                r.ix = __fdiv_rn(1.0f, r.dx); r.iy = __fdiv_rn(1.0f, r.dy); r.iz = __fdiv_rn(1.0f, r.dz);
+                best_id = -1; best_in = INFINITY; best_out = INFINITY; sp = 0;
+                float bn, bf;
+                if (p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf)) {
+                    stack[sp++] = make_uint2((uint32_t)p.root, __float_as_uint(bn));
+                } else {
+                    retire_ray(p, ray, -1, INFINITY, INFINITY);
+                    ray = -1;
+                }
+            }
         }
-        while (sp > 0) {
-            const uint2 e = stack[--sp];
-            if (__uint_as_float(e.y) > best_in) continue;          // strictly later: cannot win a tie either
-            if (e.x & LEAF_FLAG) {
-                const uint32_t id = e.x & ~LEAF_FLAG;
-                float ti, to;
-                if (voxel_hit(lat, nv, id, r, ti, to)) {
-                    if (ti < best_in || (ti == best_in && (int32_t)id < best_id)) {
-                        best_id = (int32_t)id; best_in = ti; best_out = to;
+        if (__all_sync(0xffffffffu, ray < 0)) break;      // nothing left anywhere in this warp
+
+        // ---- phase A: inner nodes until every live lane has a voxel on top or an empty stack ----
+        for (;;) {
+            // drop entries that can no longer win (strictly later than the best entry: ties stay, R12)
+            while (sp > 0 && __uint_as_float(stack[sp - 1].y) > best_in) --sp;
+            const bool inner = ray >= 0 && sp > 0 && !(stack[sp - 1].x & LEAF_FLAG);
+            if (!__any_sync(0xffffffffu, inner)) break;
+            {
+                // one node per lane, branch-free: slab tests of the octants any lane has, a sorting
+                // network on packed (t_near, octant) keys, up to 8 predicated pushes (farthest first,
+                // so the nearest child ends on top).  Lanes without an inner node run it masked off.
+                float lo[3][8], hi[3][8];
+                uint4 meta = make_uint4(0u, 0u, 0u, 0u);                     // mask, is_brick, base, -
+                if (inner) {
+                    const uint2 e = stack[--sp];
+                    const NifNode* nd = nodes + e.x;
+                    const float4* f4 = reinterpret_cast<const float4*>(nd);
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        const float4 l0 = __ldg(f4 + 2 * a), l1 = __ldg(f4 + 2 * a + 1);
+                        const float4 h0 = __ldg(f4 + 6 + 2 * a), h1 = __ldg(f4 + 6 + 2 * a + 1);
+                        lo[a][0] = l0.x; lo[a][1] = l0.y; lo[a][2] = l0.z; lo[a][3] = l0.w;
+                        lo[a][4] = l1.x; lo[a][5] = l1.y; lo[a][6] = l1.z; lo[a][7] = l1.w;
+                        hi[a][0] = h0.x; hi[a][1] = h0.y; hi[a][2] = h0.z; hi[a][3] = h0.w;
+                        hi[a][4] = h1.x; hi[a][5] = h1.y; hi[a][6] = h1.z; hi[a][7] = h1.w;
+                    }
+                    meta = __ldg(reinterpret_cast<const uint4*>(&nd->mask));
+                } else {
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) { lo[a][c] = 0.0f; hi[a][c] = 0.0f; }
+                }
+                uint32_t key[8];
+                int count = 0;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    key[c] = 0xffffffffu;
+                    if (__any_sync(0xffffffffu, (meta.x >> c) & 1u)) {       // coherent warps skip absent octants
+                        float cn, cf;
+                        const bool ok = slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf) &&
+                                        ((meta.x >> c) & 1u) && !(cn > best_in);
+                        // cn >= 0: its bit pattern orders like an integer; the 3 low mantissa bits make
+                        // room for the octant (t_near only gets smaller: pruning stays conservative).  ~
+                        // turns the ascending network into "farthest first"; rejected children sort last.
+                        if (ok) key[c] = ~((__float_as_uint(cn) & ~7u) | (uint32_t)c);
+                        count += ok ? 1 : 0;
                     }
                 }
-                continue;
-            }
-            const NifNode* nd = nodes + e.x;
-            const float4* f4 = reinterpret_cast<const float4*>(nd);
-            float lo[3][8], hi[3][8];
+#define NIF_CE(i, j) { const uint32_t lo_ = min(key[i], key[j]), hi_ = max(key[i], key[j]); key[i] = lo_; key[j] = hi_; }
+                NIF_CE(0, 1) NIF_CE(2, 3) NIF_CE(4, 5) NIF_CE(6, 7)
+                NIF_CE(0, 2) NIF_CE(1, 3) NIF_CE(4, 6) NIF_CE(5, 7)
+                NIF_CE(1, 2) NIF_CE(5, 6)
+                NIF_CE(0, 4) NIF_CE(1, 5) NIF_CE(2, 6) NIF_CE(3, 7)
+                NIF_CE(2, 4) NIF_CE(3, 5)
+                NIF_CE(1, 2) NIF_CE(3, 4) NIF_CE(5, 6)
+#undef NIF_CE
+                if (count > STACK_MAX - sp) count = STACK_MAX - sp;         // cannot happen for nv <= 512
+                const uint32_t unv = (uint32_t)p.nv;
 #pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                float4 l0 = __ldg(f4 + 2 * a), l1 = __ldg(f4 + 2 * a + 1);
-                float4 h0 = __ldg(f4 + 6 + 2 * a), h1 = __ldg(f4 + 6 + 2 * a + 1);
-                lo[a][0] = l0.x; lo[a][1] = l0.y; lo[a][2] = l0.z; lo[a][3] = l0.w;
-                lo[a][4] = l1.x; lo[a][5] = l1.y; lo[a][6] = l1.z; lo[a][7] = l1.w;
-                hi[a][0] = h0.x; hi[a][1] = h0.y; hi[a][2] = h0.z; hi[a][3] = h0.w;
-                hi[a][4] = h1.x; hi[a][5] = h1.y; hi[a][6] = h1.z; hi[a][7] = h1.w;
+                for (int i = 0; i < 8; ++i) {
+                    if (i < count) {
+                        const uint32_t k = ~key[i], c = k & 7u;
+                        const uint32_t id = meta.y
+                            ? (meta.z + (c & 1u) + unv * (((c >> 1) & 1u) + unv * (c >> 2))) | LEAF_FLAG
+                            : meta.z + (uint32_t)__popc(meta.x & ((1u << c) - 1u));
+                        stack[sp + i] = make_uint2(id, k & ~7u);
+                    }
+                }
+                sp += count;
             }
-            const uint4 c0 = __ldg(reinterpret_cast<const uint4*>(nd->child));
-            const uint4 c1 = __ldg(reinterpret_cast<const uint4*>(nd->child) + 1);
-            const uint2 meta = __ldg(reinterpret_cast<const uint2*>(&nd->mask));
-            const uint32_t child[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
-            const uint32_t leaf = meta.y ? LEAF_FLAG : 0u;
-            const int sp0 = sp;
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                if (!((meta.x >> c) & 1u)) continue;
-                float cn, cf;
-                if (slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf) &&
-                    !(cn > best_in) && sp < STACK_MAX) {
-                    // insertion sort of the new entries, farthest first (nearest ends on top)
-                    int p = sp++;
-                    while (p > sp0 && __uint_as_float(stack[p - 1].y) < cn) { stack[p] = stack[p - 1]; --p; }
-                    stack[p] = make_uint2(child[c] | leaf, __float_as_uint(cn));
+        }
+
+        // ---- phase B: every lane with a voxel on top tests it ------------------------------------
+        if (ray >= 0 && sp > 0) {
+            const uint32_t id = stack[--sp].x & ~LEAF_FLAG;
+            float ti, to;
+            if (voxel_hit(p.lat, p.nv, id, r, ti, to)) {
+                if (ti < best_in || (ti == best_in && (int32_t)id < best_id)) {
+                    best_id = (int32_t)id; best_in = ti; best_out = to;
                 }
             }
+            while (sp > 0 && __uint_as_float(stack[sp - 1].y) > best_in) --sp;
         }
-        out.voxel_id[ray] = best_id;
-        out.t_in[ray] = best_in;
-        out.t_out[ray] = best_out;
-    }
-    const bool hit = active && best_id >= 0;
-    if (flags & NIF_TRAVERSE_ONLY) return;
-    if (active && !hit) {                              // miss: every head output is 0 (R18)
-        out.occlusion[ray] = 0.0f;
-        if (!(flags & NIF_OCCLUSION_ONLY)) {
-            out.distance[ray] = 0.0f; out.dist_total[ray] = 0.0f;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) { out.normal[3 * ray + a] = 0.0f; out.albedo[3 * ray + a] = 0.0f; }
-#pragma unroll
-            for (int a = 0; a < 4; ++a) out.material_logits[4 * ray + a] = 0.0f;
-        }
-        if (out.raw_logits) {
-#pragma unroll
-            for (int a = 0; a < NIF_N_OUT; ++a) out.raw_logits[NIF_N_OUT * ray + a] = 0.0f;
+
+        // ---- retire finished lanes -------------------------------------------------------------------
+        if (ray >= 0 && sp == 0) {
+            retire_ray(p, ray, best_id, best_in, best_out);
+            ray = -1;
         }
     }
-    // hit rays are counted into the bin of the voxel they hit; the returned count is the ray's rank
-    // inside its bin (k_bin_offsets / k_scatter_hits below turn ranks into positions in hit_list)
-    if (hit) {
-        const uint32_t unv = (uint32_t)nv, id = (uint32_t)best_id;
-        const uint32_t ix = id % unv, iy = (id / unv) % unv, iz = id / (unv * unv);
-        const uint32_t bin = (ix >> bin_shift) + (uint32_t)nvb * ((iy >> bin_shift) + (uint32_t)nvb * (iz >> bin_shift));
-        rank[ray] = atomicAdd(&bin_count[bin], 1u);
+}
+
+// One thread per ray, static assignment: the right shape for coherent batches (camera rays), where
+// the 32 rays of a warp walk the same nodes and the loads of a node broadcast.  Absent octants are
+// skipped, hit children are insertion-sorted (farthest first).
+__global__ void __launch_bounds__(TRAV_BLOCK)
+k_traverse_simple(const TravParams p)
+{
+    if (*p.coherent_flag == 0u) return;                   // k_traverse_persistent takes this batch
+    const long long ray = (long long)blockIdx.x * TRAV_BLOCK + threadIdx.x;
+    if (ray >= p.n) return;
+    Ray r;
+    int32_t best_id = -1;
+    float best_in = INFINITY, best_out = INFINITY;
+    r.ox = p.origin[3 * ray]; r.oy = p.origin[3 * ray + 1]; r.oz = p.origin[3 * ray + 2];
+    r.dx = p.dir[3 * ray]; r.dy = p.dir[3 * ray + 1]; r.dz = p.dir[3 * ray + 2];
+    r.ix = __fdiv_rn(1.0f, r.dx); r.iy = __fdiv_rn(1.0f, r.dy); r.iz = __fdiv_rn(1.0f, r.dz);
+    uint2 stack[STACK_MAX];
+    int sp = 0;
+    float bn, bf;
+    if (p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf))
+        stack[sp++] = make_uint2((uint32_t)p.root, __float_as_uint(bn));
+    while (sp > 0) {
+        const uint2 e = stack[--sp];
+        if (__uint_as_float(e.y) > best_in) continue;          // strictly later: cannot win a tie either (R12)
+        if (e.x & LEAF_FLAG) {
+            const uint32_t id = e.x & ~LEAF_FLAG;
+            float ti, to;
+            if (voxel_hit(p.lat, p.nv, id, r, ti, to)) {
+                if (ti < best_in || (ti == best_in && (int32_t)id < best_id)) {
+                    best_id = (int32_t)id; best_in = ti; best_out = to;
+                }
+            }
+            continue;
+        }
+        const NifNode* nd = p.nodes + e.x;
+        const float4* f4 = reinterpret_cast<const float4*>(nd);
+        float lo[3][8], hi[3][8];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const float4 l0 = __ldg(f4 + 2 * a), l1 = __ldg(f4 + 2 * a + 1);
+            const float4 h0 = __ldg(f4 + 6 + 2 * a), h1 = __ldg(f4 + 6 + 2 * a + 1);
+            lo[a][0] = l0.x; lo[a][1] = l0.y; lo[a][2] = l0.z; lo[a][3] = l0.w;
+            lo[a][4] = l1.x; lo[a][5] = l1.y; lo[a][6] = l1.z; lo[a][7] = l1.w;
+            hi[a][0] = h0.x; hi[a][1] = h0.y; hi[a][2] = h0.z; hi[a][3] = h0.w;
+            hi[a][4] = h1.x; hi[a][5] = h1.y; hi[a][6] = h1.z; hi[a][7] = h1.w;
+        }
+        const uint4 c0 = __ldg(reinterpret_cast<const uint4*>(nd->child));
+        const uint4 c1 = __ldg(reinterpret_cast<const uint4*>(nd->child) + 1);
+        const uint2 meta = __ldg(reinterpret_cast<const uint2*>(&nd->mask));
+        const uint32_t child[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+        const uint32_t leaf = meta.y ? LEAF_FLAG : 0u;
+        const int sp0 = sp;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            if (!((meta.x >> c) & 1u)) continue;
+            float cn, cf;
+            if (slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf) &&
+                !(cn > best_in) && sp < STACK_MAX) {
+                int q = sp++;
+                while (q > sp0 && __uint_as_float(stack[q - 1].y) < cn) { stack[q] = stack[q - 1]; --q; }
+                stack[q] = make_uint2(child[c] | leaf, __float_as_uint(cn));
+            }
+        }
+    }
+    retire_ray(p, ray, best_id, best_in, best_out);
+}
+
+// Decides which traversal kernel runs (device-side: nif_query never synchronises).  Sampled groups
+// of 32 consecutive rays vote "coherent" when every direction is within ~8 degrees of the group's
+// first and all origins lie within a tenth of the object's size of each other; the batch is coherent
+// when most groups are.  NIF_TRAVERSE_COHERENT / NIF_TRAVERSE_INCOHERENT override the vote.
+__global__ void __launch_bounds__(256)
+k_ray_coherence(long long n, const float* __restrict__ origin, const float* __restrict__ dir, float extent,
+                int n_groups, unsigned flags, unsigned int* __restrict__ votes, unsigned int* __restrict__ flag_out)
+{
+    const int lane = threadIdx.x & 31;
+    const int g = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    const long long groups_total = (n + 31) / 32;
+    bool coherent = false;
+    if (g < n_groups) {
+        const long long base = 32 * ((groups_total * g) / n_groups);          // evenly spread over the batch
+        const long long i0 = base, i = base + lane < n ? base + lane : n - 1;
+        const float dx = dir[3 * i0], dy = dir[3 * i0 + 1], dz = dir[3 * i0 + 2];
+        const float c = dir[3 * i] * dx + dir[3 * i + 1] * dy + dir[3 * i + 2] * dz;
+        const float ex = origin[3 * i] - origin[3 * i0], ey = origin[3 * i + 1] - origin[3 * i0 + 1],
+                    ez = origin[3 * i + 2] - origin[3 * i0 + 2];
+        const bool ok = c > 0.99f && (ex * ex + ey * ey + ez * ez) <= 0.01f * extent * extent;
+        coherent = __all_sync(0xffffffffu, ok);
+        if (lane == 0 && coherent) atomicAdd(&votes[0], 1u);
+    }
+    __threadfence();
+    __syncthreads();
+    // last block to finish publishes the decision
+    __shared__ bool last;
+    if (threadIdx.x == 0) last = atomicAdd(&votes[1], 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        const unsigned yes = atomicAdd(&votes[0], 0u);
+        unsigned decision = 2u * yes > (unsigned)n_groups ? 1u : 0u;
+        if (flags & NIF_TRAVERSE_COHERENT) decision = 1u;
+        if (flags & NIF_TRAVERSE_INCOHERENT) decision = 0u;
+        *flag_out = decision;
     }
 }
 
@@ -280,12 +479,33 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
                         const NifQueryWs* ws, unsigned flags, cudaStream_t stream)
 {
     if (rays->n == 0) return NIF_OK;
-    const long long blocks = (rays->n + TRAV_BLOCK - 1) / TRAV_BLOCK;
-    k_traverse<<<(unsigned)blocks, TRAV_BLOCK, 0, stream>>>(
-        bvh->nodes, bvh->lattice, bvh->nv, bvh->root, bvh->lo[0], bvh->lo[1], bvh->lo[2],
-        bvh->hi[0], bvh->hi[1], bvh->hi[2], (long long)rays->n, rays->origin, rays->dir, *out,
-        ws->bin_count, ws->rank, ws->bin_shift, ws->nvb, flags);
-    nif_count_launch(1);
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        NIF_CUDA_TRY(cudaGetDevice(&dev));
+        NIF_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    TravParams p;
+    p.nodes = bvh->nodes; p.lat = bvh->lattice; p.nv = bvh->nv; p.root = bvh->root;
+    p.rlx = bvh->lo[0]; p.rly = bvh->lo[1]; p.rlz = bvh->lo[2];
+    p.rhx = bvh->hi[0]; p.rhy = bvh->hi[1]; p.rhz = bvh->hi[2];
+    p.n = (long long)rays->n; p.origin = rays->origin; p.dir = rays->dir; p.out = *out;
+    p.ray_counter = &ws->scratch->tile_counter;
+    p.bin_count = ws->bin_count; p.rank = ws->rank; p.bin_shift = ws->bin_shift; p.nvb = ws->nvb;
+    p.flags = flags;
+    p.coherent_flag = &ws->scratch->pad[0];
+    // scratch header (zeroed by nif_query): pad[0] decision, pad[1] coherent votes, pad[2] finished blocks
+    const long long groups_total = (rays->n + 31) / 32;
+    const int n_groups = (int)(groups_total < 2048 ? groups_total : 2048);
+    float extent = 0.0f;
+    for (int a = 0; a < 3; ++a) extent = fmaxf(extent, bvh->hi[a] - bvh->lo[a]);
+    k_ray_coherence<<<(n_groups * 32 + 255) / 256, 256, 0, stream>>>(
+        (long long)rays->n, rays->origin, rays->dir, extent, n_groups, flags, &ws->scratch->pad[1], &ws->scratch->pad[0]);
+    const long long want = (rays->n + TRAV_BLOCK - 1) / TRAV_BLOCK;
+    const long long cap = (long long)n_sm * TRAV_BLOCKS_PER_SM;
+    k_traverse_simple<<<(unsigned)want, TRAV_BLOCK, 0, stream>>>(p);
+    k_traverse_persistent<<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
+    nif_count_launch(3);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;
 }

@@ -166,3 +166,20 @@ def test_traversal_reduced_configs_all_rays(oracle, H, P, cfg_id, n, pose_index)
     m = P.compare_traversal(gpu, ref)
     P.assert_traversal(m)
     assert m["n_hit"] > 1000, m
+
+
+@pytest.mark.parametrize("cfg_id,pose_index,n", [(1, 0, 60_000), (3, 2, 40_000), (0, 0, None)])
+def test_both_traversal_kernels_agree_bit_for_bit(oracle, H, P, cfg_id, pose_index, n):
+    # the per-thread kernel (coherent batches) and the persistent while-while kernel (incoherent
+    # batches) implement the same definition; the device-side vote only picks the faster one
+    import paper_2604_24666_b200 as nif
+    case = H.make_case(cfg_id, n_rays=n, pose_index=pose_index, with_net=False)
+    res = {}
+    for name, fl in (("auto", 0), ("coherent", nif.NIF_TRAVERSE_COHERENT), ("incoherent", nif.NIF_TRAVERSE_INCOHERENT)):
+        res[name] = H.run_gpu(case, flags=nif.NIF_TRAVERSE_ONLY | fl, raw_logits=False)
+    for k in ("voxel_id", "t_in", "t_out"):
+        a, b, c = (res[m][k].view(np.int32) for m in ("auto", "coherent", "incoherent"))
+        assert np.array_equal(a, b) and np.array_equal(b, c), k
+    side = H.OracleSide(oracle, case)
+    idx = np.arange(0, len(case.origin), max(1, len(case.origin) // 4000))
+    P.assert_traversal(P.compare_traversal(H.subset(res["incoherent"], idx), side.query(idx, traverse_only=True)))
