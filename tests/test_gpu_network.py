@@ -155,3 +155,37 @@ def test_full_size_configs_sampled(oracle, H, P, nif, cfg_id, pose_index, n_trav
         assert (gpu["distance"][h] >= 0).all() and (gpu["distance"][h] <= ell * (1 + 1e-6) + 1e-12).all()
         np.testing.assert_allclose(np.linalg.norm(gpu["normal"][h], axis=1), 1.0, atol=1e-5)
         assert not gpu["normal"][~h].any() and not gpu["material_logits"][~h].any()
+
+
+SHAPES = [  # (pe_bands, levels, log2_T, feat, base_res, growth, hidden_layers, width)
+    (2, 8, 14, 2, 8, 1.5, 1, 32),      # smallest tensor-core shape: L*F = 16, one hidden layer, W = 32
+    (3, 4, 12, 4, 4, 2.0, 2, 32),      # F = 4, L*F = 16
+    (1, 16, 15, 4, 8, 1.3, 3, 64),     # L*F = 64: one sample per K chunk
+    (5, 4, 13, 2, 16, 1.7, 5, 128),    # L*F = 8, W = 128, deep
+    (0, 16, 16, 2, 16, 1.38, 2, 64),   # no positional bands: S = 1, a single (padded) K chunk per endpoint pair
+]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_tensor_core_kernel_shape_sweep(oracle, H, P, nif, shape):
+    """Every template instantiation / chunking case of the fused kernel against the oracle."""
+    b, L, t, f, base, growth, hl, w = shape
+    net = I.NetShape(pe_bands=b, levels=L, log2_T=t, feat=f, base_res=base, growth=growth,
+                     hidden_layers=hl, width=w, dtype="f16")
+    cfg = I.scaled(I.get_config(1), net=net)
+    case = H.make_case(1, n_rays=12_000, cfg=cfg)
+    assert nif.nif_net_uses_tensor_cores(case.net)
+    ref = H.OracleSide(oracle, case).query()
+    for name, fl in _engines(nif, case):
+        gpu = H.run_gpu(case, flags=fl)
+        P.assert_traversal(P.compare_traversal(gpu, ref))
+        m = P.compare_network(gpu, ref, fp16=True)
+        P.assert_network(m, fp16=True)
+        assert m["n_hit"] > 500, (name, m)
+
+
+def test_empty_batch_is_a_no_op(H, nif):
+    case = H.make_case(0, n_rays=16)
+    out = nif.alloc_outputs(0)
+    nif.nif_query(case.bvh, case.net, case.origin_d[:0].contiguous(), case.direction_d[:0].contiguous(), out)
+    torch.cuda.synchronize()
