@@ -293,6 +293,20 @@ def run_ours(args) -> None:
     ms_per_step = elapsed_ms / args.steps
     value = world * n_total / (ms_per_step * 1e-3) / 1e6
 
+    # ---- MLP-only probe: same kernel, gathers replaced by a constant A operand (outside the timed region)
+    mlp_probe = None
+    if rank == 0 and nif.nif_net_uses_tensor_cores(net) and not (flags & nif.NIF_ENGINE_FFMA):
+        nif.nif_profile_enable(True)
+        for _ in range(5):
+            for p in poses:
+                ws = nif.nif_query(p["bvh"], net, p["o"], p["d"], out, workspace=ws, flags=flags | nif.NIF_PROBE_SKIP_GATHER)
+        pr = nif.nif_profile_read()
+        nif.nif_profile_enable(False)
+        mlp_probe = pr["network_ms"] / max(pr["n_queries"], 1)
+        for p in poses:                                # leave real results in `out`
+            ws = nif.nif_query(p["bvh"], net, p["o"], p["d"], out, workspace=ws, flags=flags)
+        torch.cuda.synchronize()
+
     # ---- e2e: same metric through nif_query_host (pinned host buffers, copies timed) ---------
     stage = nif.Stage(args.chunk)
     out_h = nif.alloc_outputs(n_per_pose, pinned_host=True)
@@ -348,6 +362,13 @@ def run_ours(args) -> None:
                         / ((net_ms + trav_ms) * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "peak_source": f"{peaks['source']} copy bandwidth"}}
     roofline["hbm"]["frac"] = roofline["hbm"]["achieved"] / peaks["hbm_gbs"]
+    if mlp_probe:
+        tf = hits_per_launch * work["mlp_flops_per_hit_ray"] / (mlp_probe * 1e-3) / 1e12
+        roofline["tensor_mlp_only_probe"] = {
+            "what": "same kernel with NIF_PROBE_SKIP_GATHER: constant A operand, no table gathers; MLP flops of "
+                    "the real network / event-timed kernel duration", "avg_launch_ms": mlp_probe,
+            "achieved": tf, "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": tf / peaks["tf_burst"],
+            "peak_source": f"{peaks['source']} bf16 burst (fp16 same pipe)"}
     kernels = {"traverse_ms": trav_ms, "encode_mlp_ms": net_ms, "traverse_share": trav_ms * cfg.n_poses / ms_per_step,
                "bvh_build_ms_per_pose": float(np.median(build_ms))}
 

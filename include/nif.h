@@ -55,7 +55,11 @@ enum {
      * batches).  By default a device-side vote over sampled ray groups picks one; these force it.
      * Results are identical either way. */
     NIF_TRAVERSE_COHERENT   = 8u,
-    NIF_TRAVERSE_INCOHERENT = 16u
+    NIF_TRAVERSE_INCOHERENT = 16u,
+    /* Diagnostic: the tensor-core kernel fills its A operand with a constant instead of gathering from
+     * the table, so a timed query measures the tcgen05 MLP pipeline alone (head outputs are then
+     * meaningless).  bench.py --probe-mlp reports the tensor-pipe rate it reaches. */
+    NIF_PROBE_SKIP_GATHER   = 32u
 };
 
 #define NIF_N_OUT 12   /* logits per ray: occlusion 1, distance 1, normal 3, albedo 3, material 4 (B:7) */

@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libnif.so"
 
 NIF_F32, NIF_F16 = 0, 1
 NIF_OCCLUSION_ONLY, NIF_ENGINE_FFMA, NIF_TRAVERSE_ONLY = 1, 2, 4
-NIF_TRAVERSE_COHERENT, NIF_TRAVERSE_INCOHERENT = 8, 16
+NIF_TRAVERSE_COHERENT, NIF_TRAVERSE_INCOHERENT, NIF_PROBE_SKIP_GATHER = 8, 16, 32
 NIF_N_OUT = 12
 
 

@@ -548,7 +548,11 @@ k_fused_encode_mlp(const TcParams p)
                 const uint32_t row = (uint32_t)(g * 32 + lane);
                 const uint32_t a_stage = s_a + stage * STAGE_BYTES;
                 const uint32_t unit0 = (uint32_t)(esl * units_per_es);
-                if (es < p.n_es) {
+                if (p.flags & NIF_PROBE_SKIP_GATHER) {
+                    // diagnostic: synthetic features, no table access -- times the MLP pipeline alone
+                    for (int u = 0; u < units_per_es; ++u)
+                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), 0x2c002c00u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u);
+                } else if (es < p.n_es) {
                     const int e = es >= S ? 1 : 0, s = es - e * S;
                     const float* rb = ray_buf + ((size_t)b * TC_TILE + row) * 8 + 3 * e;
                     const float px = nif_pe_sample(rb[0], s), py = nif_pe_sample(rb[1], s), pz = nif_pe_sample(rb[2], s);
