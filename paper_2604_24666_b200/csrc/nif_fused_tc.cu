@@ -67,21 +67,20 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
             "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
     } while (!done);
 }
-// wait for the role warps whose waits are long (a whole tile of gathers): poll, then sleep between polls
-// so that the spin loop does not take issue slots from the gather warps
-__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, unsigned ns)
+// wait for the role warps whose waits are long (a whole tile of gathers): try_wait with a suspend-time
+// hint parks the thread in hardware until the phase completes or the hint expires, so the wait takes
+// (almost) no issue slots from the gather warps and still wakes up as soon as the barrier flips
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, unsigned hint_ns)
 {
-    for (;;) {
-        uint32_t done;
+    uint32_t done;
+    do {
         asm volatile(
             "{\n\t"
             ".reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
             "selp.u32 %0, 1, 0, p;\n\t"
-            "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-        if (done) break;
-        __nanosleep(ns);
-    }
+            "}" : "=r"(done) : "r"(bar), "r"(parity), "r"(hint_ns) : "memory");
+    } while (!done);
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -403,7 +402,7 @@ k_fused_encode_mlp(const TcParams p)
             tc_fence_after();
             for (int kc = 0; kc < KC; ++kc, ++hq) {
                 const uint32_t slot = hq % TC_HSLOTS;
-                mbar_wait_sleep(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u, 32);
+                mbar_wait_sleep(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u, 20000);
                 tc_fence_after();
                 issue_layer_chunk<W>(d_tmem, s_act, s_w + slot * HCHUNK, N, kc);
                 umma_commit(bar(BAR_HEMPTY + slot));
@@ -412,7 +411,7 @@ k_fused_encode_mlp(const TcParams p)
         };
         auto prepare = [&](int j) {                       // rest-space endpoints of tile j -> ray_buf[j&1]
             const int b = j & 1;
-            mbar_wait_sleep(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 128);
+            mbar_wait_sleep(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 20000);
             const long long tile = (long long)blockIdx.x + (long long)j * gridDim.x;
             const long long h = tile * TC_TILE + r;
             float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f;
@@ -437,7 +436,7 @@ k_fused_encode_mlp(const TcParams p)
             if (j + 1 < n_my) prepare(j + 1);
             const int b = j & 1;
             // layer 1 accumulator of tile j
-            mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1), 256);
+            mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1), 20000);
             tc_fence_after();
             drain_relu_to_act<W>(tm_acc1 + (uint32_t)(b * W) + t_row, s_act, (uint32_t)r);
             tc_fence_before();
@@ -447,7 +446,7 @@ k_fused_encode_mlp(const TcParams p)
             // hidden layers 2..H
             for (int hl = 1; hl < p.hidden_layers; ++hl) {
                 if (tid == 0) run_layer(tm_hid, W);
-                mbar_wait_sleep(bar(BAR_HID), hid_phase, 32); hid_phase ^= 1u;
+                mbar_wait_sleep(bar(BAR_HID), hid_phase, 20000); hid_phase ^= 1u;
                 tc_fence_after();
                 drain_relu_to_act<W>(tm_hid + t_row, s_act, (uint32_t)r);
                 tc_fence_before();
@@ -456,7 +455,7 @@ k_fused_encode_mlp(const TcParams p)
             }
             // output layer (12 heads padded to N = 16) and (a5) decode
             if (tid == 0) run_layer(tm_out, TC_NOUT_PAD);
-            mbar_wait_sleep(bar(BAR_HID), hid_phase, 32); hid_phase ^= 1u;
+            mbar_wait_sleep(bar(BAR_HID), hid_phase, 20000); hid_phase ^= 1u;
             tc_fence_after();
             uint32_t zr[16];
             __syncwarp();
@@ -477,11 +476,11 @@ k_fused_encode_mlp(const TcParams p)
             uint32_t q = 0;
             for (int j = 0; j < n_my; ++j) {
                 const int b = j & 1;
-                mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 64);
+                mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 20000);
                 tc_fence_after();
                 for (int c = 0; c < n_chunks; ++c, ++q) {
                     const uint32_t stage = q % TC_STAGES;
-                    mbar_wait_sleep(bar(BAR_FULL + stage), (q / TC_STAGES) & 1u, 64);
+                    mbar_wait_sleep(bar(BAR_FULL + stage), (q / TC_STAGES) & 1u, 20000);
                     tc_fence_after();
                     const uint32_t a0 = s_a + stage * STAGE_BYTES, b0 = a0 + TC_A_CHUNK_BYTES;
 #pragma unroll
@@ -503,7 +502,7 @@ k_fused_encode_mlp(const TcParams p)
             for (int j = 0; j < n_my; ++j)
                 for (int c = 0; c < n_chunks; ++c, ++q) {
                     const uint32_t stage = q % TC_STAGES;
-                    mbar_wait_sleep(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u, 128);
+                    mbar_wait_sleep(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u, 20000);
                     mbar_expect_tx(bar(BAR_FULL + stage), W1_CHUNK);
                     bulk_g2s(s_a + stage * STAGE_BYTES + TC_A_CHUNK_BYTES, p.w_img + (size_t)c * W1_CHUNK, W1_CHUNK,
                              bar(BAR_FULL + stage));
@@ -521,7 +520,7 @@ k_fused_encode_mlp(const TcParams p)
                     const uint8_t* src = wh + (size_t)(l - 1) * (size_t)(KC * HCHUNK);
                     for (int kc = 0; kc < KC; ++kc, ++hq) {
                         const uint32_t slot = hq % TC_HSLOTS;
-                        mbar_wait_sleep(bar(BAR_HEMPTY + slot), ((hq / TC_HSLOTS) & 1u) ^ 1u, 128);
+                        mbar_wait_sleep(bar(BAR_HEMPTY + slot), ((hq / TC_HSLOTS) & 1u) ^ 1u, 20000);
                         mbar_expect_tx(bar(BAR_HFULL + slot), bytes);
                         bulk_g2s(s_w + slot * HCHUNK, src + (size_t)kc * bytes, bytes, bar(BAR_HFULL + slot));
                     }
