@@ -190,6 +190,7 @@ struct TcParams {
     const float* dir;
     nif_query_out out;
     const NifQueryScratch* scratch;
+    unsigned int* tile_counter;   // dynamic tile scheduler (scratch header, zeroed per query)
     const int32_t* hit_list;
     unsigned flags;
 };
@@ -354,7 +355,7 @@ k_fused_encode_mlp(const TcParams p)
     const uint32_t s_bar = smem_base + SL.bars;
     uint32_t* s_tmem_ptr = reinterpret_cast<uint32_t*>(smem_gen + SL.bars + 240);
     TcLevel* s_lvl = reinterpret_cast<TcLevel*>(smem_gen + SL.bars + 256);      // 16 levels x 16 B, 16-byte aligned
-    static_assert(8 * BAR_COUNT <= 240, "barrier block overlaps the TMEM pointer slot");
+    static_assert(8 * BAR_COUNT <= 224, "barrier block overlaps the tile-id / TMEM pointer slots");
     auto bar = [&](int i) { return s_bar + 8u * (uint32_t)i; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -390,7 +391,9 @@ k_fused_encode_mlp(const TcParams p)
 
     const long long n_hit = (long long)p.scratch->n_hit;
     const long long n_tiles = (n_hit + TC_TILE - 1) / TC_TILE;
-    const int n_my = (int)((n_tiles > (long long)blockIdx.x) ? (n_tiles - 1 - blockIdx.x) / gridDim.x + 1 : 0);
+    // dynamic tile scheduler: row thread 0 draws tile ids from a global counter in prepare() and
+    // publishes them in s_tile[j & 1] (-1 = no more tiles); every role reads them after ray_full[j & 1]
+    volatile int* s_tile = reinterpret_cast<volatile int*>(smem_gen + SL.bars + 224);
 
     if (warp < TC_ROW_WARPS) {
         // ======================= row warps: (a2) for the next tile, MLP tail + (a5) ==============
@@ -409,11 +412,17 @@ k_fused_encode_mlp(const TcParams p)
             }
             umma_commit(bar(BAR_HID));
         };
-        auto prepare = [&](int j) {                       // rest-space endpoints of tile j -> ray_buf[j&1]
+        int nxt_tile = -1;
+        auto prepare = [&](int j) {                       // rest-space endpoints of the j-th tile -> ray_buf[j&1]
             const int b = j & 1;
             mbar_wait_sleep(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 20000);
-            const long long tile = (long long)blockIdx.x + (long long)j * gridDim.x;
-            const long long h = tile * TC_TILE + r;
+            if (tid == 0) {
+                const unsigned t = atomicAdd(p.tile_counter, 1u);
+                s_tile[b] = (long long)t < n_tiles ? (int)t : -1;
+            }
+            row_bar_sync();
+            nxt_tile = s_tile[b];
+            const long long h = nxt_tile < 0 ? n_hit : (long long)nxt_tile * TC_TILE + r;
             float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f;
             nxt_ray = -1; nxt_ti = 0.f; nxt_to = 0.f;
             if (h < n_hit) {
@@ -429,11 +438,12 @@ k_fused_encode_mlp(const TcParams p)
             rb[3] = nif_normalise(xo); rb[4] = nif_normalise(yo); rb[5] = nif_normalise(zo);
             mbar_arrive(bar(BAR_RAY_FULL + b));
         };
-        if (n_my > 0) prepare(0);
+        prepare(0);
         const uint32_t t_row = (uint32_t)(warp * 32) << 16;          // this warp's TMEM lane quarter
-        for (int j = 0; j < n_my; ++j) {
+        for (int j = 0;; ++j) {
+            if (nxt_tile < 0) break;
             cur_ray = nxt_ray; cur_ti = nxt_ti; cur_to = nxt_to;
-            if (j + 1 < n_my) prepare(j + 1);
+            prepare(j + 1);
             const int b = j & 1;
             // layer 1 accumulator of tile j
             mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1), 20000);
@@ -471,11 +481,13 @@ k_fused_encode_mlp(const TcParams p)
         }
     } else if (warp == TC_MMA_WARP) {
         // ======================= layer-1 MMA issuer =============================================
-        if (lane == 0 && n_my > 0) {
+        if (lane == 0) {
             const uint32_t idesc = idesc_f16(TC_TILE, W);
             uint32_t q = 0;
-            for (int j = 0; j < n_my; ++j) {
+            for (int j = 0;; ++j) {
                 const int b = j & 1;
+                mbar_wait_sleep(bar(BAR_RAY_FULL + b), (uint32_t)((j >> 1) & 1), 20000);
+                if (s_tile[b] < 0) break;
                 mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 20000);
                 tc_fence_after();
                 for (int c = 0; c < n_chunks; ++c, ++q) {
@@ -499,7 +511,9 @@ k_fused_encode_mlp(const TcParams p)
         if (lane == 0) {
             constexpr uint32_t W1_CHUNK = (uint32_t)W * 128u;
             uint32_t q = 0;
-            for (int j = 0; j < n_my; ++j)
+            for (int j = 0;; ++j) {
+                mbar_wait_sleep(bar(BAR_RAY_FULL + (j & 1)), (uint32_t)((j >> 1) & 1), 20000);
+                if (s_tile[j & 1] < 0) break;
                 for (int c = 0; c < n_chunks; ++c, ++q) {
                     const uint32_t stage = q % TC_STAGES;
                     mbar_wait_sleep(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u, 20000);
@@ -507,13 +521,16 @@ k_fused_encode_mlp(const TcParams p)
                     bulk_g2s(s_a + stage * STAGE_BYTES + TC_A_CHUNK_BYTES, p.w_img + (size_t)c * W1_CHUNK, W1_CHUNK,
                              bar(BAR_FULL + stage));
                 }
+            }
         } else if (lane == 1) {
             // hidden layers 2..H and the output layer: KC chunks each, per tile, in the order the row
             // warps consume them (they are small, so they share one 2-slot ring instead of living in smem)
             const uint8_t* wh = p.w_img + p.w1_bytes;
             const uint32_t out_chunk = TC_NOUT_PAD * 128u;
             uint32_t hq = 0;
-            for (int j = 0; j < n_my; ++j)
+            for (int j = 0;; ++j) {
+                mbar_wait_sleep(bar(BAR_RAY_FULL + (j & 1)), (uint32_t)((j >> 1) & 1), 20000);
+                if (s_tile[j & 1] < 0) break;
                 for (int l = 1; l <= p.hidden_layers; ++l) {
                     const bool is_out = l == p.hidden_layers;
                     const uint32_t bytes = is_out ? out_chunk : HCHUNK;
@@ -525,6 +542,7 @@ k_fused_encode_mlp(const TcParams p)
                         bulk_g2s(s_w + slot * HCHUNK, src + (size_t)kc * bytes, bytes, bar(BAR_HFULL + slot));
                     }
                 }
+            }
         }
     } else {
         // ======================= gather warps: (a3) encode into the A ring ======================
@@ -532,9 +550,10 @@ k_fused_encode_mlp(const TcParams p)
         const int items_per_chunk = 4 * epc;
         const int items_per_tile = items_per_chunk * n_chunks;
         const int units_per_es = (L * F) / 8;                          // 16-byte units one sample fills
-        for (int j = 0; j < n_my; ++j) {
+        for (int j = 0;; ++j) {
             const int b = j & 1;
             mbar_wait(bar(BAR_RAY_FULL + b), (uint32_t)((j >> 1) & 1));
+            if (s_tile[b] < 0) break;
             const long long gi0 = (long long)j * items_per_tile;
             const int first = (int)(((long long)gw - gi0 % TC_GATHER_WARPS + TC_GATHER_WARPS) % TC_GATHER_WARPS);
             for (int i = first; i < items_per_tile; i += TC_GATHER_WARPS) {
@@ -692,7 +711,7 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     p.w_img = (const uint8_t*)net->w_tc; p.w_bytes = s.w_bytes; p.w1_bytes = s.w1_bytes;
     p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
     p.origin = rays->origin; p.dir = rays->dir;
-    p.out = *out; p.scratch = scratch; p.hit_list = hit_list; p.flags = flags;
+    p.out = *out; p.scratch = scratch; p.tile_counter = &scratch->pad[4]; p.hit_list = hit_list; p.flags = flags;
     p.stages = tc_pick_stages(d->width);
     const uint32_t smem = tc_smem_layout(p.stages, d->width).total;
     static int n_sm = 0;
