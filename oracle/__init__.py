@@ -78,6 +78,12 @@ class Oracle:
                                   C.POINTER(_NetDesc), C.c_void_p, C.c_void_p, C.c_int64,
                                   C.c_void_p, C.c_void_p, C.c_uint32] + [C.c_void_p] * 10)
         L.nifo_rest_endpoints.argtypes = [C.c_float, C.c_float, C.c_int64] + [C.c_void_p] * 6
+        L.nifo_next_voxel_brute.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 7
+        L.nifo_next_voxel_bvh.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 7
+        L.nifo_query_multi.restype = C.c_int
+        L.nifo_query_multi.argtypes = ([C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float,
+                                        C.POINTER(_NetDesc), C.c_void_p, C.c_void_p, C.c_int64,
+                                        C.c_void_p, C.c_void_p, C.c_uint32, C.c_int] + [C.c_void_p] * 13)
         self.acc_bytes = L.nifo_acc_bytes()
 
     # ---- deformation -----------------------------------------------------------------
@@ -212,6 +218,46 @@ class Oracle:
         return o
 
 
+    def next_voxel_brute(self, nv, occ, lattice, origin, direction, after_t, after_id):
+        """O11 definition: successor of (after_t, after_id) in each ray's (t_in, id)-ordered voxel sequence."""
+        origin = _f32(origin); direction = _f32(direction)
+        at = _f32(after_t); ai = np.ascontiguousarray(after_id, dtype=np.int32)
+        n = len(origin)
+        vid = np.empty(n, np.int32); ti = np.empty(n, np.float32); to = np.empty(n, np.float32)
+        self.lib.nifo_next_voxel_brute(nv, occ.ctypes.data, lattice.ctypes.data, n, origin.ctypes.data,
+                                       direction.ctypes.data, at.ctypes.data, ai.ctypes.data,
+                                       vid.ctypes.data, ti.ctypes.data, to.ctypes.data)
+        return vid, ti, to
+
+    def query_multi(self, nv, occ, lattice, bvh, pose, params, origin, direction, max_steps,
+                    occlusion_only=False):
+        """O11: multi-voxel walk; returns the single-voxel outputs of the accepted (or last) voxel plus
+        status / steps / dist_accum (the literal P:61 sum)."""
+        origin = _f32(origin); direction = _f32(direction)
+        n = len(origin)
+        d = self._desc(params.shape, params.level_res)
+        table = _f32(params.table)
+        ws, arr = self._wptrs(params.weights)
+        o = {"voxel_id": np.empty(n, np.int32), "t_in": np.empty(n, np.float32), "t_out": np.empty(n, np.float32),
+             "occlusion": np.zeros(n, np.float32), "distance": np.zeros(n, np.float32),
+             "dist_total": np.zeros(n, np.float32), "normal": np.zeros((n, 3), np.float32),
+             "albedo": np.zeros((n, 3), np.float32), "material_logits": np.zeros((n, 4), np.float32),
+             "raw_logits": np.zeros((n, N_OUT), np.float32), "status": np.zeros(n, np.int32),
+             "steps": np.zeros(n, np.int32), "dist_accum": np.zeros(n, np.float32)}
+        rc = self.lib.nifo_query_multi(nv, occ.ctypes.data, lattice.ctypes.data,
+                                       bvh.handle if bvh is not None else None,
+                                       float(pose[0]), float(pose[1]), C.byref(d), table.ctypes.data, arr,
+                                       n, origin.ctypes.data, direction.ctypes.data,
+                                       FLAG_OCCLUSION_ONLY if occlusion_only else 0, int(max_steps),
+                                       *[o[k].ctypes.data for k in ("voxel_id", "t_in", "t_out", "occlusion",
+                                                                    "distance", "dist_total", "normal", "albedo",
+                                                                    "material_logits", "raw_logits", "status",
+                                                                    "steps", "dist_accum")])
+        if rc != 0:
+            raise RuntimeError(f"nifo_query_multi failed: {rc}")
+        return o
+
+
 class OracleBVH:
     def __init__(self, oracle: Oracle, nv, occ, lattice):
         self.oracle = oracle
@@ -234,6 +280,16 @@ class OracleBVH:
         vid = np.empty(n, np.int32); ti = np.empty(n, np.float32); to = np.empty(n, np.float32)
         self.oracle.lib.nifo_traverse_bvh(self.handle, n, origin.ctypes.data, direction.ctypes.data,
                                           vid.ctypes.data, ti.ctypes.data, to.ctypes.data)
+        return vid, ti, to
+
+    def next_voxel(self, origin, direction, after_t, after_id):
+        origin = _f32(origin); direction = _f32(direction)
+        at = _f32(after_t); ai = np.ascontiguousarray(after_id, dtype=np.int32)
+        n = len(origin)
+        vid = np.empty(n, np.int32); ti = np.empty(n, np.float32); to = np.empty(n, np.float32)
+        self.oracle.lib.nifo_next_voxel_bvh(self.handle, n, origin.ctypes.data, direction.ctypes.data,
+                                            at.ctypes.data, ai.ctypes.data, vid.ctypes.data, ti.ctypes.data,
+                                            to.ctypes.data)
         return vid, ti, to
 
     def __del__(self):

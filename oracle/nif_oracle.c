@@ -296,6 +296,41 @@ void nifo_traverse_brute(int nv, const uint8_t* occ, const float* lattice, int64
     }
 }
 
+/* `after_t`, `after_id`: only voxels whose (t_in, id) is lexicographically GREATER than
+   (after_t, after_id) are candidates -- the successor query of the multi-voxel walk (O11).
+   (-INFINITY, -1) = no bound = the plain first-hit query. */
+static int after_bound(float ti, int32_t id, float after_t, int32_t after_id)
+{
+    return (ti > after_t) || (ti == after_t && id > after_id);
+}
+
+/* O11 (definition)  Successor of (after_t, after_id) in the ray's sequence of hit voxels ordered by
+   (t_in, id): the voxel the walk of P:51 moves to next ("explicitly determining the voxel face
+   through which a ray exits, which allows correct selection of neighboring voxels"); gaps of empty
+   voxels are skipped because only occupied voxels are candidates.  Brute force. */
+void nifo_next_voxel_brute(int nv, const uint8_t* occ, const float* lattice, int64_t n,
+                           const float* origin, const float* dir, const float* after_t,
+                           const int32_t* after_id, int32_t* vid, float* t_in, float* t_out)
+{
+    for (int64_t r = 0; r < n; ++r) {
+        const float* o = origin + 3 * r; const float* d = dir + 3 * r;
+        float inv[3]; ray_inv(d, inv);
+        int32_t best = -1; float bti = INFINITY, bto = INFINITY;
+        for (int iz = 0; iz < nv; ++iz)
+            for (int iy = 0; iy < nv; ++iy)
+                for (int ix = 0; ix < nv; ++ix) {
+                    int32_t id = ix + nv * (iy + nv * iz);
+                    if (!occ[id]) continue;
+                    float ti, to;
+                    if (voxel_hit(lattice, nv, ix, iy, iz, o, d, inv, &ti, &to) &&
+                        after_bound(ti, id, after_t[r], after_id[r]) && ti < bti) {
+                        best = id; bti = ti; bto = to;
+                    }
+                }
+        vid[r] = best; t_in[r] = bti; t_out[r] = bto;
+    }
+}
+
 /* ------------------------------------------------------------------------------------ */
 /* O6 (large inputs)  The oracle's own "simple BVH": binary, median split on   */
 /* the longest axis of the voxel-box centres, leaves of <= 4 voxels, node box = exact      */
@@ -410,8 +445,8 @@ void nifo_bvh_bounds(const void* h, float lo[3], float hi[3])
     }
 }
 
-static void traverse_bvh_one(const obvh* b, const float* o, const float* d,
-                             int32_t* vid, float* t_in, float* t_out)
+static void traverse_bvh_after(const obvh* b, const float* o, const float* d, float after_t, int32_t after_id,
+                               int32_t* vid, float* t_in, float* t_out)
 {
     float inv[3]; ray_inv(d, inv);
     int32_t best = -1; float bti = INFINITY, bto = INFINITY;
@@ -431,7 +466,8 @@ static void traverse_bvh_one(const obvh* b, const float* o, const float* d,
                 int32_t id = b->vox[i];
                 int ix = id % nv, iy = (id / nv) % nv, iz = id / (nv * nv);
                 float ti, to;
-                if (voxel_hit(b->lattice, nv, ix, iy, iz, o, d, inv, &ti, &to)) {
+                if (voxel_hit(b->lattice, nv, ix, iy, iz, o, d, inv, &ti, &to) &&
+                    after_bound(ti, id, after_t, after_id)) {
                     if (ti < bti || (ti == bti && id < best)) { best = id; bti = ti; bto = to; }
                 }
             }
@@ -447,6 +483,20 @@ static void traverse_bvh_one(const obvh* b, const float* o, const float* d,
         else if (hr)   { stack[sp] = nd->right; stack_t[sp++] = rn; }
     }
     *vid = best; *t_in = bti; *t_out = bto;
+}
+
+static void traverse_bvh_one(const obvh* b, const float* o, const float* d,
+                             int32_t* vid, float* t_in, float* t_out)
+{
+    traverse_bvh_after(b, o, d, -INFINITY, -1, vid, t_in, t_out);
+}
+
+void nifo_next_voxel_bvh(const void* h, int64_t n, const float* origin, const float* dir,
+                         const float* after_t, const int32_t* after_id, int32_t* vid, float* t_in, float* t_out)
+{
+    const obvh* b = (const obvh*)h;
+    for (int64_t r = 0; r < n; ++r)
+        traverse_bvh_after(b, origin + 3 * r, dir + 3 * r, after_t[r], after_id[r], vid + r, t_in + r, t_out + r);
 }
 
 void nifo_traverse_bvh(const void* h, int64_t n, const float* origin, const float* dir,
@@ -629,6 +679,62 @@ void nifo_decode(int64_t n, const float* logits, const float* t_in, const float*
 /* `bvh` may be NULL: then the brute-force definition is used.                             */
 /* Network outputs may be NULL to run traversal only.                                      */
 /* ------------------------------------------------------------------------------------ */
+/* O7-O10 for ONE ray whose voxel (id, ti, to) is known: entry/exit points -> inverse deformation ->
+   normalise -> psi(entry) ++ psi(exit) -> MLP -> heads, written to the pointers given (each
+   pointing at this ray's slot; optional ones may be NULL). */
+static void nifo_eval_voxel(float theta_max, float bend_k, const nifo_net_desc* nd, const float* table,
+                            const float* const* weights, const float* o, const float* d, uint32_t flags,
+                            int32_t id, float ti, float to,
+                            int32_t* vid, float* t_in, float* t_out,
+                            float* occlusion, float* distance, float* dist_total,
+                            float* normal, float* albedo, float* material, float* raw_logits)
+{
+    int S = 1 + 2 * nd->pe_bands;
+    int per = S * nd->levels * nd->feat, d_in = 2 * per;
+    int n_out = (flags & NIFO_FLAG_OCCLUSION_ONLY) ? 1 : NIFO_N_OUT;
+    acc_t* in = (acc_t*)malloc(sizeof(acc_t) * (size_t)d_in);
+    acc_t* b0 = (acc_t*)malloc(sizeof(acc_t) * (size_t)nd->width);
+    acc_t* b1 = (acc_t*)malloc(sizeof(acc_t) * (size_t)nd->width);
+    *vid = id; *t_in = ti; *t_out = to;
+    /* O7: P = o + t d as one fma per coordinate, inverse deformation, normalise */
+    for (int e = 0; e < 2; ++e) {
+        float t = e ? to : ti;
+        float P[3], pr[3], xn[3];
+        for (int a = 0; a < 3; ++a) P[a] = fmaf(t, d[a], o[a]);
+        inverse_f32(theta_max, bend_k, P, pr);
+        for (int a = 0; a < 3; ++a) {
+            float v = (pr[a] + 1.0f) * 0.5f;
+            xn[a] = v < 0.0f ? 0.0f : (v > 1.0f ? 1.0f : v);
+        }
+        encode_point(nd, table, xn, in + (size_t)e * per);
+    }
+    acc_t z[NIFO_N_OUT];
+    float zf[NIFO_N_OUT];
+    for (int j = 0; j < NIFO_N_OUT; ++j) z[j] = 0;
+    mlp_forward(nd, weights, d_in, in, n_out, z, b0, b1);
+    for (int j = 0; j < NIFO_N_OUT; ++j) zf[j] = (float)z[j];
+    if (raw_logits) for (int j = 0; j < NIFO_N_OUT; ++j) raw_logits[j] = zf[j];
+    if (flags & NIFO_FLAG_OCCLUSION_ONLY) {
+        *occlusion = (float)sigmoid_acc(z[0]);
+    } else {
+        /* decode from the acc_t logits (not the float copies) */
+        acc_t ell = (acc_t)(to - ti);
+        acc_t s = sigmoid_acc(z[1]);
+        acc_t dd = s * ell;
+        *occlusion = (float)sigmoid_acc(z[0]);
+        *distance = (float)dd;
+        *dist_total = (float)((acc_t)ti + dd);
+        acc_t nn = z[2] * z[2] + z[3] * z[3] + z[4] * z[4];
+        acc_t inv = (acc_t)1 / ACC_SQRT(nn > (acc_t)1e-24 ? nn : (acc_t)1e-24);
+        for (int a = 0; a < 3; ++a) {
+            normal[a] = (float)(z[2 + a] * inv);
+            albedo[a] = (float)sigmoid_acc(z[5 + a]);
+        }
+        for (int a = 0; a < 4; ++a) material[a] = zf[8 + a];
+    }
+    free(in); free(b0); free(b1);
+}
+
 int nifo_query(int nv, const uint8_t* occ, const float* lattice, const void* bvh,
                float theta_max, float bend_k,
                const nifo_net_desc* nd, const float* table, const float* const* weights,
@@ -637,20 +743,12 @@ int nifo_query(int nv, const uint8_t* occ, const float* lattice, const void* bvh
                float* occlusion, float* distance, float* dist_total,
                float* normal, float* albedo, float* material, float* raw_logits)
 {
-    int S = 1 + 2 * nd->pe_bands;
-    if (S > 64) return -1;
-    int per = S * nd->levels * nd->feat, d_in = 2 * per;
-    int n_out = (flags & NIFO_FLAG_OCCLUSION_ONLY) ? 1 : NIFO_N_OUT;
-    acc_t* in = (acc_t*)malloc(sizeof(acc_t) * (size_t)d_in);
-    acc_t* b0 = (acc_t*)malloc(sizeof(acc_t) * (size_t)nd->width);
-    acc_t* b1 = (acc_t*)malloc(sizeof(acc_t) * (size_t)nd->width);
+    if (1 + 2 * nd->pe_bands > 64) return -1;
     for (int64_t r = 0; r < n; ++r) {
         const float* o = origin + 3 * r; const float* d = dir + 3 * r;
         if (bvh) traverse_bvh_one((const obvh*)bvh, o, d, vid + r, t_in + r, t_out + r);
         else nifo_traverse_brute(nv, occ, lattice, 1, o, d, vid + r, t_in + r, t_out + r);
         if (!occlusion) continue;
-        float zf[NIFO_N_OUT];
-        for (int j = 0; j < NIFO_N_OUT; ++j) zf[j] = 0.0f;
         if (vid[r] < 0) {
             occlusion[r] = 0.0f;
             if (distance) { distance[r] = 0.0f; dist_total[r] = 0.0f; }
@@ -659,43 +757,79 @@ int nifo_query(int nv, const uint8_t* occ, const float* lattice, const void* bvh
             if (raw_logits) for (int j = 0; j < NIFO_N_OUT; ++j) raw_logits[NIFO_N_OUT * r + j] = 0.0f;
             continue;
         }
-        /* O7: P = o + t d as one fma per coordinate, inverse deformation, normalise */
-        for (int e = 0; e < 2; ++e) {
-            float t = e ? t_out[r] : t_in[r];
-            float P[3], pr[3], xn[3];
-            for (int a = 0; a < 3; ++a) P[a] = fmaf(t, d[a], o[a]);
-            inverse_f32(theta_max, bend_k, P, pr);
-            for (int a = 0; a < 3; ++a) {
-                float v = (pr[a] + 1.0f) * 0.5f;
-                xn[a] = v < 0.0f ? 0.0f : (v > 1.0f ? 1.0f : v);
-            }
-            encode_point(nd, table, xn, in + (size_t)e * per);
-        }
-        acc_t z[NIFO_N_OUT];
-        for (int j = 0; j < NIFO_N_OUT; ++j) z[j] = 0;
-        mlp_forward(nd, weights, d_in, in, n_out, z, b0, b1);
-        for (int j = 0; j < NIFO_N_OUT; ++j) zf[j] = (float)z[j];
-        if (raw_logits) for (int j = 0; j < NIFO_N_OUT; ++j) raw_logits[NIFO_N_OUT * r + j] = zf[j];
-        if (flags & NIFO_FLAG_OCCLUSION_ONLY) {
-            occlusion[r] = (float)sigmoid_acc(z[0]);
-        } else {
-            /* decode from the acc_t logits (not the float copies) */
-            acc_t ell = (acc_t)(t_out[r] - t_in[r]);
-            acc_t s = sigmoid_acc(z[1]);
-            acc_t dd = s * ell;
-            occlusion[r] = (float)sigmoid_acc(z[0]);
-            distance[r] = (float)dd;
-            dist_total[r] = (float)((acc_t)t_in[r] + dd);
-            acc_t nn = z[2] * z[2] + z[3] * z[3] + z[4] * z[4];
-            acc_t inv = (acc_t)1 / ACC_SQRT(nn > (acc_t)1e-24 ? nn : (acc_t)1e-24);
-            for (int a = 0; a < 3; ++a) {
-                normal[3 * r + a] = (float)(z[2 + a] * inv);
-                albedo[3 * r + a] = (float)sigmoid_acc(z[5 + a]);
-            }
-            for (int a = 0; a < 4; ++a) material[4 * r + a] = zf[8 + a];
-        }
+        nifo_eval_voxel(theta_max, bend_k, nd, table, weights, o, d, flags, vid[r], t_in[r], t_out[r],
+                        vid + r, t_in + r, t_out + r, occlusion + r, distance ? distance + r : 0,
+                        dist_total ? dist_total + r : 0, normal ? normal + 3 * r : 0, albedo ? albedo + 3 * r : 0,
+                        material ? material + 4 * r : 0, raw_logits ? raw_logits + NIFO_N_OUT * r : 0);
     }
-    free(in); free(b0); free(b1);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* O11  Multi-voxel walk at evaluation time (P:51 voxel traversal under deformation, P:53 BVH   */
+/* start, P:59-61 segmented distance, "During evaluation, we reconstruct hit positions     */
+/* along the same segmented ray").  For one ray: visit the occupied voxels it crosses in order   */
+/* of (t_in, id); evaluate the network on each voxel's rest-space segment; stop at the first     */
+/* voxel k whose predicted occlusion is >= 0.5 (logit z0 >= 0; R22).  Distance:        */
+/* D = sum_{j<k}(delta_j + l_j) + delta_k + t_k accumulated segment by segment along the */
+/* ray, with x_{-1}^1 := ray origin (R13), t_k = sigmoid(z1) * l_k (R14), l_j = t_out,j - t_in,j */
+/* and the gap delta_j = t_in,j - t_out,j-1 taken SIGNED (R23): P:59 defines it as a norm, which */
+/* is the same number whenever consecutive segments do not overlap; warped voxels can overlap    */
+/* along the ray, and a norm would then count the overlap twice.  status: 1 = hit accepted at voxel k, 0 = the ray left the     */
+/* object without a predicted hit (outputs as for a miss, R18), 2 = max_steps voxels evaluated   */
+/* without a hit (outputs of the last voxel evaluated).  steps = voxels evaluated.               */
+/* ------------------------------------------------------------------------------------ */
+int nifo_query_multi(int nv, const uint8_t* occ, const float* lattice, const void* bvh,
+                     float theta_max, float bend_k,
+                     const nifo_net_desc* nd, const float* table, const float* const* weights,
+                     int64_t n, const float* origin, const float* dir, uint32_t flags, int max_steps,
+                     int32_t* vid, float* t_in, float* t_out,
+                     float* occlusion, float* distance, float* dist_total,
+                     float* normal, float* albedo, float* material, float* raw_logits,
+                     int32_t* status, int32_t* steps, float* dist_accum)
+{
+    for (int64_t r = 0; r < n; ++r) {
+        const float* o = origin + 3 * r; const float* d = dir + 3 * r;
+        float after_t = -INFINITY; int32_t after_id = -1;
+        float prev_exit = 0.0f;                              /* x_{-1}^1 := ray origin (R13): parameter 0 */
+        float acc = 0.0f;                                    /* sum_{j<k} (delta_j + l_j) */
+        int32_t st = 0, k = 0;
+        for (;;) {
+            int32_t id; float ti, to;
+            if (bvh) traverse_bvh_after((const obvh*)bvh, o, d, after_t, after_id, &id, &ti, &to);
+            else nifo_next_voxel_brute(nv, occ, lattice, 1, o, d, &after_t, &after_id, &id, &ti, &to);
+            if (id < 0) {                                    /* left the object: miss outputs */
+                vid[r] = -1; t_in[r] = INFINITY; t_out[r] = INFINITY;
+                occlusion[r] = 0.0f;
+                if (distance) { distance[r] = 0.0f; dist_total[r] = 0.0f; }
+                if (normal) for (int a = 0; a < 3; ++a) { normal[3 * r + a] = 0.0f; albedo[3 * r + a] = 0.0f; }
+                if (material) for (int a = 0; a < 4; ++a) material[4 * r + a] = 0.0f;
+                if (raw_logits) for (int j = 0; j < NIFO_N_OUT; ++j) raw_logits[NIFO_N_OUT * r + j] = 0.0f;
+                if (dist_accum) dist_accum[r] = 0.0f;
+                st = 0;
+                break;
+            }
+            /* evaluate the network on this voxel: reuse the single-voxel pipeline on a one-ray batch whose
+               traversal result is forced to (id, ti, to) */
+            nifo_eval_voxel(theta_max, bend_k, nd, table, weights, o, d, flags, id, ti, to,
+                            vid + r, t_in + r, t_out + r, occlusion + r, distance ? distance + r : 0,
+                            dist_total ? dist_total + r : 0, normal ? normal + 3 * r : 0, albedo ? albedo + 3 * r : 0,
+                            material ? material + 4 * r : 0, raw_logits ? raw_logits + NIFO_N_OUT * r : 0);
+            ++k;
+            float delta = ti - prev_exit, ell = to - ti;     /* unit direction: lengths = parameter differences */
+            if (occlusion[r] >= 0.5f) {                      /* first voxel containing a hit: k */
+                float tk = distance ? distance[r] : 0.0f;    /* t_k = sigmoid(z1) * (t_out - t_in) (R14) */
+                if (dist_accum) dist_accum[r] = acc + delta + tk;
+                st = 1;
+                break;
+            }
+            acc += delta + ell;
+            prev_exit = to;
+            after_t = ti; after_id = id;
+            if (k >= max_steps) { if (dist_accum) dist_accum[r] = acc; st = 2; break; }
+        }
+        status[r] = st; steps[r] = k;
+    }
     return 0;
 }
 

@@ -1,0 +1,176 @@
+"""Pins for O11, the multi-voxel walk of the oracle (R22).
+CPU only.  Each pin is something the paper or the geometry fixes, not a re-run of the oracle's
+own formula: brute force over all voxels, the per-voxel test enumerated independently, the
+straight-line closed form of the segmented distance, the DDA sequence on the undeformed grid,
+and networks built so that the walk's outcome is known in advance."""
+import math
+
+import numpy as np
+import pytest
+
+import nif_inputs as I
+
+
+def _setup(oracle, nv=8, fill=0.5, seed=0, pose=(0.7, 0.5)):
+    occ = I.random_occupancy(nv, fill, seed)
+    lat = oracle.deform_lattice(nv, *pose)
+    bvh = oracle.bvh_build(nv, occ, lat)
+    cfg = I.scaled(I.get_config(0), nv=nv)
+    o, d = I.rays(cfg, 0, n=200)
+    return occ, lat, bvh, o, d
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_successor_bvh_equals_brute_force(oracle, seed):
+    nv = [8, 6, 10][seed]
+    occ, lat, bvh, o, d = _setup(oracle, nv=nv, fill=0.4 + 0.1 * seed, seed=seed)
+    n = len(o)
+    at = np.full(n, -np.inf, np.float32); ai = np.full(n, -1, np.int32)
+    for _ in range(6):                                   # walk six voxels deep, both ways in lockstep
+        vb, tib, tob = oracle.next_voxel_brute(nv, occ, lat, o, d, at, ai)
+        vh, tih, toh = bvh.next_voxel(o, d, at, ai)
+        assert np.array_equal(vb, vh)
+        assert np.array_equal(tib.view(np.int32), tih.view(np.int32))
+        assert np.array_equal(tob.view(np.int32), toh.view(np.int32))
+        live = vb >= 0
+        at = np.where(live, tib, at); ai = np.where(live, vb, ai)
+    # the first successor of (-inf, -1) is the plain nearest-voxel query
+    v0, t0, _ = oracle.traverse_brute(nv, occ, lat, o, d)
+    v1, t1, _ = oracle.next_voxel_brute(nv, occ, lat, o, d, np.full(n, -np.inf, np.float32), np.full(n, -1, np.int32))
+    assert np.array_equal(v0, v1) and np.array_equal(t0.view(np.int32), t1.view(np.int32))
+
+
+def test_walk_enumerates_exactly_the_voxels_the_ray_hits_in_order(oracle):
+    nv = 8
+    occ, lat, bvh, o, d = _setup(oracle, nv=nv, fill=0.6, seed=3)
+    ids = np.nonzero(occ)[0]
+    for r in range(0, len(o), 7):
+        # independent enumeration: the per-voxel test on every occupied voxel
+        want = []
+        for vid in ids:
+            hit, ti, _ = oracle.voxel_hit(lat, nv, int(vid), o[r], d[r])
+            if hit:
+                want.append((np.float32(ti), int(vid)))
+        want.sort()
+        got = []
+        at = np.array([-np.inf], np.float32); ai = np.array([-1], np.int32)
+        while True:
+            v, ti, _ = bvh.next_voxel(o[r:r + 1], d[r:r + 1], at, ai)
+            if v[0] < 0:
+                break
+            got.append((np.float32(ti[0]), int(v[0])))
+            at, ai = ti.copy(), v.copy()
+        assert got == want
+
+
+def test_identity_pose_axis_ray_visits_the_row_like_a_dda(oracle):
+    # undeformed grid: a ray along +x through the middle of a row visits that row's occupied
+    # voxels left to right, entering voxel i at x = -1 + i*h (closed form)
+    nv = 8; h = 2.0 / nv
+    occ = np.zeros(nv ** 3, np.uint8)
+    iy, iz = 3, 5
+    row = [0, 2, 3, 6]
+    for ix in row:
+        occ[ix + nv * (iy + nv * iz)] = 1
+    lat = oracle.deform_lattice(nv, 0.0, 0.0)
+    bvh = oracle.bvh_build(nv, occ, lat)
+    o = np.array([[-3.0, -1 + (iy + 0.5) * h, -1 + (iz + 0.5) * h]], np.float32)
+    d = np.array([[1.0, 0.0, 0.0]], np.float32)
+    at = np.array([-np.inf], np.float32); ai = np.array([-1], np.int32)
+    for ix in row:
+        v, ti, to = bvh.next_voxel(o, d, at, ai)
+        assert v[0] == ix + nv * (iy + nv * iz)
+        assert abs(ti[0] - (2.0 + ix * h)) < 1e-6 and abs(to[0] - (2.0 + (ix + 1) * h)) < 1e-6
+        at, ai = ti.copy(), v.copy()
+    assert bvh.next_voxel(o, d, at, ai)[0][0] == -1
+
+
+def _params(cfg, kind):
+    P = I.net_params(cfg, "varpres")
+    if kind == "always_accept":           # all weights zero -> every logit 0 -> occlusion = 0.5 >= 0.5
+        P.weights = [np.zeros_like(w) for w in P.weights]
+    elif kind == "never_accept":          # positive table and hidden weights -> positive activations; z0 = -sum
+        P.table = np.full_like(P.table, 0.5)
+        P.weights = [np.full_like(w, 0.01) for w in P.weights]
+        P.weights[-1][0, :] = -1.0
+    return P
+
+
+def test_all_zero_network_accepts_the_first_voxel(oracle):
+    cfg = I.get_config(0)
+    occ = I.occupancy(cfg); pose = I.poses(cfg)[0]
+    lat = oracle.deform_lattice(cfg.nv, *map(float, pose)); bvh = oracle.bvh_build(cfg.nv, occ, lat)
+    o, d = I.rays(cfg, 0, n=300)
+    P = _params(cfg, "always_accept")
+    single = oracle.query(cfg.nv, occ, lat, bvh, pose, P, o, d)
+    multi = oracle.query_multi(cfg.nv, occ, lat, bvh, pose, P, o, d, max_steps=8)
+    hit = single["voxel_id"] >= 0
+    assert np.array_equal(multi["voxel_id"], single["voxel_id"])
+    assert np.array_equal(multi["status"], hit.astype(np.int32)) and np.array_equal(multi["steps"], hit.astype(np.int32))
+    for k in ("t_in", "occlusion", "distance", "dist_total", "normal"):
+        assert np.array_equal(multi[k][hit], single[k][hit]), k
+
+
+def test_never_accepting_network_walks_every_voxel_and_reports_a_miss(oracle):
+    cfg = I.scaled(I.get_config(0), nv=8)
+    occ = I.random_occupancy(8, 0.5, 11); pose = (0.6, 0.4)
+    lat = oracle.deform_lattice(8, *pose); bvh = oracle.bvh_build(8, occ, lat)
+    o, d = I.rays(cfg, 0, n=120)
+    P = _params(cfg, "never_accept")
+    multi = oracle.query_multi(8, occ, lat, bvh, pose, P, o, d, max_steps=64)
+    ids = np.nonzero(occ)[0]
+    for r in range(len(o)):
+        crossed = sum(oracle.voxel_hit(lat, 8, int(v), o[r], d[r])[0] for v in ids)
+        assert multi["steps"][r] == crossed and multi["status"][r] == 0
+    assert (multi["voxel_id"] == -1).all() and not multi["occlusion"].any() and np.isinf(multi["t_in"]).all()
+    # with a step budget smaller than the crossing count the walk stops with status 2 on the budget-th voxel
+    capped = oracle.query_multi(8, occ, lat, bvh, pose, P, o, d, max_steps=2)
+    long = multi["steps"] > 2
+    assert (capped["status"][long] == 2).all() and (capped["steps"][long] == 2).all()
+    assert (capped["voxel_id"][long] >= 0).all()
+
+
+def test_segmented_distance_sum_reduces_to_the_straight_line_parameter(oracle):
+    # P:61 sums segment and gap lengths along one straight ray with a unit direction; with signed
+    # gaps (R23) the sum telescopes to t_in,k + t_k (= dist_total of voxel k).  The oracle
+    # accumulates it term by term: a dropped or doubled term breaks this equality.
+    cfg = I.get_config(0)
+    occ = I.occupancy(cfg); pose = I.poses(cfg)[0]
+    lat = oracle.deform_lattice(cfg.nv, *map(float, pose)); bvh = oracle.bvh_build(cfg.nv, occ, lat)
+    o, d = I.rays(cfg, 0, n=400)
+    multi = oracle.query_multi(cfg.nv, occ, lat, bvh, pose, I.net_params(cfg, "varpres"), o, d, max_steps=16)
+    acc = multi["status"] == 1
+    assert acc.sum() > 50 and (multi["steps"][acc] > 1).sum() > 10      # some rays accept beyond the first voxel
+    np.testing.assert_allclose(multi["dist_accum"][acc], multi["dist_total"][acc], rtol=3e-6, atol=3e-6)
+    assert (multi["occlusion"][acc] >= 0.5).all()
+    ell = multi["t_out"][acc] - multi["t_in"][acc]
+    assert (multi["distance"][acc] >= 0).all() and (multi["distance"][acc] <= ell * (1 + 1e-6)).all()
+
+
+def test_paper_norm_form_of_the_sum_on_non_overlapping_segments(oracle):
+    # P:59 defines delta_i and l_i as NORMS of differences of entry/exit points.  On the undeformed
+    # grid the segments of a row do not overlap, and the norm form, evaluated here in numpy from the
+    # points, must equal the oracle's accumulated value.
+    nv = 8; h = 2.0 / nv
+    occ = np.zeros(nv ** 3, np.uint8)
+    iy, iz = 2, 4
+    row = [1, 2, 5, 7]
+    for ix in row:
+        occ[ix + nv * (iy + nv * iz)] = 1
+    lat = oracle.deform_lattice(nv, 0.0, 0.0); bvh = oracle.bvh_build(nv, occ, lat)
+    o = np.array([[-2.5, -1 + (iy + 0.4) * h, -1 + (iz + 0.6) * h]], np.float32)
+    d = np.array([[1.0, 0.0, 0.0]], np.float32)
+    cfg = I.scaled(I.get_config(0), nv=nv)
+    P = _params(cfg, "never_accept")
+    m = oracle.query_multi(nv, occ, lat, bvh, (0.0, 0.0), P, o, d, max_steps=3)     # stops on the 3rd voxel
+    assert m["status"][0] == 2 and m["steps"][0] == 3
+    pts = []                                                                      # (entry, exit) points, in order
+    at = np.array([-np.inf], np.float32); ai = np.array([-1], np.int32)
+    for _ in range(3):
+        v, ti, to = bvh.next_voxel(o, d, at, ai)
+        pts.append((o[0] + ti[0] * d[0], o[0] + to[0] * d[0]))
+        at, ai = ti.copy(), v.copy()
+    prev = o[0].astype(np.float64); total = 0.0
+    for x0, x1 in pts:
+        total += np.linalg.norm(x0 - prev) + np.linalg.norm(x1 - x0); prev = x1
+    assert abs(m["dist_accum"][0] - total) < 1e-5
