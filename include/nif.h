@@ -181,6 +181,40 @@ int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
               const nif_query_out* out, void* workspace, size_t workspace_bytes,
               unsigned flags, void* stream);
 
+/* -------- evaluation-time multi-voxel walk (R22, R23) ------------------- */
+
+/* Outcome of a walk, per ray. */
+enum {
+    NIF_WALK_MISS      = 0,    /* the ray left the object without a predicted hit: outputs as for a miss (R18) */
+    NIF_WALK_HIT       = 1,    /* accepted in voxel k = steps-1: `out` holds that voxel's outputs              */
+    NIF_WALK_MAX_STEPS = 2     /* max_steps voxels evaluated, none accepted: `out` holds the last one's        */
+};
+
+typedef struct {
+    int32_t* status;              /* n   NIF_WALK_*                                                         */
+    int32_t* steps;               /* n   voxels on which the network was evaluated                          */
+    float* dist_accum;            /* n   sum_{j<k}(delta_j + l_j) + delta_k + t_k of P:61, accumulated term  */
+                                  /*     by term along the ray (delta signed, R23); the partial sum for     */
+                                  /*     NIF_WALK_MAX_STEPS; 0 for NIF_WALK_MISS                            */
+} nif_walk_out;
+
+/* Scratch bytes nif_query_multi needs for a batch of n rays.  Host-only. */
+int nif_query_multi_workspace_bytes(int64_t n, size_t* bytes);
+
+/* The intersection query continued across voxels.  Each ray visits the occupied deformed voxels it
+ * crosses in order of (t_in, id) -- the first by the BVH, each next one the successor of the
+ * one before, which is the neighbour across the exit face on a conforming lattice and skips empty
+ * gaps (R22) -- and the network is evaluated on each voxel's rest-space segment exactly as in
+ * nif_query.  The walk stops at the first voxel whose predicted occlusion is >= 0.5; `out` then holds
+ * that voxel's id, t_in, t_out and head outputs (dist_total = t_in + distance is the ray parameter of
+ * the predicted hit) and walk->dist_accum the literal segmented sum of P:61.  1 <= max_steps <= 4096.
+ * Flags as nif_query (not NIF_TRAVERSE_ONLY).  Enqueues max_steps rounds of
+ * {successor traversal, encode+MLP, accept/continue} on `stream`; rounds with no ray left are empty
+ * launches.  Does not synchronise.  All pointers DEVICE. */
+int nif_query_multi(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                    const nif_query_out* out, const nif_walk_out* walk, int32_t max_steps,
+                    void* workspace, size_t workspace_bytes, unsigned flags, void* stream);
+
 /* -------- end-to-end with HOST buffers ---------------------------------------------------- */
 
 /* Staging for nif_query_host: device buffers for `chunk_rays` rays x 2 (double buffer), three

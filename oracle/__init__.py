@@ -84,6 +84,10 @@ class Oracle:
         L.nifo_query_multi.argtypes = ([C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float,
                                         C.POINTER(_NetDesc), C.c_void_p, C.c_void_p, C.c_int64,
                                         C.c_void_p, C.c_void_p, C.c_uint32, C.c_int] + [C.c_void_p] * 13)
+        L.nifo_walk_trace.restype = C.c_int
+        L.nifo_walk_trace.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float,
+                                      C.POINTER(_NetDesc), C.c_void_p, C.c_void_p, C.c_int64,
+                                      C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         self.acc_bytes = L.nifo_acc_bytes()
 
     # ---- deformation -----------------------------------------------------------------
@@ -256,6 +260,23 @@ class Oracle:
         if rc != 0:
             raise RuntimeError(f"nifo_query_multi failed: {rc}")
         return o
+
+
+    def walk_trace(self, nv, occ, lattice, bvh, pose, params, origin, direction, max_steps):
+        """O11 trace: (trace_id, trace_z0), each [n, max_steps]; id -1 past the end of a ray's voxel sequence."""
+        origin = _f32(origin); direction = _f32(direction)
+        n = len(origin)
+        d = self._desc(params.shape, params.level_res)
+        table = _f32(params.table)
+        ws, arr = self._wptrs(params.weights)
+        tid = np.empty((n, max_steps), np.int32); tz = np.empty((n, max_steps), np.float32)
+        rc = self.lib.nifo_walk_trace(nv, occ.ctypes.data, lattice.ctypes.data,
+                                      bvh.handle if bvh is not None else None, float(pose[0]), float(pose[1]),
+                                      C.byref(d), table.ctypes.data, arr, n, origin.ctypes.data,
+                                      direction.ctypes.data, int(max_steps), tid.ctypes.data, tz.ctypes.data)
+        if rc != 0:
+            raise RuntimeError(f"nifo_walk_trace failed: {rc}")
+        return tid, tz
 
 
 class OracleBVH:

@@ -833,6 +833,37 @@ int nifo_query_multi(int nv, const uint8_t* occ, const float* lattice, const voi
     return 0;
 }
 
+/* O11 trace: the first `max_steps` voxels of each ray's (t_in, id)-ordered sequence with the occlusion
+   logit z0 the network predicts on each, WITHOUT stopping at an accepted voxel.  trace_id = -1 past
+   the end of the sequence.  Tests use it to tell rays whose accept decisions are clear of the
+   threshold (the CUDA path must agree exactly) from rays with a logit within rounding of 0 (where
+   the fp16 path may legitimately decide the other way and any consistent outcome is valid). */
+int nifo_walk_trace(int nv, const uint8_t* occ, const float* lattice, const void* bvh,
+                    float theta_max, float bend_k,
+                    const nifo_net_desc* nd, const float* table, const float* const* weights,
+                    int64_t n, const float* origin, const float* dir, int max_steps,
+                    int32_t* trace_id, float* trace_z0)
+{
+    for (int64_t r = 0; r < n; ++r) {
+        const float* o = origin + 3 * r; const float* d = dir + 3 * r;
+        float after_t = -INFINITY; int32_t after_id = -1;
+        int k = 0;
+        for (; k < max_steps; ++k) {
+            int32_t id; float ti, to;
+            if (bvh) traverse_bvh_after((const obvh*)bvh, o, d, after_t, after_id, &id, &ti, &to);
+            else nifo_next_voxel_brute(nv, occ, lattice, 1, o, d, &after_t, &after_id, &id, &ti, &to);
+            if (id < 0) break;
+            int32_t v; float a, b, occl, raw[NIFO_N_OUT];
+            nifo_eval_voxel(theta_max, bend_k, nd, table, weights, o, d, NIFO_FLAG_OCCLUSION_ONLY, id, ti, to,
+                            &v, &a, &b, &occl, 0, 0, 0, 0, 0, raw);
+            trace_id[r * max_steps + k] = id; trace_z0[r * max_steps + k] = raw[0];
+            after_t = ti; after_id = id;
+        }
+        for (; k < max_steps; ++k) { trace_id[r * max_steps + k] = -1; trace_z0[r * max_steps + k] = 0.0f; }
+    }
+    return 0;
+}
+
 /* rest-space normalised endpoints of hit rays (exposed for the "inside the hit voxel's rest
    cell" invariant): out[r*6 + e*3 + a]; NaN for a miss. */
 void nifo_rest_endpoints(float theta_max, float bend_k, int64_t n, const float* origin,

@@ -19,6 +19,7 @@ NIF_F32, NIF_F16 = 0, 1
 NIF_OCCLUSION_ONLY, NIF_ENGINE_FFMA, NIF_TRAVERSE_ONLY = 1, 2, 4
 NIF_TRAVERSE_COHERENT, NIF_TRAVERSE_INCOHERENT, NIF_PROBE_SKIP_GATHER = 8, 16, 32
 NIF_N_OUT = 12
+NIF_WALK_MISS, NIF_WALK_HIT, NIF_WALK_MAX_STEPS = 0, 1, 2
 
 
 class NifError(RuntimeError):
@@ -51,6 +52,10 @@ _OUT_FIELDS = ["voxel_id", "t_in", "t_out", "occlusion", "distance", "dist_total
 
 class _QueryOut(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in _OUT_FIELDS]
+
+
+class _WalkOut(C.Structure):
+    _fields_ = [("status", C.c_void_p), ("steps", C.c_void_p), ("dist_accum", C.c_void_p)]
 
 
 class _BvhInfo(C.Structure):
@@ -88,6 +93,9 @@ def lib() -> C.CDLL:
         L.nif_query_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_query.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut),
                                 C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
+        L.nif_query_multi_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
+        L.nif_query_multi.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut),
+                                      C.POINTER(_WalkOut), C.c_int32, C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
         L.nif_stage_create.argtypes = [C.c_int64, C.POINTER(C.c_void_p)]
         L.nif_stage_destroy.argtypes = [C.c_void_p]
         L.nif_stage_destroy.restype = None
@@ -254,6 +262,36 @@ def nif_query(bvh: Bvh, net: Net | None, origin: torch.Tensor, direction: torch.
     q = _out_struct(out)
     _check(lib().nif_query(bvh.handle, net.handle if net is not None else None, C.byref(rb), C.byref(q),
                            workspace.data_ptr(), workspace.numel(), flags, _stream_ptr(stream)), "nif_query")
+    return workspace
+
+
+def nif_query_multi_workspace_bytes(n: int) -> int:
+    b = C.c_size_t()
+    _check(lib().nif_query_multi_workspace_bytes(n, C.byref(b)), "nif_query_multi_workspace_bytes")
+    return b.value
+
+
+def alloc_walk_outputs(n: int, device="cuda") -> dict:
+    return {"status": torch.empty(n, dtype=torch.int32, device=device),
+            "steps": torch.empty(n, dtype=torch.int32, device=device),
+            "dist_accum": torch.empty(n, dtype=torch.float32, device=device)}
+
+
+def nif_query_multi(bvh: Bvh, net: Net, origin: torch.Tensor, direction: torch.Tensor, out: dict, walk: dict,
+                    max_steps: int, workspace: torch.Tensor | None = None, flags: int = 0,
+                    stream=None) -> torch.Tensor:
+    """Multi-voxel walk (include/nif.h); enqueues on the stream, returns the workspace tensor."""
+    n = origin.shape[0]
+    assert origin.is_cuda and direction.is_cuda and origin.dtype == torch.float32
+    assert origin.is_contiguous() and direction.is_contiguous() and direction.shape[0] == n
+    if workspace is None:
+        workspace = _ws(nif_query_multi_workspace_bytes(n))
+    rb = _RayBatch(n, origin.data_ptr(), direction.data_ptr())
+    q = _out_struct(out)
+    w = _WalkOut(walk["status"].data_ptr(), walk["steps"].data_ptr(), walk["dist_accum"].data_ptr())
+    _check(lib().nif_query_multi(bvh.handle, net.handle, C.byref(rb), C.byref(q), C.byref(w), int(max_steps),
+                                 workspace.data_ptr(), workspace.numel(), flags, _stream_ptr(stream)),
+           "nif_query_multi")
     return workspace
 
 

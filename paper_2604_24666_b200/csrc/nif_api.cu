@@ -120,6 +120,24 @@ extern "C" int nif_query_workspace_bytes(int64_t n, size_t* bytes)
     return NIF_OK;
 }
 
+void nif_query_ws_layout(const nif_bvh* bvh, int64_t n, void* workspace, NifQueryWs* ws)
+{
+    ws->scratch = (NifQueryScratch*)workspace;
+    ws->bin_count = (uint32_t*)((char*)workspace + sizeof(NifQueryScratch));
+    ws->rank = ws->bin_count + NIF_MAX_BINS;
+    ws->hit_list = (int32_t*)(ws->rank + n);
+    ws->bin_shift = 0;
+    for (;;) {                                               // bricks of 2^s voxels until the bins fit
+        ws->nvb = (bvh->nv + (1 << ws->bin_shift) - 1) >> ws->bin_shift;
+        if ((unsigned long long)ws->nvb * ws->nvb * ws->nvb <= NIF_MAX_BINS) break;
+        ++ws->bin_shift;
+    }
+    ws->n_bins = (uint32_t)(ws->nvb * ws->nvb * ws->nvb);
+}
+
+int nif_validate_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                       const nif_query_out* out, unsigned flags);
+
 static int validate_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                           const nif_query_out* out, unsigned flags)
 {
@@ -136,6 +154,12 @@ static int validate_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_
     return NIF_OK;
 }
 
+int nif_validate_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                       const nif_query_out* out, unsigned flags)
+{
+    return validate_query(bvh, net, rays, out, flags);
+}
+
 extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                          const nif_query_out* out, void* workspace, size_t workspace_bytes,
                          unsigned flags, void* stream_)
@@ -148,24 +172,14 @@ extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_b
     if (!workspace || ((uintptr_t)workspace & 255u) != 0 || workspace_bytes < need - 256) return NIF_ERR_WORKSPACE;
     cudaStream_t stream = (cudaStream_t)stream_;
     NifQueryWs ws;
-    ws.scratch = (NifQueryScratch*)workspace;
-    ws.bin_count = (uint32_t*)((char*)workspace + sizeof(NifQueryScratch));
-    ws.rank = ws.bin_count + NIF_MAX_BINS;
-    ws.hit_list = (int32_t*)(ws.rank + rays->n);
-    ws.bin_shift = 0;
-    for (;;) {                                               // bricks of 2^s voxels until the bins fit
-        ws.nvb = (bvh->nv + (1 << ws.bin_shift) - 1) >> ws.bin_shift;
-        if ((unsigned long long)ws.nvb * ws.nvb * ws.nvb <= NIF_MAX_BINS) break;
-        ++ws.bin_shift;
-    }
-    ws.n_bins = (uint32_t)(ws.nvb * ws.nvb * ws.nvb);
+    nif_query_ws_layout(bvh, rays->n, workspace, &ws);
     NifQueryScratch* scratch = ws.scratch;
     int32_t* hit_list = ws.hit_list;
     const bool traverse_only = (flags & NIF_TRAVERSE_ONLY) != 0;
     NIF_CUDA_TRY(cudaMemsetAsync(workspace, 0, sizeof(NifQueryScratch) + (traverse_only ? 0 : (size_t)ws.n_bins * 4), stream));
     const int prof = nif_prof_begin(stream);                 // -1 unless nif_profile_enable(1)
-    rc = nif_launch_traverse(bvh, rays, out, &ws, flags, stream);
-    if (rc == NIF_OK && !traverse_only) rc = nif_launch_bin_hits(bvh, rays, out, &ws, stream);
+    rc = nif_launch_traverse(bvh, rays, out, &ws, flags, nullptr, stream);
+    if (rc == NIF_OK && !traverse_only) rc = nif_launch_bin_hits(bvh, rays, out, &ws, nullptr, stream);
     nif_prof_mark(prof, 1, stream);
     if (rc != NIF_OK || traverse_only) return rc;
     const bool use_tc = net->desc.dtype == NIF_F16 && net->tc_supported && !(flags & NIF_ENGINE_FFMA);

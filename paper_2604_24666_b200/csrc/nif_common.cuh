@@ -80,6 +80,15 @@ struct NifQueryWs {                    // pointers into the caller's workspace
     int bin_shift, nvb;                // bin = (ix >> s) + nvb * ((iy >> s) + nvb * (iz >> s))
 };
 
+// one round of the multi-voxel walk (nif_walk.cu): round 0 is the plain nearest-voxel query over all
+// rays; rounds >= 1 run over `ray_list` (rays still walking) and look for each ray's next voxel
+struct NifWalkRound {
+    int round;
+    const int32_t* ray_list;           // device, *n_list entries
+    const unsigned int* n_list;        // device
+    float* dist_accum;                 // nif_walk_out.dist_accum
+};
+
 extern "C" void nif_count_launch(int n);
 
 #define NIF_CUDA_TRY(expr)                                   \
@@ -90,9 +99,10 @@ extern "C" void nif_count_launch(int n);
 
 // launchers implemented in the individual .cu files
 int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        const NifQueryWs* ws, unsigned flags, cudaStream_t stream);
+                        const NifQueryWs* ws, unsigned flags, const NifWalkRound* walk, cudaStream_t stream);
 int nif_launch_bin_hits(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        const NifQueryWs* ws, cudaStream_t stream);
+                        const NifQueryWs* ws, const NifWalkRound* walk, cudaStream_t stream);
+void nif_query_ws_layout(const nif_bvh* bvh, int64_t n, void* workspace, NifQueryWs* ws);
 int nif_launch_ffma(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                     const nif_query_out* out, const NifQueryScratch* scratch,
                     const int32_t* hit_list, unsigned flags, cudaStream_t stream);

@@ -150,7 +150,19 @@ struct TravParams {
     uint32_t* rank;
     int bin_shift, nvb;
     unsigned flags;
+    // multi-voxel walk (nif_query_multi, R22): rounds >= 1 run over the list of rays still
+    // walking and look for the successor of the voxel each ray evaluated last
+    const int32_t* ray_list;                  // NULL: rays 0..n-1
+    const unsigned int* n_list;               // device count of ray_list
+    float* walk_dist_accum;                   // NULL outside a walk; a ray that runs out of voxels gets 0
 };
+
+// successor bound of the walk: only voxels whose (t_in, id) is lexicographically greater than the
+// voxel the ray evaluated last are candidates (R22)
+__device__ __forceinline__ bool after_bound(float ti, int32_t id, float after_t, int32_t after_id)
+{
+    return (ti > after_t) || (ti == after_t && id > after_id);
+}
 
 // results of one finished ray: ids/t always; zero heads for a miss (R18); bin count for a hit
 __device__ __forceinline__ void retire_ray(const TravParams& p, long long ray, int32_t best_id, float best_in, float best_out)
@@ -172,6 +184,7 @@ __device__ __forceinline__ void retire_ray(const TravParams& p, long long ray, i
 #pragma unroll
             for (int a = 0; a < NIF_N_OUT; ++a) p.out.raw_logits[NIF_N_OUT * ray + a] = 0.0f;
         }
+        if (p.walk_dist_accum) p.walk_dist_accum[ray] = 0.0f;
     } else {
         // counted into the bin of the voxel it hit; the returned count is the ray's rank inside its
         // bin (k_bin_offsets / k_scatter_hits below turn ranks into positions in hit_list)
@@ -187,10 +200,14 @@ __device__ __forceinline__ void retire_ray(const TravParams& p, long long ray, i
 // then all of them run the expensive 12-triangle voxel test together; finished lanes are refilled
 // from a global counter once enough of them are idle.  Incoherent rays (config 3) otherwise leave
 // 4 of 32 lanes active on average.
+template <bool AFTER>
 __global__ void __launch_bounds__(TRAV_BLOCK, TRAV_BLOCKS_PER_SM)
 k_traverse_persistent(const TravParams p)
 {
-    if (*p.coherent_flag != 0u) return;                   // k_traverse_simple takes this batch
+    if (!AFTER && *p.coherent_flag != 0u) return;         // k_traverse_simple takes this batch
+    const long long n_rays = p.ray_list ? (long long)*p.n_list : p.n;
+    float after_t = -INFINITY;                            // AFTER: successor bound (R22)
+    int32_t after_id = -1;
     const int lane = threadIdx.x & 31;
     const NifNode* __restrict__ nodes = p.nodes;
     uint2 stack[STACK_MAX];
@@ -210,10 +227,11 @@ k_traverse_persistent(const TravParams p)
             unsigned base = 0;
             if (lane == 0) base = atomicAdd(p.ray_counter, (unsigned)__popc(idle));
             base = __shfl_sync(0xffffffffu, base, 0);
-            if ((long long)base + __popc(idle) >= p.n) exhausted = true;
+            if ((long long)base + __popc(idle) >= n_rays) exhausted = true;
             const long long cand = (long long)base + __popc(idle & ((1u << lane) - 1u));
-            if (ray < 0 && cand < p.n) {
-                ray = cand;
+            if (ray < 0 && cand < n_rays) {
+                ray = p.ray_list ? (long long)p.ray_list[cand] : cand;
+                if (AFTER) { after_t = p.out.t_in[ray]; after_id = p.out.voxel_id[ray]; }
                 r.ox = p.origin[3 * ray]; r.oy = p.origin[3 * ray + 1]; r.oz = p.origin[3 * ray + 2];
                 r.dx = p.dir[3 * ray]; r.dy = p.dir[3 * ray + 1]; r.dz = p.dir[3 * ray + 2];
                 r.ix = __fdiv_rn(1.0f, r.dx); r.iy = __fdiv_rn(1.0f, r.dy); r.iz = __fdiv_rn(1.0f, r.dz);
@@ -268,8 +286,10 @@ k_traverse_persistent(const TravParams p)
                     key[c] = 0xffffffffu;
                     if (__any_sync(0xffffffffu, (meta.x >> c) & 1u)) {       // coherent warps skip absent octants
                         float cn, cf;
+                        // AFTER: every voxel below has t_in <= its box's far end <= cf (boxes nest, R10), so a
+                        // child that ends before after_t holds no successor
                         const bool ok = slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf) &&
-                                        ((meta.x >> c) & 1u) && !(cn > best_in);
+                                        ((meta.x >> c) & 1u) && !(cn > best_in) && !(AFTER && cf < after_t);
                         // cn >= 0: its bit pattern orders like an integer; the 3 low mantissa bits make
                         // room for the octant (t_near only gets smaller: pruning stays conservative).  ~
                         // turns the ascending network into "farthest first"; rejected children sort last.
@@ -305,7 +325,7 @@ k_traverse_persistent(const TravParams p)
         if (ray >= 0 && sp > 0) {
             const uint32_t id = stack[--sp].x & ~LEAF_FLAG;
             float ti, to;
-            if (voxel_hit(p.lat, p.nv, id, r, ti, to)) {
+            if (voxel_hit(p.lat, p.nv, id, r, ti, to) && (!AFTER || after_bound(ti, (int32_t)id, after_t, after_id))) {
                 if (ti < best_in || (ti == best_in && (int32_t)id < best_id)) {
                     best_id = (int32_t)id; best_in = ti; best_out = to;
                 }
@@ -461,10 +481,12 @@ k_bin_offsets(uint32_t* __restrict__ bin_count, uint32_t n_bins, NifQueryScratch
 __global__ void __launch_bounds__(256)
 k_scatter_hits(long long n, int nv, int bin_shift, int nvb, const int32_t* __restrict__ voxel_id,
                const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ rank,
-               int32_t* __restrict__ hit_list)
+               int32_t* __restrict__ hit_list, const int32_t* __restrict__ ray_list,
+               const unsigned int* __restrict__ n_list)
 {
-    const long long ray = (long long)blockIdx.x * 256 + threadIdx.x;
-    if (ray >= n) return;
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= (ray_list ? (long long)*n_list : n)) return;
+    const long long ray = ray_list ? (long long)ray_list[i] : i;
     const int32_t vid = voxel_id[ray];
     if (vid < 0) return;
     const uint32_t unv = (uint32_t)nv, id = (uint32_t)vid;
@@ -476,7 +498,7 @@ k_scatter_hits(long long n, int nv, int bin_shift, int nvb, const int32_t* __res
 }  // namespace
 
 int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        const NifQueryWs* ws, unsigned flags, cudaStream_t stream)
+                        const NifQueryWs* ws, unsigned flags, const NifWalkRound* walk, cudaStream_t stream)
 {
     if (rays->n == 0) return NIF_OK;
     static int n_sm = 0;
@@ -493,7 +515,19 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
     p.ray_counter = &ws->scratch->tile_counter;
     p.bin_count = ws->bin_count; p.rank = ws->rank; p.bin_shift = ws->bin_shift; p.nvb = ws->nvb;
     p.flags = flags;
+    p.ray_list = walk && walk->round > 0 ? walk->ray_list : nullptr;
+    p.n_list = walk ? walk->n_list : nullptr;
+    p.walk_dist_accum = walk ? walk->dist_accum : nullptr;
     p.coherent_flag = &ws->scratch->pad[0];
+    const long long want = (rays->n + TRAV_BLOCK - 1) / TRAV_BLOCK;
+    const long long cap = (long long)n_sm * TRAV_BLOCKS_PER_SM;
+    if (p.ray_list) {
+        // walk rounds >= 1: the live rays are in voxel-bin order, not pixel order -> persistent kernel
+        k_traverse_persistent<true><<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
+        nif_count_launch(1);
+        NIF_CUDA_TRY(cudaGetLastError());
+        return NIF_OK;
+    }
     // scratch header (zeroed by nif_query): pad[0] decision, pad[1] coherent votes, pad[2] finished blocks
     const long long groups_total = (rays->n + 31) / 32;
     const int n_groups = (int)(groups_total < 2048 ? groups_total : 2048);
@@ -501,22 +535,21 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
     for (int a = 0; a < 3; ++a) extent = fmaxf(extent, bvh->hi[a] - bvh->lo[a]);
     k_ray_coherence<<<(n_groups * 32 + 255) / 256, 256, 0, stream>>>(
         (long long)rays->n, rays->origin, rays->dir, extent, n_groups, flags, &ws->scratch->pad[1], &ws->scratch->pad[0]);
-    const long long want = (rays->n + TRAV_BLOCK - 1) / TRAV_BLOCK;
-    const long long cap = (long long)n_sm * TRAV_BLOCKS_PER_SM;
     k_traverse_simple<<<(unsigned)want, TRAV_BLOCK, 0, stream>>>(p);
-    k_traverse_persistent<<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
+    k_traverse_persistent<false><<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
     nif_count_launch(3);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;
 }
 
 int nif_launch_bin_hits(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        const NifQueryWs* ws, cudaStream_t stream)
+                        const NifQueryWs* ws, const NifWalkRound* walk, cudaStream_t stream)
 {
     if (rays->n == 0) return NIF_OK;
     k_bin_offsets<<<(ws->n_bins + 1023u) / 1024u, 1024, 0, stream>>>(ws->bin_count, ws->n_bins, ws->scratch);
     k_scatter_hits<<<(unsigned)((rays->n + 255) / 256), 256, 0, stream>>>(
-        (long long)rays->n, bvh->nv, ws->bin_shift, ws->nvb, out->voxel_id, ws->bin_count, ws->rank, ws->hit_list);
+        (long long)rays->n, bvh->nv, ws->bin_shift, ws->nvb, out->voxel_id, ws->bin_count, ws->rank, ws->hit_list,
+        walk && walk->round > 0 ? walk->ray_list : nullptr, walk ? walk->n_list : nullptr);
     nif_count_launch(2);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;

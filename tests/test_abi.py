@@ -53,6 +53,8 @@ def test_host_only_entry_points(lib):
     assert nif.nif_query_workspace_bytes(0) >= 64
     assert nif.nif_query_workspace_bytes(1 << 20) >= 64 + 4 * (1 << 20)
     assert lib.nif_query_workspace_bytes(-1, C.byref(n)) == -1
+    assert nif.nif_query_multi_workspace_bytes(1 << 20) >= nif.nif_query_workspace_bytes(1 << 20) + 8 * (1 << 20)
+    assert lib.nif_query_multi_workspace_bytes(-1, C.byref(n)) == -1
     assert lib.nif_error_string(0) == b"ok"
     for s in range(-5, 0):
         assert lib.nif_error_string(s) not in (b"ok", b"unknown status")
@@ -65,6 +67,7 @@ def test_argument_validation_without_touching_the_device(lib):
     assert lib.nif_net_create(None, None, None, None, None) == -1
     assert lib.nif_query(None, None, None, None, None, 0, 0, None) == -1
     assert lib.nif_query_host(None, None, None, None, None, 0) == -1
+    assert lib.nif_query_multi(None, None, None, None, None, 4, None, 0, 0, None) == -1
     h = C.c_void_p()
     assert lib.nif_stage_create(0, C.byref(h)) == -1
 

@@ -174,3 +174,35 @@ def test_paper_norm_form_of_the_sum_on_non_overlapping_segments(oracle):
     for x0, x1 in pts:
         total += np.linalg.norm(x0 - prev) + np.linalg.norm(x1 - x0); prev = x1
     assert abs(m["dist_accum"][0] - total) < 1e-5
+
+
+def test_trace_is_the_walk_without_stopping(oracle):
+    # the trace lists the ray's voxel sequence with each voxel's occlusion logit; the walk must stop at
+    # the first non-negative one (sigmoid(z) >= 0.5 <=> z >= 0), and the sequence must be the successor
+    # chain (ids from next_voxel).
+    cfg = I.get_config(0)
+    occ = I.occupancy(cfg); pose = I.poses(cfg)[0]
+    lat = oracle.deform_lattice(cfg.nv, *map(float, pose)); bvh = oracle.bvh_build(cfg.nv, occ, lat)
+    o, d = I.rays(cfg, 0, n=300)
+    P = I.net_params(cfg, "varpres")
+    K = 12
+    tid, tz = oracle.walk_trace(cfg.nv, occ, lat, bvh, pose, P, o, d, K)
+    multi = oracle.query_multi(cfg.nv, occ, lat, bvh, pose, P, o, d, max_steps=K)
+    at = np.full(len(o), -np.inf, np.float32); ai = np.full(len(o), -1, np.int32)
+    for k in range(K):
+        v, ti, _ = bvh.next_voxel(o, d, at, ai)
+        assert np.array_equal(v, tid[:, k])
+        live = v >= 0
+        at = np.where(live, ti, at); ai = np.where(live, v, ai)
+    clear = np.abs(tz) > 1e-6
+    for r in range(len(o)):
+        if not clear[r][tid[r] >= 0].all():
+            continue
+        acc = np.nonzero((tid[r] >= 0) & (tz[r] >= 0))[0]
+        n_vox = int((tid[r] >= 0).sum())
+        if len(acc):
+            assert multi["status"][r] == 1 and multi["steps"][r] == acc[0] + 1 and multi["voxel_id"][r] == tid[r, acc[0]]
+        elif n_vox < K:
+            assert multi["status"][r] == 0 and multi["steps"][r] == n_vox and multi["voxel_id"][r] == -1
+        else:
+            assert multi["status"][r] == 2 and multi["steps"][r] == K and multi["voxel_id"][r] == tid[r, K - 1]
