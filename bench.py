@@ -249,12 +249,18 @@ def run_ours(args) -> None:
     n_per_pose = cfg.rays_per_pose
     n_total = n_per_pose * cfg.n_poses
     out = nif.alloc_outputs(n_per_pose, device=dev)
+    walk_out = nif.alloc_walk_outputs(n_per_pose, device=dev) if args.walk else None
     ws = None
+    ws_multi = None
 
     def step():
-        nonlocal ws
+        nonlocal ws, ws_multi
         for p in poses:
-            ws = nif.nif_query(p["bvh"], net, p["o"], p["d"], out, workspace=ws, flags=flags)
+            if args.walk:                              # multi-voxel walk, --walk K rounds
+                ws_multi = nif.nif_query_multi(p["bvh"], net, p["o"], p["d"], out, walk_out, args.walk,
+                                               workspace=ws_multi, flags=flags)
+            else:
+                ws = nif.nif_query(p["bvh"], net, p["o"], p["d"], out, workspace=ws, flags=flags)
 
     def sync_all():
         if world > 1:
@@ -293,9 +299,17 @@ def run_ours(args) -> None:
     ms_per_step = elapsed_ms / args.steps
     value = world * n_total / (ms_per_step * 1e-3) / 1e6
 
+    walk_stats = None
+    if args.walk:
+        torch.cuda.synchronize()
+        st = walk_out["status"]; sp = walk_out["steps"]
+        walk_stats = {"max_steps": args.walk, "last_pose_status_counts": [int((st == k).sum()) for k in range(3)],
+                      "last_pose_network_evals": int(sp.sum()), "last_pose_mean_steps_of_entering_rays":
+                      float(sp[sp > 0].float().mean()) if bool((sp > 0).any()) else 0.0}
+
     # ---- MLP-only probe: same kernel, gathers replaced by a constant A operand (outside the timed region)
     mlp_probe = None
-    if rank == 0 and nif.nif_net_uses_tensor_cores(net) and not (flags & nif.NIF_ENGINE_FFMA):
+    if rank == 0 and not args.walk and nif.nif_net_uses_tensor_cores(net) and not (flags & nif.NIF_ENGINE_FFMA):
         nif.nif_profile_enable(True)
         for _ in range(5):
             for p in poses:
@@ -340,20 +354,32 @@ def run_ours(args) -> None:
     net_ms = prof["network_ms"] / nq                    # average launch duration, CUDA events
     trav_ms = prof["traverse_ms"] / nq
     hits_per_launch = n_hit / cfg.n_poses
+    table_bytes = params.table_storage().nbytes
+    l2_resident = table_bytes <= (64 << 20)              # 126 MB L2: a 32 MiB table stays resident, 512 MiB does not
+    probe_bytes = (32 << 20) if l2_resident else (256 << 20)
     probe = nif.nif_probe_gather(torch.from_numpy(params.table_storage()).to(dev).view(torch.uint8).reshape(-1)
-                                 if args.probe_table else torch.empty(32 << 20, dtype=torch.uint8, device=dev))
+                                 if args.probe_table else torch.empty(probe_bytes, dtype=torch.uint8, device=dev))
+    useful_gbs = hits_per_launch * work["useful_gather_bytes"] / (net_ms * 1e-3) / 1e9
     gather_gbs = hits_per_launch * work["sector_gather_bytes"] / (net_ms * 1e-3) / 1e9
     tensor_tfs = hits_per_launch * work["mlp_flops_per_hit_ray"] / (net_ms * 1e-3) / 1e12
     traffic = NCU_TRAFFIC.get(cfg.cfg_id, (None, None))
     roofline = {"kernel": "k_fused_encode_mlp (tcgen05)" if not (flags & nif.NIF_ENGINE_FFMA) and cfg.net.dtype == "f16"
                 and nif.nif_net_uses_tensor_cores(net) else "k_encode_mlp_ffma",
-                "bound": "l2-gather", "achieved": gather_gbs, "peak": probe["gbps"], "unit": "GB/s",
-                "frac": gather_gbs / probe["gbps"], "traffic": traffic[0],
-                "peak_source": "measured live: nif_probe_gather, random 32 B sectors over a 32 MiB buffer, all SMs",
-                "algorithmic": f"{work['gathers_per_hit_ray']} gathers x 32 B sector per hit ray x "
+                "bound": "l2-gather" if l2_resident else "hbm-gather",
+                "achieved": useful_gbs, "peak": probe["gbps"], "unit": "GB/s",
+                "frac": useful_gbs / probe["gbps"], "traffic": traffic[0],
+                "peak_source": f"measured live: nif_probe_gather, independent random 32 B sectors over a "
+                               f"{probe_bytes >> 20} MiB buffer ({'L2' if l2_resident else 'HBM'}-resident like the table), all SMs; "
+                               "MEASURED_PEAKS.json has no gather figure (its HBM and tensor peaks are in .hbm / .tensor)",
+                "algorithmic": f"useful gather bytes (SURVEY 8(d).2): {work['gathers_per_hit_ray']} gathers x "
+                               f"{work['useful_gather_bytes'] // work['gathers_per_hit_ray']} B per hit ray x "
                                f"{hits_per_launch:.0f} hit rays per launch",
-                "frac_note": "per-lane gathers counted as one 32 B sector each (SURVEY 8(d).2 worst case); coherent "
-                             "rays share sectors and lines, so frac can exceed 1 -- see profiles/ for the sectors ncu counted",
+                "frac_note": "useful bytes delivered per second over the best rate at which the memory system delivers "
+                             "32 B sectors; the sectors ncu counted at L2 (profiles/) are within 8 % of the useful bytes "
+                             "on config 1 because binned rays share sectors",
+                "sector_worst_case": {"achieved": gather_gbs, "frac": gather_gbs / probe["gbps"],
+                                      "what": "every lane's gather counted as its own 32 B sector (SURVEY 8(d).2 worst case); "
+                                              "exceeds 1 when the 32 rays of a warp share sectors"},
                 "avg_launch_ms": net_ms, "share_of_step": net_ms * cfg.n_poses / ms_per_step,
                 "tensor": {"bound": "tensor", "achieved": tensor_tfs, "peak": peaks["tf_sustained"],
                            "unit": "TFLOP/s", "frac": tensor_tfs / peaks["tf_sustained"],
@@ -386,6 +412,9 @@ def run_ours(args) -> None:
                     "api": "nif_query_host (pinned host buffers, chunked, 3 streams)", "steps": e2e_steps},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "kernels": kernels,
             "mhit_rays_per_s": world * n_hit / (ms_per_step * 1e-3) / 1e6}
+    if walk_stats is not None:
+        line["config"]["walk"] = walk_stats
+        line["config"]["workload"] += f", multi-voxel walk max_steps={args.walk}"
     if base is not None:
         line["cpu_baseline"] = base
     print(json.dumps(line), flush=True)
@@ -406,6 +435,8 @@ def main() -> None:
     ap.add_argument("--ref-sample", type=int, default=32768, help="rays per step of --impl reference")
     ap.add_argument("--probe-table", action="store_true", help="run the gather probe over the real table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--walk", type=int, default=0, help="time nif_query_multi with this max_steps instead of nif_query "
+                                                        "(SURVEY 8(f) f1; not the headline; use --params varpres)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
