@@ -59,7 +59,12 @@ enum {
     /* Diagnostic: the tensor-core kernel fills its A operand with a constant instead of gathering from
      * the table, so a timed query measures the tcgen05 MLP pipeline alone (head outputs are then
      * meaningless).  bench.py --probe-mlp reports the tensor-pipe rate it reaches. */
-    NIF_PROBE_SKIP_GATHER   = 32u
+    NIF_PROBE_SKIP_GATHER   = 32u,
+    /* Distance head variant of P:87 ("We replace the sigmoid output with ReLU and regress
+     * log-transformed distances"; R24): y = ReLU(z1) is log(1 + D) of the ACCUMULATED distance, so
+     * dist_total = expm1(max(z1, 0)) and distance = dist_total - t_in.  Default is the
+     * scale-invariant head sigmoid(z1) * (t_out - t_in) (B:7; R14). */
+    NIF_DIST_LOG            = 64u
 };
 
 #define NIF_N_OUT 12   /* logits per ray: occlusion 1, distance 1, normal 3, albedo 3, material 4 (B:7) */
@@ -116,6 +121,12 @@ typedef struct {
     float* albedo;                /* 3n  sigmoid(z5..7)                                            */
     float* material_logits;       /* 4n  z8..11                                                    */
     float* raw_logits;            /* 12n optional                                                  */
+    /* Hit positions ("we reconstruct hit positions along the same segmented ray in rest space"),
+     * both optional (NULL to skip), zeros for a miss, not written with NIF_OCCLUSION_ONLY:          */
+    float* hit_position;          /* 3n  deformed space: o + dist_total * d                        */
+    float* hit_position_rest;     /* 3n  rest space, [-1,1]^3 coordinates: on the straight segment */
+                                  /*     between the rest images of entry and exit at the   */
+                                  /*     fraction clamp(distance / (t_out - t_in), 0, 1)           */
 } nif_query_out;
 
 typedef struct {

@@ -19,6 +19,7 @@ _SRC = _HERE / "nif_oracle.c"
 _CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
 
 FLAG_OCCLUSION_ONLY = 1
+FLAG_DIST_LOG = 2
 N_OUT = 12
 
 
@@ -88,6 +89,7 @@ class Oracle:
         L.nifo_walk_trace.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float,
                                       C.POINTER(_NetDesc), C.c_void_p, C.c_void_p, C.c_int64,
                                       C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.nifo_hit_positions.argtypes = [C.c_float, C.c_float, C.c_int64] + [C.c_void_p] * 9
         self.acc_bytes = L.nifo_acc_bytes()
 
     # ---- deformation -----------------------------------------------------------------
@@ -192,7 +194,7 @@ class Oracle:
         return out
 
     def query(self, nv, occ, lattice, bvh, pose, params, origin, direction,
-              occlusion_only=False, traverse_only=False):
+              occlusion_only=False, traverse_only=False, dist_log=False, hit_positions=False):
         """Whole pipeline.  bvh=None -> brute-force definition."""
         origin = _f32(origin); direction = _f32(direction)
         n = len(origin)
@@ -213,13 +215,26 @@ class Oracle:
                                  bvh.handle if bvh is not None else None,
                                  float(pose[0]), float(pose[1]), C.byref(d), table.ctypes.data, arr,
                                  n, origin.ctypes.data, direction.ctypes.data,
-                                 FLAG_OCCLUSION_ONLY if occlusion_only else 0,
+                                 (FLAG_OCCLUSION_ONLY if occlusion_only else 0) | (FLAG_DIST_LOG if dist_log else 0),
                                  g("voxel_id"), g("t_in"), g("t_out"), g("occlusion"), g("distance"),
                                  g("dist_total"), g("normal"), g("albedo"), g("material_logits"),
                                  g("raw_logits"))
         if rc != 0:
             raise RuntimeError(f"nifo_query failed: {rc}")
+        if hit_positions and not traverse_only and not occlusion_only:
+            o["hit_position"], o["hit_position_rest"] = self.hit_positions(pose, origin, direction, o)
         return o
+
+    def hit_positions(self, pose, origin, direction, res):
+        """O12: (deformed-space, rest-space) hit positions from a query's outputs."""
+        origin = _f32(origin); direction = _f32(direction)
+        n = len(origin)
+        hp = np.empty((n, 3), np.float32); hr = np.empty((n, 3), np.float32)
+        self.lib.nifo_hit_positions(float(pose[0]), float(pose[1]), n, origin.ctypes.data, direction.ctypes.data,
+                                    res["voxel_id"].ctypes.data, res["t_in"].ctypes.data, res["t_out"].ctypes.data,
+                                    res["distance"].ctypes.data, res["dist_total"].ctypes.data,
+                                    hp.ctypes.data, hr.ctypes.data)
+        return hp, hr
 
 
     def next_voxel_brute(self, nv, occ, lattice, origin, direction, after_t, after_id):

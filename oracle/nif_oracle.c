@@ -37,15 +37,18 @@
 #ifdef NIFO_ACC_DOUBLE
 typedef double acc_t;
 #define ACC_EXP exp
+#define ACC_EXPM1 expm1
 #define ACC_SQRT sqrt
 #else
 typedef float acc_t;
 #define ACC_EXP expf
+#define ACC_EXPM1 expm1f
 #define ACC_SQRT sqrtf
 #endif
 
 #define NIFO_N_OUT 12
 #define NIFO_FLAG_OCCLUSION_ONLY 1u
+#define NIFO_FLAG_DIST_LOG 2u       /* O10b: ReLU + log-transformed distance head (R24) */
 
 int nifo_acc_bytes(void) { return (int)sizeof(acc_t); }
 
@@ -719,11 +722,21 @@ static void nifo_eval_voxel(float theta_max, float bend_k, const nifo_net_desc* 
     } else {
         /* decode from the acc_t logits (not the float copies) */
         acc_t ell = (acc_t)(to - ti);
-        acc_t s = sigmoid_acc(z[1]);
-        acc_t dd = s * ell;
         *occlusion = (float)sigmoid_acc(z[0]);
-        *distance = (float)dd;
-        *dist_total = (float)((acc_t)ti + dd);
+        if (flags & NIFO_FLAG_DIST_LOG) {
+            /* O10b ("We replace the sigmoid output with ReLU and regress log-transformed distances";
+               R24): y = ReLU(z1) is the log-transformed ACCUMULATED distance, y = log(1 + D), so
+               D = exp(y) - 1 >= 0; the part inside the voxel is D - t_in. */
+            acc_t y = z[1] > (acc_t)0 ? z[1] : (acc_t)0;
+            acc_t D = ACC_EXPM1(y);
+            *dist_total = (float)D;
+            *distance = (float)(D - (acc_t)ti);
+        } else {
+            acc_t s = sigmoid_acc(z[1]);
+            acc_t dd = s * ell;
+            *distance = (float)dd;
+            *dist_total = (float)((acc_t)ti + dd);
+        }
         acc_t nn = z[2] * z[2] + z[3] * z[3] + z[4] * z[4];
         acc_t inv = (acc_t)1 / ACC_SQRT(nn > (acc_t)1e-24 ? nn : (acc_t)1e-24);
         for (int a = 0; a < 3; ++a) {
@@ -862,6 +875,33 @@ int nifo_walk_trace(int nv, const uint8_t* occ, const float* lattice, const void
         for (; k < max_steps; ++k) { trace_id[r * max_steps + k] = -1; trace_z0[r * max_steps + k] = 0.0f; }
     }
     return 0;
+}
+
+/* O12  Hit positions ("During evaluation, we reconstruct hit positions along the same segmented
+   ray in rest space").  From the outputs of the query: in deformed space the hit lies on the straight
+   ray at the accumulated distance, x = o + D d (one fma per coordinate); in rest space it lies on the
+   straight segment between the rest images of the voxel's entry and exit points (the local linear
+   approximation of P:43) at the fraction u = clamp(distance / l, 0, 1) of the segment (u = 0 if l = 0).
+   Miss: zeros (R18). */
+void nifo_hit_positions(float theta_max, float bend_k, int64_t n, const float* origin, const float* dir,
+                        const int32_t* vid, const float* t_in, const float* t_out,
+                        const float* distance, const float* dist_total, float* hit_pos, float* hit_rest)
+{
+    for (int64_t r = 0; r < n; ++r) {
+        const float* o = origin + 3 * r; const float* d = dir + 3 * r;
+        if (vid[r] < 0) { for (int a = 0; a < 3; ++a) { hit_pos[3 * r + a] = 0.0f; hit_rest[3 * r + a] = 0.0f; } continue; }
+        float Pi[3], Po[3], ri[3], ro[3];
+        for (int a = 0; a < 3; ++a) {
+            hit_pos[3 * r + a] = fmaf(dist_total[r], d[a], o[a]);
+            Pi[a] = fmaf(t_in[r], d[a], o[a]); Po[a] = fmaf(t_out[r], d[a], o[a]);
+        }
+        inverse_f32(theta_max, bend_k, Pi, ri);
+        inverse_f32(theta_max, bend_k, Po, ro);
+        float ell = t_out[r] - t_in[r];
+        float u = ell > 0.0f ? distance[r] / ell : 0.0f;
+        u = u < 0.0f ? 0.0f : (u > 1.0f ? 1.0f : u);
+        for (int a = 0; a < 3; ++a) hit_rest[3 * r + a] = fmaf(u, ro[a] - ri[a], ri[a]);
+    }
 }
 
 /* rest-space normalised endpoints of hit rays (exposed for the "inside the hit voxel's rest

@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libnif.so"
 
 NIF_F32, NIF_F16 = 0, 1
 NIF_OCCLUSION_ONLY, NIF_ENGINE_FFMA, NIF_TRAVERSE_ONLY = 1, 2, 4
-NIF_TRAVERSE_COHERENT, NIF_TRAVERSE_INCOHERENT, NIF_PROBE_SKIP_GATHER = 8, 16, 32
+NIF_TRAVERSE_COHERENT, NIF_TRAVERSE_INCOHERENT, NIF_PROBE_SKIP_GATHER, NIF_DIST_LOG = 8, 16, 32, 64
 NIF_N_OUT = 12
 NIF_WALK_MISS, NIF_WALK_HIT, NIF_WALK_MAX_STEPS = 0, 1, 2
 
@@ -47,7 +47,7 @@ class _RayBatch(C.Structure):
 
 
 _OUT_FIELDS = ["voxel_id", "t_in", "t_out", "occlusion", "distance", "dist_total", "normal",
-               "albedo", "material_logits", "raw_logits"]
+               "albedo", "material_logits", "raw_logits", "hit_position", "hit_position_rest"]
 
 
 class _QueryOut(C.Structure):
@@ -227,7 +227,8 @@ def nif_query_workspace_bytes(n: int) -> int:
     return b.value
 
 
-def alloc_outputs(n: int, device="cuda", raw_logits: bool = False, pinned_host: bool = False) -> dict:
+def alloc_outputs(n: int, device="cuda", raw_logits: bool = False, pinned_host: bool = False,
+                  hit_positions: bool = False) -> dict:
     kw = dict(device="cpu", pin_memory=True) if pinned_host else dict(device=device)
     o = {"voxel_id": torch.empty(n, dtype=torch.int32, **kw),
          "t_in": torch.empty(n, dtype=torch.float32, **kw),
@@ -240,6 +241,9 @@ def alloc_outputs(n: int, device="cuda", raw_logits: bool = False, pinned_host: 
          "material_logits": torch.empty(n, 4, dtype=torch.float32, **kw)}
     if raw_logits:
         o["raw_logits"] = torch.empty(n, NIF_N_OUT, dtype=torch.float32, **kw)
+    if hit_positions:
+        o["hit_position"] = torch.empty(n, 3, dtype=torch.float32, **kw)
+        o["hit_position_rest"] = torch.empty(n, 3, dtype=torch.float32, **kw)
     return o
 
 

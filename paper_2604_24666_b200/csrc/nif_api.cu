@@ -212,7 +212,7 @@ struct nif_stage {
     char* dev[NSLOT];            // one allocation per slot
     size_t slot_bytes, ws_bytes;
     // offsets inside a slot
-    size_t o_origin, o_dir, o_vid, o_tin, o_tout, o_occ, o_dist, o_dtot, o_nrm, o_alb, o_mat, o_raw, o_ws;
+    size_t o_origin, o_dir, o_vid, o_tin, o_tout, o_occ, o_dist, o_dtot, o_nrm, o_alb, o_mat, o_raw, o_hit, o_hitr, o_ws;
 };
 
 extern "C" int nif_stage_create(int64_t chunk_rays, nif_stage** out)
@@ -230,6 +230,7 @@ extern "C" int nif_stage_create(int64_t chunk_rays, nif_stage** out)
     s->o_vid = take(n * 4); s->o_tin = take(n * 4); s->o_tout = take(n * 4);
     s->o_occ = take(n * 4); s->o_dist = take(n * 4); s->o_dtot = take(n * 4);
     s->o_nrm = take(n * 12); s->o_alb = take(n * 12); s->o_mat = take(n * 16); s->o_raw = take(n * 48);
+    s->o_hit = take(n * 12); s->o_hitr = take(n * 12);
     nif_query_workspace_bytes(chunk_rays, &s->ws_bytes);
     s->o_ws = take(s->ws_bytes);
     s->slot_bytes = off;
@@ -278,6 +279,8 @@ extern "C" int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage*
         qo.dist_total = (float*)(d + st->o_dtot); qo.normal = (float*)(d + st->o_nrm);
         qo.albedo = (float*)(d + st->o_alb); qo.material_logits = (float*)(d + st->o_mat);
         qo.raw_logits = (heads && out->raw_logits) ? (float*)(d + st->o_raw) : nullptr;
+        qo.hit_position = (full && out->hit_position) ? (float*)(d + st->o_hit) : nullptr;
+        qo.hit_position_rest = (full && out->hit_position_rest) ? (float*)(d + st->o_hitr) : nullptr;
         rc = nif_query(bvh, net, &rb, &qo, d + st->o_ws, st->ws_bytes, flags, stream);
         if (rc != NIF_OK) return rc;
         auto back = [&](void* host, size_t host_off, size_t dev_off, size_t bytes) -> cudaError_t {
@@ -296,6 +299,8 @@ extern "C" int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage*
             NIF_CUDA_TRY(back(out->material_logits, b * 16, st->o_mat, mm * 16));
         }
         if (heads && out->raw_logits) NIF_CUDA_TRY(back(out->raw_logits, b * 48, st->o_raw, mm * 48));
+        if (qo.hit_position) NIF_CUDA_TRY(back(out->hit_position, b * 12, st->o_hit, mm * 12));
+        if (qo.hit_position_rest) NIF_CUDA_TRY(back(out->hit_position_rest, b * 12, st->o_hitr, mm * 12));
     }
     for (int i = 0; i < NSLOT; ++i) NIF_CUDA_TRY(cudaStreamSynchronize(st->stream[i]));
     return NIF_OK;

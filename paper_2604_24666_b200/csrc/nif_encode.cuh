@@ -115,8 +115,16 @@ __device__ __forceinline__ void nif_level_features(const T* __restrict__ level_t
 // (a5) heads from the 12 logits (B:7; R13, R16, R17)
 __device__ __forceinline__ float nif_sigmoid(float z) { return 1.0f / (1.0f + expf(-z)); }
 
+// what the optional hit-position outputs need beyond the logits
+struct NifDecodeCtx {
+    const float* origin;
+    const float* dir;
+    float theta_max, bend_k;
+};
+
 __device__ __forceinline__ void nif_decode_store(const float* __restrict__ z, float t_in, float t_out,
-                                                 long long ray, const nif_query_out& out, unsigned flags)
+                                                 long long ray, const nif_query_out& out, unsigned flags,
+                                                 const NifDecodeCtx& ctx)
 {
     out.occlusion[ray] = nif_sigmoid(z[0]);
     if (flags & NIF_OCCLUSION_ONLY) {
@@ -128,9 +136,16 @@ __device__ __forceinline__ void nif_decode_store(const float* __restrict__ z, fl
         return;
     }
     const float ell = t_out - t_in;
-    const float d = nif_sigmoid(z[1]) * ell;
+    float d, D;
+    if (flags & NIF_DIST_LOG) {                  // P:87, R24: ReLU output = log(1 + accumulated distance)
+        D = expm1f(fmaxf(z[1], 0.0f));
+        d = D - t_in;
+    } else {                                     // P:59-61, R14: local distance in [0, l], D = t_in + d
+        d = nif_sigmoid(z[1]) * ell;
+        D = t_in + d;
+    }
     out.distance[ray] = d;
-    out.dist_total[ray] = t_in + d;
+    out.dist_total[ray] = D;
     const float nn = z[2] * z[2] + z[3] * z[3] + z[4] * z[4];
     const float inv = rsqrtf(fmaxf(nn, 1e-24f));
 #pragma unroll
@@ -143,5 +158,23 @@ __device__ __forceinline__ void nif_decode_store(const float* __restrict__ z, fl
     if (out.raw_logits) {
 #pragma unroll
         for (int a = 0; a < NIF_N_OUT; ++a) out.raw_logits[NIF_N_OUT * ray + a] = z[a];
+    }
+    if (out.hit_position || out.hit_position_rest) {
+        const float ox = ctx.origin[3 * ray], oy = ctx.origin[3 * ray + 1], oz = ctx.origin[3 * ray + 2];
+        const float dx = ctx.dir[3 * ray], dy = ctx.dir[3 * ray + 1], dz = ctx.dir[3 * ray + 2];
+        if (out.hit_position) {
+            out.hit_position[3 * ray] = fmaf(D, dx, ox);
+            out.hit_position[3 * ray + 1] = fmaf(D, dy, oy);
+            out.hit_position[3 * ray + 2] = fmaf(D, dz, oz);
+        }
+        if (out.hit_position_rest) {
+            float ix, iy, iz, ex, ey, ez;
+            nif_inverse_deform(ctx.theta_max, ctx.bend_k, fmaf(t_in, dx, ox), fmaf(t_in, dy, oy), fmaf(t_in, dz, oz), ix, iy, iz);
+            nif_inverse_deform(ctx.theta_max, ctx.bend_k, fmaf(t_out, dx, ox), fmaf(t_out, dy, oy), fmaf(t_out, dz, oz), ex, ey, ez);
+            const float u = ell > 0.0f ? __saturatef(d / ell) : 0.0f;
+            out.hit_position_rest[3 * ray] = fmaf(u, ex - ix, ix);
+            out.hit_position_rest[3 * ray + 1] = fmaf(u, ey - iy, iy);
+            out.hit_position_rest[3 * ray + 2] = fmaf(u, ez - iz, iz);
+        }
     }
 }

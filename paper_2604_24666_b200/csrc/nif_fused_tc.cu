@@ -476,7 +476,7 @@ k_fused_encode_mlp(const TcParams p)
                 float z[NIF_N_OUT];
 #pragma unroll
                 for (int a = 0; a < NIF_N_OUT; ++a) z[a] = __uint_as_float(zr[a]);
-                nif_decode_store(z, cur_ti, cur_to, cur_ray, p.out, p.flags);
+                nif_decode_store(z, cur_ti, cur_to, cur_ray, p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.theta_max, p.bend_k});
             }
         }
     } else if (warp == TC_MMA_WARP) {

@@ -144,7 +144,7 @@ k_encode_mlp_ffma(const FfmaParams p)
             float z[NIF_N_OUT];
 #pragma unroll
             for (int a = 0; a < NIF_N_OUT; ++a) z[a] = a < p.n_out ? nxt[r * 16 + a] : 0.0f;
-            nif_decode_store(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags);
+            nif_decode_store(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.theta_max, p.bend_k});
         }
         __syncthreads();
     }

@@ -179,6 +179,11 @@ __device__ __forceinline__ void retire_ray(const TravParams& p, long long ray, i
             for (int a = 0; a < 3; ++a) { p.out.normal[3 * ray + a] = 0.0f; p.out.albedo[3 * ray + a] = 0.0f; }
 #pragma unroll
             for (int a = 0; a < 4; ++a) p.out.material_logits[4 * ray + a] = 0.0f;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                if (p.out.hit_position) p.out.hit_position[3 * ray + a] = 0.0f;
+                if (p.out.hit_position_rest) p.out.hit_position_rest[3 * ray + a] = 0.0f;
+            }
         }
         if (p.out.raw_logits) {
 #pragma unroll

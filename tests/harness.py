@@ -48,9 +48,9 @@ def make_case(cfg_id: int, n_rays: int | None = None, variant: str = "varpres", 
                 torch.from_numpy(o).cuda(), torch.from_numpy(d).cuda())
 
 
-def run_gpu(case: Case, flags: int = 0, raw_logits: bool = True) -> dict:
+def run_gpu(case: Case, flags: int = 0, raw_logits: bool = True, hit_positions: bool = False) -> dict:
     n = len(case.origin)
-    out = nif.alloc_outputs(n, raw_logits=raw_logits)
+    out = nif.alloc_outputs(n, raw_logits=raw_logits, hit_positions=hit_positions)
     for v in out.values():
         v.fill_(float("nan") if v.dtype.is_floating_point else -7)     # poison: everything must be written
     ws = nif.nif_query(case.bvh, case.net, case.origin_d, case.direction_d, out, flags=flags)
@@ -68,12 +68,12 @@ class OracleSide:
         self.lattice = oracle.deform_lattice(case.cfg.nv, float(case.pose[0]), float(case.pose[1]))
         self.bvh = oracle.bvh_build(case.cfg.nv, case.occ, self.lattice)
 
-    def query(self, idx=None, occlusion_only=False, traverse_only=False) -> dict:
+    def query(self, idx=None, occlusion_only=False, traverse_only=False, **kw) -> dict:
         c = self.case
         o = c.origin if idx is None else c.origin[idx]
         d = c.direction if idx is None else c.direction[idx]
         return self.oracle.query(c.cfg.nv, c.occ, self.lattice, self.bvh, c.pose, c.params, o, d,
-                                 occlusion_only=occlusion_only, traverse_only=traverse_only)
+                                 occlusion_only=occlusion_only, traverse_only=traverse_only, **kw)
 
 
 def subset(res: dict, idx) -> dict:
