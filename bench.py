@@ -246,6 +246,16 @@ def run_ours(args) -> None:
         o, d = I.rays(cfg, pi, info["lo"], info["hi"])
         poses.append({"bvh": bvh, "o_h": torch.from_numpy(o).pin_memory(), "d_h": torch.from_numpy(d).pin_memory(),
                       "o": torch.from_numpy(o).to(dev), "d": torch.from_numpy(d).to(dev)})
+    # refit (same voxel set, new pose): back to the first pose's neighbour and home again, timed
+    refit_ms = []
+    for pi in range(cfg.n_poses):
+        th, kk = float(pose_list[pi][0]), float(pose_list[pi][1])
+        poses[pi]["bvh"].refit(th * 0.5, kk * 0.5)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        poses[pi]["bvh"].refit(th, kk)
+        e1.record(); torch.cuda.synchronize()
+        refit_ms.append(e0.elapsed_time(e1))
     n_per_pose = cfg.rays_per_pose
     n_total = n_per_pose * cfg.n_poses
     out = nif.alloc_outputs(n_per_pose, device=dev)
@@ -396,7 +406,8 @@ def run_ours(args) -> None:
             "achieved": tf, "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": tf / peaks["tf_burst"],
             "peak_source": f"{peaks['source']} bf16 burst (fp16 same pipe)"}
     kernels = {"traverse_ms": trav_ms, "encode_mlp_ms": net_ms, "traverse_share": trav_ms * cfg.n_poses / ms_per_step,
-               "bvh_build_ms_per_pose": float(np.median(build_ms))}
+               "bvh_build_ms_per_pose": float(np.median(build_ms)),
+               "bvh_refit_ms_per_pose": float(np.median(refit_ms))}
 
     base = cpu_baseline(cfg, args.params) if (world == 1 and not args.no_cpu_baseline) else None
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

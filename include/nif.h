@@ -155,6 +155,14 @@ int nif_bvh_workspace_bytes(int32_t nv, int64_t max_occupied, size_t* bytes);
 int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_deform_params* pose,
                            void* workspace, size_t workspace_bytes, void* stream, nif_bvh** out);
 
+/* New pose for the same voxel set: recomputes the deformed corner lattice and every box of the
+ * hierarchy in place; the topology (which is the sparse octree of the REST lattice) is reused, so no
+ * occupancy pass, scan or allocation happens.  The result is bit-identical to a fresh
+ * nif_build_deformed_bvh with that pose.  SYNCHRONISES `stream` (reads the root box back).  On
+ * NIF_ERR_DEFORM_SINGULAR the BVH keeps its previous pose.  Queries enqueued earlier on another
+ * stream must have finished. */
+int nif_bvh_refit(nif_bvh* bvh, const nif_deform_params* pose, void* stream);
+
 int nif_bvh_get_info(const nif_bvh* bvh, nif_bvh_info* info);      /* host-only */
 
 /* DEVICE pointer to the deformed corner lattice: (nv+1)^3 float4 (x,y,z,0), lattice point

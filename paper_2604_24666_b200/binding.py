@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
         L.nif_bvh_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_build_deformed_bvh.argtypes = [C.POINTER(_VoxelSet), C.POINTER(_DeformParams), C.c_void_p,
                                              C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
+        L.nif_bvh_refit.argtypes = [C.c_void_p, C.POINTER(_DeformParams), C.c_void_p]
         L.nif_bvh_get_info.argtypes = [C.c_void_p, C.POINTER(_BvhInfo)]
         L.nif_bvh_get_lattice.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
         L.nif_bvh_destroy.argtypes = [C.c_void_p]
@@ -148,6 +149,11 @@ class Bvh:
         return {"nv": i.nv, "n_occupied": i.n_occupied, "n_nodes": i.n_nodes, "depth": i.depth,
                 "lo": np.array(list(i.lo), np.float32), "hi": np.array(list(i.hi), np.float32),
                 "theta_max": i.theta_max, "bend_k": i.bend_k}
+
+    def refit(self, theta_max: float, bend_k: float, stream=None):
+        """nif_bvh_refit: new pose, same voxel set (synchronises)."""
+        dp = _DeformParams(float(theta_max), float(bend_k))
+        _check(lib().nif_bvh_refit(self.handle, C.byref(dp), _stream_ptr(stream)), "nif_bvh_refit")
 
     def lattice(self) -> torch.Tensor:
         """Copy of the deformed corner lattice, [(nv+1)^3, 3] float32 (for parity tests)."""

@@ -321,6 +321,57 @@ int device_is_sm100()
     return major == 10;
 }
 
+// fold-over check (R7): the twist keeps y, so the largest k*y over occupied corners is
+// k * rest-y of the highest occupied corner.
+bool pose_folds_over(const nif_deform_params* pose, int nv, uint32_t top_iy)
+{
+    if (fabsf(pose->bend_k) < 1e-6f) return false;
+    double ytop = (2.0 * (double)top_iy - nv) / nv;
+    double ybot = -1.0;                           // k < 0 folds at the bottom; be conservative
+    double worst = pose->bend_k > 0 ? (double)pose->bend_k * ytop : (double)pose->bend_k * ybot;
+    return worst >= 1.0 - 1e-3;
+}
+
+void launch_deform(int nv, const nif_deform_params* pose, float4* lattice, cudaStream_t stream)
+{
+    const size_t np1 = (size_t)nv + 1, total = np1 * np1 * np1;
+    int blocks = (int)((total + 255) / 256);
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    k_deform_lattice<<<blocks, 256, 0, stream>>>(nv, (double)pose->twist_theta_max, (double)pose->bend_k, lattice);
+    nif_count_launch(1);
+}
+
+// boxes of every node from the deformed lattice, bottom-up, with the topology (masks, scan offsets,
+// node ranges) already in the workspace; reads the root box back (SYNCHRONISES).
+int write_levels(nif_bvh* b, const BuildLayout& L, cudaStream_t stream)
+{
+    char* ws = b->ws;
+    NifNode* nodes = (NifNode*)(ws + L.off_nodes);
+    float4* boxes = (float4*)(ws + L.off_nodes + align_up(b->node_capacity * sizeof(NifNode), 256));
+    const float4* lattice = (const float4*)(ws + L.off_lattice);
+    for (int l = 1; l <= L.levels; ++l) {
+        const uint32_t c = (uint32_t)L.cells[l];
+        const uint8_t* mask = (const uint8_t*)(ws + L.off_mask[l]);
+        const uint32_t* offs = (const uint32_t*)(ws + L.off_offs[l]);
+        if (l == 1)
+            k_write_bricks<<<(c + 127) / 128, 128, 0, stream>>>(b->nv, c, mask, offs, b->level_base[1], lattice, nodes, boxes);
+        else
+            k_write_level<<<(c + 127) / 128, 128, 0, stream>>>(
+                c, mask, offs, b->level_base[l], (const uint8_t*)(ws + L.off_mask[l - 1]),
+                (const uint32_t*)(ws + L.off_offs[l - 1]), b->level_base[l - 1], nodes, boxes);
+        nif_count_launch(1);
+    }
+    b->root = (int32_t)b->level_base[L.levels];
+    float4 rb[2];
+    cudaError_t e = cudaMemcpyAsync(rb, boxes + 2 * (size_t)b->root, sizeof(rb), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return NIF_ERR_CUDA; }
+    b->lo[0] = rb[0].x; b->lo[1] = rb[0].y; b->lo[2] = rb[0].z;
+    b->hi[0] = rb[1].x; b->hi[1] = rb[1].y; b->hi[2] = rb[1].z;
+    return NIF_OK;
+}
+
 }  // namespace
 
 extern "C" int nif_device_supported(void) { return device_is_sm100(); }
@@ -355,14 +406,7 @@ extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_def
     const size_t node_capacity = (workspace_bytes - L.off_nodes) / NODE_BYTES;
 
     NIF_CUDA_TRY(cudaMemsetAsync(counters, 0, 64 * sizeof(uint32_t), stream));
-    {
-        const size_t np1 = (size_t)nv + 1, total = np1 * np1 * np1;
-        int blocks = (int)((total + 255) / 256);
-        if (blocks > 148 * 32) blocks = 148 * 32;
-        k_deform_lattice<<<blocks, 256, 0, stream>>>(nv, (double)pose->twist_theta_max,
-                                                     (double)pose->bend_k, lattice);
-        nif_count_launch(1);
-    }
+    launch_deform(nv, pose, lattice, stream);
     for (int l = 1; l <= L.levels; ++l) {
         const uint32_t c = (uint32_t)L.cells[l];
         uint8_t* mask = (uint8_t*)(ws + L.off_mask[l]);
@@ -383,14 +427,7 @@ extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_def
     NIF_CUDA_TRY(cudaGetLastError());
 
     const uint32_t n_occ = h_counters[0];
-    // fold-over check (R7): the twist keeps y, so the largest k*y over occupied corners
-    // is k * rest-y of the highest occupied corner.
-    if (n_occ && fabsf(pose->bend_k) >= 1e-6f) {
-        double ytop = (2.0 * (double)h_counters[1] - nv) / nv;
-        double ybot = -1.0;                       // k < 0 folds at the bottom; be conservative
-        double worst = pose->bend_k > 0 ? (double)pose->bend_k * ytop : (double)pose->bend_k * ybot;
-        if (worst >= 1.0 - 1e-3) return NIF_ERR_DEFORM_SINGULAR;
-    }
+    if (n_occ && pose_folds_over(pose, nv, h_counters[1])) return NIF_ERR_DEFORM_SINGULAR;
     uint32_t base[12] = {0};
     size_t n_nodes = 0;
     for (int l = 1; l <= L.levels; ++l) { base[l] = (uint32_t)n_nodes; n_nodes += h_counters[2 + l]; }
@@ -407,29 +444,30 @@ extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_def
     b->theta_max = pose->twist_theta_max; b->bend_k = pose->bend_k;
     b->lattice = lattice; b->nodes = nodes;
     for (int a = 0; a < 3; ++a) { b->lo[a] = 0.f; b->hi[a] = 0.f; }
+    b->ws = ws; b->node_capacity = node_capacity; b->top_iy = h_counters[1];
+    for (int l = 0; l < 12; ++l) b->level_base[l] = base[l];
     if (n_occ) {
-        for (int l = 1; l <= L.levels; ++l) {
-            const uint32_t c = (uint32_t)L.cells[l];
-            const uint8_t* mask = (const uint8_t*)(ws + L.off_mask[l]);
-            const uint32_t* offs = (const uint32_t*)(ws + L.off_offs[l]);
-            if (l == 1)
-                k_write_bricks<<<(c + 127) / 128, 128, 0, stream>>>(nv, c, mask, offs, base[1], lattice, nodes, boxes);
-            else
-                k_write_level<<<(c + 127) / 128, 128, 0, stream>>>(
-                    c, mask, offs, base[l], (const uint8_t*)(ws + L.off_mask[l - 1]),
-                    (const uint32_t*)(ws + L.off_offs[l - 1]), base[l - 1], nodes, boxes);
-            nif_count_launch(1);
-        }
-        b->root = (int32_t)base[L.levels];
-        float4 rb[2];
-        cudaError_t e = cudaMemcpyAsync(rb, boxes + 2 * (size_t)b->root, sizeof(rb), cudaMemcpyDeviceToHost, stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
-        if (e == cudaSuccess) e = cudaGetLastError();
-        if (e != cudaSuccess) { (void)cudaGetLastError(); delete b; return NIF_ERR_CUDA; }
-        b->lo[0] = rb[0].x; b->lo[1] = rb[0].y; b->lo[2] = rb[0].z;
-        b->hi[0] = rb[1].x; b->hi[1] = rb[1].y; b->hi[2] = rb[1].z;
+        int rc = write_levels(b, L, stream);
+        if (rc != NIF_OK) { delete b; return rc; }
     }
     *out = b;
+    return NIF_OK;
+}
+
+// Same voxel set, new pose: the hierarchy's topology is the rest lattice's octree (pose-independent),
+// so only the corner lattice and the boxes are recomputed.
+extern "C" int nif_bvh_refit(nif_bvh* b, const nif_deform_params* pose, void* stream_)
+{
+    if (!b || !pose) return NIF_ERR_INVALID_ARG;
+    if (!isfinite(pose->twist_theta_max) || !isfinite(pose->bend_k)) return NIF_ERR_INVALID_ARG;
+    if (!device_is_sm100()) return NIF_ERR_UNSUPPORTED;
+    if (b->n_occupied && pose_folds_over(pose, b->nv, b->top_iy)) return NIF_ERR_DEFORM_SINGULAR;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const BuildLayout L = make_layout(b->nv);
+    launch_deform(b->nv, pose, (float4*)(b->ws + L.off_lattice), stream);
+    b->theta_max = pose->twist_theta_max; b->bend_k = pose->bend_k;
+    if (b->n_occupied) return write_levels(b, L, stream);
+    NIF_CUDA_TRY(cudaStreamSynchronize(stream));
     return NIF_OK;
 }
 

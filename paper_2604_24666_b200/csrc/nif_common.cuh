@@ -38,6 +38,11 @@ struct nif_bvh {
     float theta_max, bend_k;
     const float4* lattice; // device, (nv+1)^3
     const NifNode* nodes;  // device
+    // kept for nif_bvh_refit: the topology (masks, offsets, node ranges) is pose-independent
+    char* ws;              // caller workspace the BVH lives in
+    size_t node_capacity;
+    uint32_t level_base[12];
+    uint32_t top_iy;       // max (iy+1) over occupied voxels: fold-over check (R7)
 };
 
 // Encoding geometry handed to kernels by value.
