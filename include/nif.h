@@ -93,7 +93,8 @@ typedef struct {
     int32_t pe_bands;             /* B: sinusoidal bands (the paper's "F"), 0..8          */
     int32_t levels;               /* L: hash-grid levels, 1..16                                 */
     int32_t log2_T;               /* table entries per level = 2^log2_T, 4..24                  */
-    int32_t feat;                 /* F: features per entry: 1, 2 or 4 (NIF_F16: 2 or 4)         */
+    int32_t feat;                 /* F: features per entry, 1..4.  F = 3 (the paper's own setup) is
+                                   * stored padded to 4 inside the library: the table is then COPIED   */
     const int32_t* level_res;     /* HOST, `levels` entries: grid resolution N_l of each level  */
     int32_t hidden_layers;        /* H: 1..8                                                    */
     int32_t width;                /* W: 16..128, multiple of 16                                 */
@@ -174,7 +175,8 @@ void nif_bvh_destroy(nif_bvh* bvh);                                /* frees the 
 /* -------- network ------------------------------------------------------------------------ */
 
 /* `table`: DEVICE, layout table[l][index][f], every level 2^log2_T entries, float (NIF_F32) or
- * __half (NIF_F16); borrowed for the lifetime of the net (not copied).
+ * __half (NIF_F16); borrowed for the lifetime of the net (not copied, except feat = 3: the
+ * library keeps its own copy padded to 4 features per entry, levels * 2^log2_T * 4 elements).
  * `weights`: HOST array of hidden_layers+1 DEVICE pointers; weights[i] is row-major
  * (fan_out, fan_in): (W, D_in), (W, W)..., (12, W); same element type as the table.  Copied and
  * repacked on `stream` (tensor-core operand images, zero-padded output layer).  SYNCHRONISES. */

@@ -87,6 +87,12 @@ _NET1 = NetShape(pe_bands=6, levels=16, log2_T=19, feat=2, base_res=16, growth=1
 _NET4 = NetShape(pe_bands=6, levels=16, log2_T=22, feat=4, base_res=16, growth=1.38,
                  hidden_layers=4, width=128, dtype="f16")
 
+# The paper's own experimental shape: "voxel resolution 32^3, a two-level hash grid (base 64,
+# feature dim 3), and F=3 positional encoding bands".  Table size, growth and the MLP are not stated:
+# T = 2^19, growth 2 (levels 64 dense, 128 hashed) and config 1's 3x64 fp16 MLP are assumed (R26).
+_NET5 = NetShape(pe_bands=3, levels=2, log2_T=19, feat=3, base_res=64, growth=2.0,
+                 hidden_layers=3, width=64, dtype="f16")
+
 CONFIGS = {
     0: Config(0, "tiny", 16, _NET0, 1, 4096, "sphere_to_cube",
               geom_seed=0, net_seed=0, ray_seed=0),
@@ -98,6 +104,9 @@ CONFIGS = {
               occlusion_only=True, geom_seed=2, pose_seed=1, net_seed=11, ray_seed=3),
     4: Config(4, "large_4k", 256, _NET4, 1, 3840 * 2160, "camera",
               image_wh=(3840, 2160), geom_seed=4, net_seed=14, ray_seed=4),
+    # not a BASELINE.json config: the paper's shape on config 1's kind of object and camera
+    5: Config(5, "paper_shape_32", 32, _NET5, 1, 1920 * 1080, "camera",
+              image_wh=(1920, 1080), geom_seed=1, net_seed=15, ray_seed=5),
 }
 
 
@@ -125,7 +134,7 @@ def occupancy(cfg: Config) -> np.ndarray:
     if cfg.cfg_id == 0:                                   # ball of radius 0.8 (B:7)
         z, y, x = np.meshgrid(c, c, c, indexing="ij")
         occ = (x * x + y * y + z * z) <= 0.8 * 0.8
-    elif cfg.cfg_id == 1:                                 # 8 Gaussian blobs, threshold 0.5 (B:8)
+    elif cfg.cfg_id in (1, 5):                            # 8 Gaussian blobs, threshold 0.5 (B:8)
         rng = np.random.default_rng(cfg.geom_seed)
         ctr = rng.uniform(-0.5, 0.5, size=(8, 3))
         sig = rng.uniform(0.12, 0.25, size=8)
@@ -179,6 +188,8 @@ def poses(cfg: Config) -> np.ndarray:
              for _ in range(cfg.n_poses)]
     elif cfg.cfg_id == 4:
         p = [[math.pi, 1.2]]                              # B:11
+    elif cfg.cfg_id == 5:
+        p = [[0.6, 0.5]]                                  # a twist followed by a bend (paper shape, not in BASELINE)
     else:
         raise ValueError(cfg.cfg_id)
     return np.asarray(p, dtype=np.float32)

@@ -33,6 +33,28 @@ extern "C" const char* nif_error_string(int status)
 // ---------------------------------------------------------------------------------------------
 // network
 // ---------------------------------------------------------------------------------------------
+namespace {
+// feat == 3 (the paper's own configuration, "feature dim 3"): entries are stored padded to 4
+// features (8- or 16-byte aligned vector loads) and the first layer gets a zero column per pad
+// feature, so the network function is unchanged.
+template <typename T>
+__global__ void k_pad_table_3to4(const T* __restrict__ src, T* __restrict__ dst, size_t n_entries)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_entries) return;
+    dst[4 * i] = src[3 * i]; dst[4 * i + 1] = src[3 * i + 1]; dst[4 * i + 2] = src[3 * i + 2];
+    dst[4 * i + 3] = (T)0.0f;
+}
+template <typename T>
+__global__ void k_pad_w1_3to4(const T* __restrict__ src, T* __restrict__ dst, int rows, int groups)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;        // over rows * groups * 4
+    if (i >= rows * groups * 4) return;
+    const int f = i & 3, g = (i >> 2) % groups, r = i / (groups * 4);
+    dst[i] = f < 3 ? src[(size_t)r * groups * 3 + (size_t)g * 3 + f] : (T)0.0f;
+}
+}  // namespace
+
 static int validate_desc(const nif_net_desc* d)
 {
     if (!d || !d->level_res) return NIF_ERR_INVALID_ARG;
@@ -43,7 +65,7 @@ static int validate_desc(const nif_net_desc* d)
     if (d->dtype != NIF_F32 && d->dtype != NIF_F16) return NIF_ERR_INVALID_ARG;
     for (int l = 0; l < d->levels; ++l)
         if (d->level_res[l] < 1 || d->level_res[l] > (1 << 20)) return NIF_ERR_INVALID_ARG;
-    if (d->feat != 1 && d->feat != 2 && d->feat != 4) return NIF_ERR_UNSUPPORTED;
+    if (d->feat < 1 || d->feat > 4) return NIF_ERR_UNSUPPORTED;
     if (d->width < 16 || d->width > 128 || (d->width % 16) != 0) return NIF_ERR_UNSUPPORTED;
     return NIF_OK;
 }
@@ -73,19 +95,47 @@ extern "C" int nif_net_create(const nif_net_desc* desc, const void* table, const
         const unsigned long long np1 = (unsigned long long)desc->level_res[l] + 1ull;   // 64-bit compare (R6)
         if (np1 * np1 * np1 <= T) net->enc.dense_mask |= 1u << l;
     }
-    net->d_in = 2 * (1 + 2 * desc->pe_bands) * desc->levels * desc->feat;
+    const bool pad3 = desc->feat == 3;
+    const int feat = pad3 ? 4 : desc->feat;
+    net->desc.feat = feat; net->enc.feat = feat;
+    const int groups = 2 * (1 + 2 * desc->pe_bands) * desc->levels;      // (endpoint, sample, level) triples
+    net->d_in = groups * feat;
     net->table = table;
     const size_t eb = elem_bytes(desc->dtype);
+    if (pad3) {
+        const size_t n_entries = (size_t)desc->levels << desc->log2_T;
+        if (cudaMalloc(&net->table_owned, n_entries * 4 * eb) != cudaSuccess) {
+            (void)cudaGetLastError(); nif_net_destroy(net); return NIF_ERR_CUDA;
+        }
+        const unsigned blocks = (unsigned)((n_entries + 255) / 256);
+        if (desc->dtype == NIF_F16)
+            k_pad_table_3to4<__half><<<blocks, 256, 0, stream>>>((const __half*)table, (__half*)net->table_owned, n_entries);
+        else
+            k_pad_table_3to4<float><<<blocks, 256, 0, stream>>>((const float*)table, (float*)net->table_owned, n_entries);
+        nif_count_launch(1);
+        net->table = net->table_owned;
+    }
     for (int i = 0; i <= desc->hidden_layers; ++i) {
         const size_t fan_out = i == desc->hidden_layers ? NIF_N_OUT : (size_t)desc->width;
         const size_t fan_in = i == 0 ? (size_t)net->d_in : (size_t)desc->width;
         const size_t bytes = fan_out * fan_in * eb;
         cudaError_t e = cudaMalloc(&net->w_plain[i], bytes);
-        if (e == cudaSuccess)
-            e = cudaMemcpyAsync(net->w_plain[i], weights[i], bytes, cudaMemcpyDeviceToDevice, stream);
+        if (e == cudaSuccess) {
+            if (i == 0 && pad3) {
+                const int total = (int)fan_out * groups * 4;
+                if (desc->dtype == NIF_F16)
+                    k_pad_w1_3to4<__half><<<(total + 255) / 256, 256, 0, stream>>>((const __half*)weights[0], (__half*)net->w_plain[0], (int)fan_out, groups);
+                else
+                    k_pad_w1_3to4<float><<<(total + 255) / 256, 256, 0, stream>>>((const float*)weights[0], (float*)net->w_plain[0], (int)fan_out, groups);
+                nif_count_launch(1);
+                e = cudaGetLastError();
+            } else {
+                e = cudaMemcpyAsync(net->w_plain[i], weights[i], bytes, cudaMemcpyDeviceToDevice, stream);
+            }
+        }
         if (e != cudaSuccess) { (void)cudaGetLastError(); nif_net_destroy(net); return NIF_ERR_CUDA; }
     }
-    net->tc_supported = nif_tc_supported(desc);
+    net->tc_supported = nif_tc_supported(&net->desc);
     if (net->tc_supported) {
         rc = nif_tc_pack_weights(net, stream);
         if (rc != NIF_OK) { nif_net_destroy(net); return rc; }
@@ -101,6 +151,7 @@ extern "C" void nif_net_destroy(nif_net* net)
     for (int i = 0; i < NIF_MAX_LAYERS; ++i)
         if (net->w_plain[i]) cudaFree(net->w_plain[i]);
     if (net->w_tc) cudaFree(net->w_tc);
+    if (net->table_owned) cudaFree(net->table_owned);
     delete net;
 }
 

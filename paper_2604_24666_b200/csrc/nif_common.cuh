@@ -56,7 +56,8 @@ struct nif_net {
     nif_net_desc desc;
     NifEnc enc;
     int32_t d_in;
-    const void* table;                 // borrowed device pointer
+    const void* table;                 // borrowed device pointer (or table_owned)
+    void* table_owned;                 // feat == 3: the library's copy padded to 4 features per entry
     void* w_plain[NIF_MAX_LAYERS];     // device copies, row-major (fan_out, fan_in), net dtype
     void* w_tc;                        // device: tensor-core operand images (NIF_F16 only)
     size_t w_tc_bytes;

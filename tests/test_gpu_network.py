@@ -163,6 +163,8 @@ SHAPES = [  # (pe_bands, levels, log2_T, feat, base_res, growth, hidden_layers, 
     (1, 16, 15, 4, 8, 1.3, 3, 64),     # L*F = 64: one sample per K chunk
     (5, 4, 13, 2, 16, 1.7, 5, 128),    # L*F = 8, W = 128, deep
     (0, 16, 16, 2, 16, 1.38, 2, 64),   # no positional bands: S = 1, a single (padded) K chunk per endpoint pair
+    (3, 2, 19, 3, 64, 2.0, 3, 64),     # the paper's own shape: two levels, F = 3 (stored padded to 4), B = 3
+    (2, 8, 14, 3, 8, 1.5, 2, 32),      # F = 3, L*F(padded) = 32
 ]
 
 
@@ -182,6 +184,30 @@ def test_tensor_core_kernel_shape_sweep(oracle, H, P, nif, shape):
         m = P.compare_network(gpu, ref, fp16=True)
         P.assert_network(m, fp16=True)
         assert m["n_hit"] > 500, (name, m)
+
+
+@pytest.mark.parametrize("variant", ["uniform0.1", "varpres"])
+def test_paper_shape_config5(oracle, H, P, nif, variant):
+    """32^3 voxels, two-level hash grid (base 64, feature dim 3), 3 PE bands."""
+    case = H.make_case(5, n_rays=40_000, variant=variant)
+    assert nif.nif_net_uses_tensor_cores(case.net)
+    ref = H.OracleSide(oracle, case).query()
+    for name, fl in _engines(nif, case):
+        gpu = H.run_gpu(case, flags=fl)
+        P.assert_traversal(P.compare_traversal(gpu, ref))
+        m = P.compare_network(gpu, ref, fp16=True)
+        P.assert_network(m, fp16=True)
+        assert m["n_hit"] > 2000, (name, m)
+
+
+def test_three_features_fp32(oracle, H, P, nif):
+    net = I.NetShape(pe_bands=2, levels=3, log2_T=12, feat=3, base_res=4, growth=2.0,
+                     hidden_layers=2, width=32, dtype="f32")
+    case = H.make_case(0, cfg=I.scaled(I.get_config(0), net=net))
+    ref = H.OracleSide(oracle, case).query()
+    gpu = H.run_gpu(case)
+    P.assert_traversal(P.compare_traversal(gpu, ref))
+    P.assert_network(P.compare_network(gpu, ref, fp16=False), fp16=False)
 
 
 def test_empty_batch_is_a_no_op(H, nif):
