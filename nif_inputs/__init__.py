@@ -35,13 +35,16 @@ class NetShape:
     hidden_layers: int  # H
     width: int          # W
     dtype: str          # "f32" | "f16"  (parameter storage / MMA operand type)
+    enc_mode: str = "compose"   # "compose": psi = phi(gamma(x)) (Eq. 1, R1); "concat": psi = [gamma(x), phi(x)]
 
     @property
     def samples(self) -> int:          # S = 1 + 2B three-vectors per endpoint
         return 1 + 2 * self.pe_bands
 
     @property
-    def d_in(self) -> int:             # 2 endpoints * S * L * F
+    def d_in(self) -> int:             # 2 endpoints * S * L * F  (concat: 2 * (3 + 6B + L * F))
+        if self.enc_mode == "concat":
+            return 2 * (3 + 6 * self.pe_bands + self.levels * self.feat)
         return 2 * self.samples * self.levels * self.feat
 
     @property

@@ -39,7 +39,7 @@ def build(force: bool = False) -> dict:
 class _NetDesc(C.Structure):
     _fields_ = [("pe_bands", C.c_int32), ("levels", C.c_int32), ("log2_T", C.c_int32),
                 ("feat", C.c_int32), ("hidden_layers", C.c_int32), ("width", C.c_int32),
-                ("level_res", C.POINTER(C.c_int32))]
+                ("level_res", C.POINTER(C.c_int32)), ("enc_mode", C.c_int32)]
 
 
 def _f32(a):
@@ -133,7 +133,8 @@ class Oracle:
     def _desc(self, shape, level_res):
         lr = np.ascontiguousarray(level_res, dtype=np.int32)
         d = _NetDesc(shape.pe_bands, shape.levels, shape.log2_T, shape.feat,
-                     shape.hidden_layers, shape.width, lr.ctypes.data_as(C.POINTER(C.c_int32)))
+                     shape.hidden_layers, shape.width, lr.ctypes.data_as(C.POINTER(C.c_int32)),
+                     1 if getattr(shape, "enc_mode", "compose") == "concat" else 0)
         d._keep = lr
         return d
 
@@ -155,7 +156,7 @@ class Oracle:
         xn = _f32(xn).reshape(-1, 3)
         d = self._desc(sh, params.level_res)
         table = _f32(params.table)
-        out = np.empty((len(xn), sh.samples * sh.levels * sh.feat), np.float32)
+        out = np.empty((len(xn), sh.d_in // 2), np.float32)
         self.lib.nifo_encode(C.byref(d), table.ctypes.data, len(xn), xn.ctypes.data, out.ctypes.data)
         return out
 

@@ -522,7 +522,15 @@ typedef struct {
     int32_t pe_bands, levels, log2_T, feat;
     int32_t hidden_layers, width;
     const int32_t* level_res;                 /* N_l, L entries */
+    int32_t enc_mode;                         /* 0: psi = phi(gamma(x)) (Eq. 1); 1: psi = [gamma(x), phi(x)] (O8b) */
 } nifo_net_desc;
+
+/* features per endpoint */
+static int enc_per_endpoint(const nifo_net_desc* nd)
+{
+    if (nd->enc_mode == 1) return 3 + 6 * nd->pe_bands + nd->levels * nd->feat;
+    return (1 + 2 * nd->pe_bands) * nd->levels * nd->feat;
+}
 
 /* samples: S x 3 floats. p_0 = x_n; p_{1+2k} = (sin(2^k x_n)+1)/2; p_{2+2k} = (cos(2^k x_n)+1)/2 */
 void nifo_pe_samples(int bands, const float xn[3], float* samples)
@@ -575,7 +583,27 @@ static void encode_point(const nifo_net_desc* nd, const float* table, const floa
     int S = 1 + 2 * nd->pe_bands, L = nd->levels, F = nd->feat;
     size_t T = (size_t)1 << nd->log2_T;
     float samples[3 * 64];
-    nifo_pe_samples(nd->pe_bands, xn, samples);
+    if (nd->enc_mode == 1) {
+        /* O8b  Concatenation reading of the hybrid encoding (B:5 "positional frequency terms plus a
+           multiresolution hash grid"; R1 alternative): psi(x) = [ x, sin(2^0 x), cos(2^0 x), ...,
+           sin(2^(B-1) x), cos(2^(B-1) x), phi(x) ] -- gamma(x) of P:75 handed to the MLP as it is
+           (3 + 6B scalars, per band sin of the three axes then cos of the three axes, no pi: R4),
+           followed by the grid features of the point itself, out[3 + 6B + l*F + f]. */
+        for (int a = 0; a < 3; ++a) out[a] = (acc_t)xn[a];
+        for (int k = 0; k < nd->pe_bands; ++k) {
+            float f = ldexpf(1.0f, k);
+            for (int a = 0; a < 3; ++a) {
+                float arg = f * xn[a];
+                out[3 + 6 * k + a] = (acc_t)sinf(arg);
+                out[3 + 6 * k + 3 + a] = (acc_t)cosf(arg);
+            }
+        }
+        out += 3 + 6 * nd->pe_bands;
+        S = 1;
+        for (int a = 0; a < 3; ++a) samples[a] = xn[a];
+    } else {
+        nifo_pe_samples(nd->pe_bands, xn, samples);
+    }
     for (int s = 0; s < S; ++s)
         for (int l = 0; l < L; ++l) {
             uint32_t idx[8]; float w[8];
@@ -592,7 +620,7 @@ static void encode_point(const nifo_net_desc* nd, const float* table, const floa
 /* exposed for pins: features of n points (each an already normalised x_n), float output */
 void nifo_encode(const nifo_net_desc* nd, const float* table, int64_t n, const float* xn, float* out)
 {
-    int per = (1 + 2 * nd->pe_bands) * nd->levels * nd->feat;
+    int per = enc_per_endpoint(nd);
     acc_t* tmp = (acc_t*)malloc(sizeof(acc_t) * (size_t)per);
     for (int64_t i = 0; i < n; ++i) {
         encode_point(nd, table, xn + 3 * i, tmp);
@@ -692,8 +720,7 @@ static void nifo_eval_voxel(float theta_max, float bend_k, const nifo_net_desc* 
                             float* occlusion, float* distance, float* dist_total,
                             float* normal, float* albedo, float* material, float* raw_logits)
 {
-    int S = 1 + 2 * nd->pe_bands;
-    int per = S * nd->levels * nd->feat, d_in = 2 * per;
+    int per = enc_per_endpoint(nd), d_in = 2 * per;
     int n_out = (flags & NIFO_FLAG_OCCLUSION_ONLY) ? 1 : NIFO_N_OUT;
     acc_t* in = (acc_t*)malloc(sizeof(acc_t) * (size_t)d_in);
     acc_t* b0 = (acc_t*)malloc(sizeof(acc_t) * (size_t)nd->width);

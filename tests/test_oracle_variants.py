@@ -83,3 +83,43 @@ def test_rest_hit_position_fraction_special_cases(oracle):
     r2 = oracle.query(cfg.nv, occ, lat, bvh, pose, P, o, d, dist_log=True, hit_positions=True)
     np.testing.assert_allclose(r2["hit_position_rest"][hit], ends[hit, 0], atol=1e-7)
     np.testing.assert_allclose(r2["hit_position"][hit], o[hit], atol=0)       # D = 0: the ray origin
+
+
+def test_concatenation_encoding_layout_and_values(oracle):
+    """O8b: psi(x) = [x, sin/cos bands, phi(x)].  gamma against numpy in fp64; the grid part against
+    the composition encoding's sample-0 block (same phi, already pinned by test_oracle_encode.py)."""
+    from dataclasses import replace
+    cfg = I.get_config(0)
+    shape_c = replace(cfg.net, enc_mode="concat")
+    assert shape_c.d_in == 2 * (3 + 6 * cfg.net.pe_bands + cfg.net.levels * cfg.net.feat) == 70
+    P = I.net_params(cfg, "varpres")
+    Pc = I.net_params(replace(cfg, net=shape_c), "varpres")
+    assert np.array_equal(P.table, Pc.table) and Pc.weights[0].shape == (cfg.net.width, 70)
+    xn = np.random.default_rng(3).uniform(0, 1, (200, 3)).astype(np.float32)
+    comp = oracle.encode(P, xn)
+    cat = oracle.encode(Pc, xn)
+    B, LF = cfg.net.pe_bands, cfg.net.levels * cfg.net.feat
+    assert cat.shape == (200, 3 + 6 * B + LF)
+    assert np.array_equal(cat[:, :3], xn)
+    x64 = xn.astype(np.float64)
+    for k in range(B):
+        np.testing.assert_allclose(cat[:, 3 + 6 * k:6 + 6 * k], np.sin(2.0 ** k * x64), atol=2e-7)
+        np.testing.assert_allclose(cat[:, 6 + 6 * k:9 + 6 * k], np.cos(2.0 ** k * x64), atol=2e-7)
+    assert np.array_equal(cat[:, 3 + 6 * B:], comp[:, :LF])          # phi(x) = the s = 0 block of phi(gamma(x))
+
+
+def test_concatenation_query_equals_mlp_of_the_concatenated_endpoint_encodings(oracle):
+    from dataclasses import replace
+    cfg = I.get_config(0)
+    cfgc = replace(cfg, net=replace(cfg.net, enc_mode="concat"))
+    occ = I.occupancy(cfg); pose = I.poses(cfg)[0]
+    lat = oracle.deform_lattice(cfg.nv, *map(float, pose)); bvh = oracle.bvh_build(cfg.nv, occ, lat)
+    o, d = I.rays(cfg, 0, n=300)
+    Pc = I.net_params(cfgc, "varpres")
+    r = oracle.query(cfg.nv, occ, lat, bvh, pose, Pc, o, d)
+    hit = r["voxel_id"] >= 0
+    ends = oracle.rest_endpoints(float(pose[0]), float(pose[1]), o, d, r["voxel_id"], r["t_in"], r["t_out"])[hit]
+    xn = np.clip((ends + 1.0) * 0.5, 0.0, 1.0).astype(np.float32)
+    feats = np.concatenate([oracle.encode(Pc, xn[:, 0]), oracle.encode(Pc, xn[:, 1])], axis=1)   # entry then exit (R15)
+    z = oracle.mlp(Pc, feats)
+    np.testing.assert_allclose(r["raw_logits"][hit], z, atol=2e-6, rtol=1e-5)
