@@ -120,7 +120,7 @@ def physical_gpu_index(local_rank: int) -> int:
 # ------------------------------------------------------------------------------------------
 def algorithmic_work(cfg: I.Config) -> dict:
     n = cfg.net
-    gathers = 2 * n.samples * n.levels * 8
+    gathers = 2 * (1 if n.enc_mode == "concat" else n.samples) * n.levels * 8
     elem = 2 if n.dtype == "f16" else 4
     dims = n.layer_dims()
     if cfg.occlusion_only:
@@ -132,7 +132,16 @@ def algorithmic_work(cfg: I.Config) -> dict:
 
 
 def workload_name(cfg: I.Config) -> str:
-    return f"configs[{cfg.cfg_id}] {cfg.name}: {cfg.nv}^3 voxels, {cfg.n_poses} pose(s) x {cfg.rays_per_pose} rays"
+    enc = ", concatenation encoding" if cfg.net.enc_mode == "concat" else ""
+    return f"configs[{cfg.cfg_id}] {cfg.name}: {cfg.nv}^3 voxels, {cfg.n_poses} pose(s) x {cfg.rays_per_pose} rays{enc}"
+
+
+def configured(args) -> I.Config:
+    cfg = I.get_config(args.config)
+    if args.enc == "concat":                       # SURVEY 8(f) f3 variant, not the headline
+        from dataclasses import replace
+        cfg = replace(cfg, net=replace(cfg.net, enc_mode="concat"))
+    return cfg
 
 
 # ------------------------------------------------------------------------------------------
@@ -181,7 +190,7 @@ def run_reference(args) -> None:
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg = I.get_config(args.config)
+    cfg = configured(args)
     run = OracleRun(cfg, args.params)
     o, d, stride = run.sample(args.ref_sample)
     for _ in range(args.warmup):
@@ -221,7 +230,7 @@ def run_ours(args) -> None:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = torch.device("cuda", local_rank)
 
-    cfg = I.get_config(args.config)
+    cfg = configured(args)
     flags = nif.NIF_OCCLUSION_ONLY if cfg.occlusion_only else 0
     if args.engine == "ffma":
         flags |= nif.NIF_ENGINE_FFMA
@@ -446,6 +455,8 @@ def main() -> None:
     ap.add_argument("--ref-sample", type=int, default=32768, help="rays per step of --impl reference")
     ap.add_argument("--probe-table", action="store_true", help="run the gather probe over the real table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--enc", default="compose", choices=["compose", "concat"],
+                    help="hybrid-encoding reading: the paper's composition (default, headline) or concatenation")
     ap.add_argument("--walk", type=int, default=0, help="time nif_query_multi with this max_steps instead of nif_query "
                                                         "(SURVEY 8(f) f1; not the headline; use --params varpres)")
     args = ap.parse_args()

@@ -45,6 +45,16 @@ typedef enum {
 
 enum { NIF_F32 = 0, NIF_F16 = 1 };            /* nif_net_desc.dtype */
 
+/* nif_net_desc.enc_mode: how positional encoding gamma and hash grid phi are combined (R1).
+ *   NIF_ENC_COMPOSE  psi(x) = phi(gamma(x)), Eq. 1: every one of the S = 1 + 2B samples of
+ *                    gamma goes through the grid; D_in = 2 * S * L * F.  The paper's encoding; default.
+ *   NIF_ENC_CONCAT   psi(x) = [ x, sin(2^0 x), cos(2^0 x), ..., sin(2^(B-1) x), cos(2^(B-1) x), phi(x) ]
+ *                    (B:5 "positional frequency terms plus a multiresolution hash grid"): per band sin of
+ *                    the three axes then cos of the three axes, raw values, then the L*F grid features of
+ *                    the point; D_in = 2 * (3 + 6B + L * F), entry endpoint then exit endpoint.
+ *                    Not with feat = 3. */
+enum { NIF_ENC_COMPOSE = 0, NIF_ENC_CONCAT = 1 };
+
 /* nif_query flags */
 enum {
     NIF_OCCLUSION_ONLY = 1u,   /* decode only the occlusion head (B:10); other head outputs untouched */
@@ -88,7 +98,8 @@ typedef struct {
     float bend_k;
 } nif_deform_params;
 
-/* Encoding + MLP shape (B:7-11).  D_in = 2 * (1 + 2*pe_bands) * levels * feat. */
+/* Encoding + MLP shape (B:7-11).  D_in = 2 * (1 + 2*pe_bands) * levels * feat
+ * (NIF_ENC_COMPOSE). */
 typedef struct {
     int32_t pe_bands;             /* B: sinusoidal bands (the paper's "F"), 0..8          */
     int32_t levels;               /* L: hash-grid levels, 1..16                                 */
@@ -99,6 +110,7 @@ typedef struct {
     int32_t hidden_layers;        /* H: 1..8                                                    */
     int32_t width;                /* W: 16..128, multiple of 16                                 */
     int32_t dtype;                /* NIF_F32: table/weights float; NIF_F16: table/weights __half */
+    int32_t enc_mode;             /* NIF_ENC_COMPOSE (0) or NIF_ENC_CONCAT                      */
 } nif_net_desc;
 
 typedef struct {

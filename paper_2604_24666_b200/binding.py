@@ -16,6 +16,7 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libnif.so"
 
 NIF_F32, NIF_F16 = 0, 1
+NIF_ENC_COMPOSE, NIF_ENC_CONCAT = 0, 1
 NIF_OCCLUSION_ONLY, NIF_ENGINE_FFMA, NIF_TRAVERSE_ONLY = 1, 2, 4
 NIF_TRAVERSE_COHERENT, NIF_TRAVERSE_INCOHERENT, NIF_PROBE_SKIP_GATHER, NIF_DIST_LOG = 8, 16, 32, 64
 NIF_N_OUT = 12
@@ -39,7 +40,8 @@ class _DeformParams(C.Structure):
 class _NetDesc(C.Structure):
     _fields_ = [("pe_bands", C.c_int32), ("levels", C.c_int32), ("log2_T", C.c_int32),
                 ("feat", C.c_int32), ("level_res", C.POINTER(C.c_int32)),
-                ("hidden_layers", C.c_int32), ("width", C.c_int32), ("dtype", C.c_int32)]
+                ("hidden_layers", C.c_int32), ("width", C.c_int32), ("dtype", C.c_int32),
+                ("enc_mode", C.c_int32)]
 
 
 class _RayBatch(C.Structure):
@@ -213,7 +215,8 @@ def nif_net_create(shape, level_res, table: torch.Tensor, weights: list, stream=
     lr = np.ascontiguousarray(level_res, dtype=np.int32)
     d = _NetDesc(shape.pe_bands, shape.levels, shape.log2_T, shape.feat,
                  lr.ctypes.data_as(C.POINTER(C.c_int32)), shape.hidden_layers, shape.width,
-                 NIF_F16 if shape.dtype == "f16" else NIF_F32)
+                 NIF_F16 if shape.dtype == "f16" else NIF_F32,
+                 NIF_ENC_CONCAT if getattr(shape, "enc_mode", "compose") == "concat" else NIF_ENC_COMPOSE)
     wp = (C.c_void_p * len(weights))(*[w.data_ptr() for w in weights])
     h = C.c_void_p()
     _check(lib().nif_net_create(C.byref(d), table.data_ptr(), wp, _stream_ptr(stream), C.byref(h)),

@@ -66,6 +66,8 @@ static int validate_desc(const nif_net_desc* d)
     for (int l = 0; l < d->levels; ++l)
         if (d->level_res[l] < 1 || d->level_res[l] > (1 << 20)) return NIF_ERR_INVALID_ARG;
     if (d->feat < 1 || d->feat > 4) return NIF_ERR_UNSUPPORTED;
+    if (d->enc_mode != NIF_ENC_COMPOSE && d->enc_mode != NIF_ENC_CONCAT) return NIF_ERR_INVALID_ARG;
+    if (d->enc_mode == NIF_ENC_CONCAT && d->feat == 3) return NIF_ERR_UNSUPPORTED;
     if (d->width < 16 || d->width > 128 || (d->width % 16) != 0) return NIF_ERR_UNSUPPORTED;
     return NIF_OK;
 }
@@ -89,6 +91,7 @@ extern "C" int nif_net_create(const nif_net_desc* desc, const void* table, const
     net->enc.bands = desc->pe_bands; net->enc.levels = desc->levels;
     net->enc.log2_T = desc->log2_T; net->enc.feat = desc->feat;
     net->enc.dense_mask = 0;
+    net->enc.mode = desc->enc_mode;
     const unsigned long long T = 1ull << desc->log2_T;
     for (int l = 0; l < desc->levels; ++l) {
         net->enc.res[l] = desc->level_res[l];
@@ -99,7 +102,7 @@ extern "C" int nif_net_create(const nif_net_desc* desc, const void* table, const
     const int feat = pad3 ? 4 : desc->feat;
     net->desc.feat = feat; net->enc.feat = feat;
     const int groups = 2 * (1 + 2 * desc->pe_bands) * desc->levels;      // (endpoint, sample, level) triples
-    net->d_in = groups * feat;
+    net->d_in = desc->enc_mode == NIF_ENC_CONCAT ? 2 * (3 + 6 * desc->pe_bands + desc->levels * feat) : groups * feat;
     net->table = table;
     const size_t eb = elem_bytes(desc->dtype);
     if (pad3) {

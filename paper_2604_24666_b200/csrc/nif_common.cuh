@@ -50,6 +50,7 @@ struct NifEnc {
     int32_t bands, levels, log2_T, feat;
     int32_t res[NIF_MAX_LEVELS];
     uint32_t dense_mask;   // bit l set <=> level l is dense ((N+1)^3 <= T)
+    int32_t mode;          // NIF_ENC_COMPOSE | NIF_ENC_CONCAT
 };
 
 struct nif_net {

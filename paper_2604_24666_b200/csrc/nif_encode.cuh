@@ -39,6 +39,17 @@ __device__ __forceinline__ float nif_pe_sample(float xn, int s)
     return (v + 1.0f) * 0.5f;
 }
 
+// NIF_ENC_CONCAT: scalar j of gamma(x_n) handed to the MLP as it is: j < 3 -> x; then per band k:
+// sin(2^k x) of the three axes, cos(2^k x) of the three axes (raw values, no pi); 0 beyond 3 + 6B
+__device__ __forceinline__ float nif_pe_scalar(const float* __restrict__ xn, int j, int bands)
+{
+    if (j < 3) return xn[j];
+    const int jj = j - 3, k = jj / 6, r = jj - 6 * k;
+    if (k >= bands) return 0.0f;
+    const float arg = ldexpf(1.0f, k) * xn[r >= 3 ? r - 3 : r];
+    return r >= 3 ? cosf(arg) : sinf(arg);
+}
+
 template <typename T, int F> struct NifEntry;
 template <> struct NifEntry<float, 1> {
     static __device__ __forceinline__ void load(const float* t, uint32_t i, float* v) { v[0] = __ldg(t + i); }

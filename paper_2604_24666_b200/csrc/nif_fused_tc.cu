@@ -191,6 +191,7 @@ struct TcParams {
     nif_query_out out;
     const NifQueryScratch* scratch;
     unsigned int* tile_counter;   // dynamic tile scheduler (scratch header, zeroed per query)
+    int enc_mode;                 // NIF_ENC_COMPOSE | NIF_ENC_CONCAT
     const int32_t* hit_list;
     unsigned flags;
 };
@@ -339,7 +340,7 @@ __device__ __forceinline__ void issue_layer_chunk(uint32_t d_tmem, uint32_t act_
                  smem_desc_sw128(w_chunk + (uint32_t)k * 32u), idesc, (uint32_t)((kc | k) != 0));
 }
 
-template <int W, int F>
+template <int W, int F, bool CONCAT>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_fused_encode_mlp(const TcParams p)
 {
@@ -570,8 +571,24 @@ k_fused_encode_mlp(const TcParams p)
                     // diagnostic: synthetic features, no table access -- times the MLP pipeline alone
                     for (int u = 0; u < units_per_es; ++u)
                         st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), 0x2c002c00u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u);
+                } else if (CONCAT && es >= 2 && es < p.n_es) {
+                    // NIF_ENC_CONCAT: items 0, 1 are phi(entry), phi(exit); the rest carry the gamma scalars as
+                    // they are: L*F = 32 -> two 32-column items per endpoint, L*F = 64 -> one 64-column item
+                    const int pe_item = es - 2;
+                    const int e = (L * F == 32) ? pe_item >> 1 : pe_item;
+                    const int jbase = (L * F == 32) ? (pe_item & 1) * 32 : 0;
+                    const float* rb = ray_buf + ((size_t)b * TC_TILE + row) * 8 + 3 * e;
+                    const float xr[3] = {rb[0], rb[1], rb[2]};
+                    for (int u = 0; u < units_per_es; ++u) {
+                        float v[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) v[i] = nif_pe_scalar(xr, jbase + 8 * u + i, p.enc.bands);
+                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), pack_half2(v[0], v[1]), pack_half2(v[2], v[3]),
+                                     pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
+                    }
                 } else if (es < p.n_es) {
-                    const int e = es >= S ? 1 : 0, s = es - e * S;
+                    const int e = CONCAT ? es : (es >= S ? 1 : 0);
+                    const int s = CONCAT ? 0 : es - e * S;
                     const float* rb = ray_buf + ((size_t)b * TC_TILE + row) * 8 + 3 * e;
                     const float px = nif_pe_sample(rb[0], s), py = nif_pe_sample(rb[1], s), pz = nif_pe_sample(rb[2], s);
                     GatherBatch<F> ba, bb;                                     // two batches in flight
@@ -608,11 +625,18 @@ k_fused_encode_mlp(const TcParams p)
 // image of one layer = ceil(K/64) chunks of [n_rows x 128 B]; element (n, k) sits in chunk k/64 at
 // sw128_off(n, (k%64)/8) + (k%8)*2.  Rows/columns beyond the real matrix stay zero.
 __global__ void k_pack_weights(const __half* __restrict__ w, int fan_out, int fan_in, int n_rows,
-                               uint8_t* __restrict__ img)
+                               uint8_t* __restrict__ img, int concat_lf, int concat_npe)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= fan_out * fan_in) return;
-    const int n = i / fan_in, k = i - n * fan_in;
+    const int n = i / fan_in;
+    int k = i - n * fan_in;
+    if (concat_lf) {
+        // NIF_ENC_CONCAT, layer 1: user column e*per + j (per = npe + L*F, gamma scalars first) -> K index of
+        // the kernel's item layout: phi(e, j) at e*L*F + j, gamma(e, j) at 2*L*F + 64*e + j
+        const int per = concat_npe + concat_lf, e = k / per, j = k - e * per;
+        k = j < concat_npe ? 2 * concat_lf + 64 * e + j : e * concat_lf + (j - concat_npe);
+    }
     const uint32_t off = (uint32_t)(k / 64) * (uint32_t)(n_rows * 128) + sw128_off((uint32_t)n, (uint32_t)((k % 64) / 8)) +
                          (uint32_t)(k % 8) * 2u;
     *reinterpret_cast<__half*>(img + off) = w[i];
@@ -626,6 +650,7 @@ TcShape tc_shape(const nif_net_desc* d)
 {
     TcShape s{};
     s.S = 1 + 2 * d->pe_bands; s.n_es = 2 * s.S; s.lf = d->levels * d->feat;
+    if (d->enc_mode == NIF_ENC_CONCAT) s.n_es = 2 + 128 / (s.lf > 0 ? s.lf : 128);     // phi(entry), phi(exit) + gamma items of lf columns
     s.epc = s.lf > 0 && s.lf <= 64 ? 64 / s.lf : 0;
     s.n_chunks = s.epc ? (s.n_es + s.epc - 1) / s.epc : 0;
     s.KC = (d->width + 63) / 64;
@@ -649,11 +674,11 @@ int tc_pick_stages(int W)
     return 0;
 }
 
-template <int W, int F>
+template <int W, int F, bool CONCAT>
 int launch_tc(const TcParams& p, uint32_t smem, int blocks, cudaStream_t stream)
 {
-    NIF_CUDA_TRY(cudaFuncSetAttribute(k_fused_encode_mlp<W, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_fused_encode_mlp<W, F><<<blocks, TC_THREADS, smem, stream>>>(p);
+    NIF_CUDA_TRY(cudaFuncSetAttribute(k_fused_encode_mlp<W, F, CONCAT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_fused_encode_mlp<W, F, CONCAT><<<blocks, TC_THREADS, smem, stream>>>(p);
     nif_count_launch(1);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;
@@ -668,6 +693,7 @@ int nif_tc_supported(const nif_net_desc* d)
     if (d->width != 32 && d->width != 64 && d->width != 128) return 0;
     const int lf = d->levels * d->feat;
     if (lf != 8 && lf != 16 && lf != 32 && lf != 64) return 0;
+    if (d->enc_mode == NIF_ENC_CONCAT && ((lf != 32 && lf != 64) || 3 + 6 * d->pe_bands > 64)) return 0;
     if (d->hidden_layers < 1) return 0;
     const TcShape s = tc_shape(d);
     (void)s;
@@ -689,7 +715,9 @@ int nif_tc_pack_weights(nif_net* net, cudaStream_t stream)
         const int n_rows = i == d->hidden_layers ? TC_NOUT_PAD : d->width;
         net->w_tc_layer_off[i] = off;
         const int total = fan_out * fan_in;
-        k_pack_weights<<<(total + 255) / 256, 256, 0, stream>>>((const __half*)net->w_plain[i], fan_out, fan_in, n_rows, img + off);
+        const bool cat = i == 0 && d->enc_mode == NIF_ENC_CONCAT;
+        k_pack_weights<<<(total + 255) / 256, 256, 0, stream>>>((const __half*)net->w_plain[i], fan_out, fan_in, n_rows, img + off,
+                                                                cat ? s.lf : 0, cat ? 3 + 6 * d->pe_bands : 0);
         nif_count_launch(1);
         off += i == 0 ? s.w1_bytes : (size_t)s.KC * n_rows * 128;
     }
@@ -712,6 +740,7 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
     p.origin = rays->origin; p.dir = rays->dir;
     p.out = *out; p.scratch = scratch; p.tile_counter = &scratch->pad[4]; p.hit_list = hit_list; p.flags = flags;
+    p.enc_mode = d->enc_mode;
     p.stages = tc_pick_stages(d->width);
     const uint32_t smem = tc_smem_layout(p.stages, d->width).total;
     static int n_sm = 0;
@@ -722,7 +751,10 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     }
     const long long max_tiles = (rays->n + TC_TILE - 1) / TC_TILE;
     const int blocks = (int)(max_tiles < n_sm ? max_tiles : n_sm);
-#define NIF_TC_CASE(WW, FF) if (d->width == WW && d->feat == FF) return launch_tc<WW, FF>(p, smem, blocks, stream)
+    // the concatenation variant is its own instantiation so that the composition kernel's code is untouched
+#define NIF_TC_CASE(WW, FF) if (d->width == WW && d->feat == FF) \
+        return d->enc_mode == NIF_ENC_CONCAT ? launch_tc<WW, FF, true>(p, smem, blocks, stream) \
+                                             : launch_tc<WW, FF, false>(p, smem, blocks, stream)
     NIF_TC_CASE(32, 2); NIF_TC_CASE(64, 2); NIF_TC_CASE(128, 2);
     NIF_TC_CASE(32, 4); NIF_TC_CASE(64, 4); NIF_TC_CASE(128, 4);
 #undef NIF_TC_CASE

@@ -71,7 +71,9 @@ __global__ void __launch_bounds__(FF_THREADS)
 k_encode_mlp_ffma(const FfmaParams p)
 {
     extern __shared__ float smem[];
-    const int S = 1 + 2 * p.enc.bands, L = p.enc.levels;
+    const bool concat = p.enc.mode == NIF_ENC_CONCAT;
+    const int S = concat ? 1 : 1 + 2 * p.enc.bands, L = p.enc.levels;     // samples that go through the grid
+    const int n_pe = concat ? 3 + 6 * p.enc.bands : 0;                    // gamma scalars handed to the MLP directly
     const int d_in = p.d_in, W = p.width;
     float* act0 = smem;                                  // [FF_TILE][d_in]
     float* actA = act0 + FF_TILE * d_in;                 // [FF_TILE][W]
@@ -116,7 +118,12 @@ k_encode_mlp_ffma(const FfmaParams p)
             samp[i] = nif_pe_sample(xn[re * 3 + a], s);
         }
         __syncthreads();
-        // (a3) phi of every sample, flattened input[((e*S + s)*L + l)*F + f]
+        // NIF_ENC_CONCAT: input[e*per + j] = gamma scalar j, per = n_pe + L*F
+        for (int i = threadIdx.x; i < FF_TILE * 2 * n_pe; i += FF_THREADS) {
+            const int j = i % n_pe, re = i / n_pe;
+            act0[(re >> 1) * d_in + (re & 1) * (n_pe + L * F) + j] = nif_pe_scalar(xn + re * 3, j, p.enc.bands);
+        }
+        // (a3) phi of every sample, flattened input[((e*S + s)*L + l)*F + f]  (concat: after the gamma scalars)
         for (int i = threadIdx.x; i < FF_TILE * 2 * S * L; i += FF_THREADS) {
             const int l = i % L, s = (i / L) % S, re = i / (L * S);
             const int r = re >> 1, e = re & 1;
@@ -125,7 +132,7 @@ k_encode_mlp_ffma(const FfmaParams p)
             nif_level_features<T, F>(table + (size_t)l * level_stride, p.enc.res[l],
                                      (p.enc.dense_mask >> l) & 1u, t_mask, sp[0], sp[1], sp[2], feat);
 #pragma unroll
-            for (int f = 0; f < F; ++f) act0[r * d_in + ((e * S + s) * L + l) * F + f] = feat[f];
+            for (int f = 0; f < F; ++f) act0[r * d_in + n_pe * (e + 1) + ((e * S + s) * L + l) * F + f] = feat[f];
         }
         __syncthreads();
         // (a4) MLP

@@ -110,3 +110,32 @@ def test_query_host_carries_the_hit_positions(H, nif):
                        torch.from_numpy(case.direction).pin_memory(), out_h)
     for k in ("voxel_id", "dist_total", "hit_position", "hit_position_rest"):
         assert np.array_equal(out_h[k].numpy(), dev[k]), k
+
+
+@pytest.mark.parametrize("cfg_id,n_rays,tc", [(0, None, False), (1, 30_000, True), (4, 12_000, True)])
+def test_concatenation_encoding(oracle, H, P, nif, cfg_id, n_rays, tc):
+    """NIF_ENC_CONCAT (psi = [gamma(x), phi(x)], B:5 reading of the hybrid encoding; oracle O8b): config 0
+    on the fp32 engine, the shapes of config 1 (L*F = 32) and config 4 (L*F = 64) on the tcgen05 kernel
+    and on the FFMA cross-check."""
+    from dataclasses import replace
+    base = I.get_config(cfg_id)
+    cfg = replace(base, net=replace(base.net, enc_mode="concat"))
+    case = H.make_case(cfg_id, n_rays=n_rays, cfg=cfg)
+    assert case.params.weights[0].shape[1] == 2 * (3 + 6 * base.net.pe_bands + base.net.levels * base.net.feat)
+    assert nif.nif_net_uses_tensor_cores(case.net) == tc
+    fp16 = base.net.dtype == "f16"
+    side = H.OracleSide(oracle, case)
+    idx = None
+    if cfg_id == 4:
+        t = H.run_gpu(case, flags=nif.NIF_TRAVERSE_ONLY, raw_logits=False)
+        hit = np.nonzero(t["voxel_id"] >= 0)[0]
+        idx = np.unique(np.concatenate([hit[:: max(1, len(hit) // 1000)], np.arange(0, len(case.origin), 131)]))
+    ref = side.query(idx)
+    for fl in _engines(nif, case):
+        gpu = H.run_gpu(case, flags=fl)
+        if idx is not None:
+            gpu = H.subset(gpu, idx)
+        P.assert_traversal(P.compare_traversal(gpu, ref))
+        m = P.compare_network(gpu, ref, fp16=fp16)
+        P.assert_network(m, fp16=fp16)
+        assert m["n_hit"] > 500
