@@ -227,6 +227,37 @@ struct TcLevel {            // per-level constants, staged in shared memory (one
     uint32_t pad;
 };
 
+// L1 eviction priority of the table gathers.  Measured (cfg 1 / cfg 4 encode+MLP ms): plain __ldg 0.711 /
+// 10.69; evict_last on every level 0.708 / 10.47; evict_first or no_allocate on the fine (hashed) levels
+// 0.96 / 11.8 and 1.21 / 20.3 -- even the random fine-level gathers live on L1 reuse (the two x-corners of
+// a cell share a sector half of the time, entry and exit points share cells), so nothing is streamed past L1.
+#ifndef NIF_TC_FINE_FROM
+#define NIF_TC_FINE_FROM 0             // levels >= this use the hint below
+#endif
+#ifndef NIF_TC_FINE_HINT
+#define NIF_TC_FINE_HINT "L1::evict_last"
+#endif
+template <bool FINE> __device__ __forceinline__ uint32_t ldg_hint(const uint32_t* p)
+{
+    uint32_t v;
+    if constexpr (FINE) asm volatile("ld.global.nc." NIF_TC_FINE_HINT ".b32 %0, [%1];" : "=r"(v) : "l"(p));
+    else {
+#ifdef NIF_TC_COARSE_HINT
+        asm volatile("ld.global.nc." NIF_TC_COARSE_HINT ".b32 %0, [%1];" : "=r"(v) : "l"(p));
+#else
+        v = __ldg(p);
+#endif
+    }
+    return v;
+}
+template <bool FINE> __device__ __forceinline__ uint2 ldg_hint(const uint2* p)
+{
+    uint2 v;
+    if constexpr (FINE) asm volatile("ld.global.nc." NIF_TC_FINE_HINT ".v2.b32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    else v = __ldg(p);
+    return v;
+}
+
 template <int F>
 struct GatherBatch {
     static constexpr int NL = 4 / F;                          // levels per batch
@@ -236,6 +267,13 @@ struct GatherBatch {
 
     __device__ __forceinline__ void issue(const __half* __restrict__ table, const TcLevel* __restrict__ s_lvl,
                                           int log2_T, int l0, float px, float py, float pz)
+    {
+        if (l0 >= NIF_TC_FINE_FROM) issue_t<true>(table, s_lvl, log2_T, l0, px, py, pz);
+        else issue_t<false>(table, s_lvl, log2_T, l0, px, py, pz);
+    }
+    template <bool FINE>
+    __device__ __forceinline__ void issue_t(const __half* __restrict__ table, const TcLevel* __restrict__ s_lvl,
+                                            int log2_T, int l0, float px, float py, float pz)
     {
         const uint32_t t_mask = (1u << log2_T) - 1u;
 #pragma unroll
@@ -268,7 +306,7 @@ struct GatherBatch {
             }
             const char* lvl = reinterpret_cast<const char*>(table) + ((size_t)l << (log2_T + SH));
 #pragma unroll
-            for (int c = 0; c < 8; ++c) raw[li][c] = __ldg(reinterpret_cast<const raw_t*>(lvl + off[c]));
+            for (int c = 0; c < 8; ++c) raw[li][c] = ldg_hint<FINE>(reinterpret_cast<const raw_t*>(lvl + off[c]));
         }
     }
 
