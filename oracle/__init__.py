@@ -20,6 +20,7 @@ _CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared", 
 
 FLAG_OCCLUSION_ONLY = 1
 FLAG_DIST_LOG = 2
+FLAG_LATTICE_INVERSE = 4
 N_OUT = 12
 
 
@@ -88,8 +89,9 @@ class Oracle:
         L.nifo_walk_trace.restype = C.c_int
         L.nifo_walk_trace.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float,
                                       C.POINTER(_NetDesc), C.c_void_p, C.c_void_p, C.c_int64,
-                                      C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
-        L.nifo_hit_positions.argtypes = [C.c_float, C.c_float, C.c_int64] + [C.c_void_p] * 9
+                                      C.c_void_p, C.c_void_p, C.c_uint32, C.c_int, C.c_void_p, C.c_void_p]
+        L.nifo_hit_positions.argtypes = [C.c_void_p, C.c_int, C.c_uint32, C.c_float, C.c_float, C.c_int64] + [C.c_void_p] * 9
+        L.nifo_inverse_trilinear.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         self.acc_bytes = L.nifo_acc_bytes()
 
     # ---- deformation -----------------------------------------------------------------
@@ -102,6 +104,14 @@ class Oracle:
     def deform_lattice(self, nv, theta_max, k):
         out = np.empty(((nv + 1) ** 3, 3), dtype=np.float32)
         self.lib.nifo_deform_lattice(int(nv), float(theta_max), float(k), out.ctypes.data)
+        return out
+
+    def inverse_trilinear(self, lattice, nv, voxel_id, P):
+        """O7b: rest points of P[i], each taken to lie in deformed voxel voxel_id[i]."""
+        P = _f32(P).reshape(-1, 3)
+        vid = np.ascontiguousarray(voxel_id, dtype=np.int32)
+        out = np.empty_like(P)
+        self.lib.nifo_inverse_trilinear(lattice.ctypes.data, int(nv), len(P), vid.ctypes.data, P.ctypes.data, out.ctypes.data)
         return out
 
     def inverse_f32(self, theta_max, k, P):
@@ -195,7 +205,8 @@ class Oracle:
         return out
 
     def query(self, nv, occ, lattice, bvh, pose, params, origin, direction,
-              occlusion_only=False, traverse_only=False, dist_log=False, hit_positions=False):
+              occlusion_only=False, traverse_only=False, dist_log=False, hit_positions=False,
+              lattice_inverse=False):
         """Whole pipeline.  bvh=None -> brute-force definition."""
         origin = _f32(origin); direction = _f32(direction)
         n = len(origin)
@@ -216,22 +227,26 @@ class Oracle:
                                  bvh.handle if bvh is not None else None,
                                  float(pose[0]), float(pose[1]), C.byref(d), table.ctypes.data, arr,
                                  n, origin.ctypes.data, direction.ctypes.data,
-                                 (FLAG_OCCLUSION_ONLY if occlusion_only else 0) | (FLAG_DIST_LOG if dist_log else 0),
+                                 (FLAG_OCCLUSION_ONLY if occlusion_only else 0) | (FLAG_DIST_LOG if dist_log else 0) |
+                                 (FLAG_LATTICE_INVERSE if lattice_inverse else 0),
                                  g("voxel_id"), g("t_in"), g("t_out"), g("occlusion"), g("distance"),
                                  g("dist_total"), g("normal"), g("albedo"), g("material_logits"),
                                  g("raw_logits"))
         if rc != 0:
             raise RuntimeError(f"nifo_query failed: {rc}")
         if hit_positions and not traverse_only and not occlusion_only:
-            o["hit_position"], o["hit_position_rest"] = self.hit_positions(pose, origin, direction, o)
+            o["hit_position"], o["hit_position_rest"] = self.hit_positions(
+                pose, origin, direction, o, lattice=lattice if lattice_inverse else None, nv=nv)
         return o
 
-    def hit_positions(self, pose, origin, direction, res):
-        """O12: (deformed-space, rest-space) hit positions from a query's outputs."""
+    def hit_positions(self, pose, origin, direction, res, lattice=None, nv=0):
+        """O12: (deformed-space, rest-space) hit positions from a query's outputs (lattice given: O7b inverse)."""
         origin = _f32(origin); direction = _f32(direction)
         n = len(origin)
         hp = np.empty((n, 3), np.float32); hr = np.empty((n, 3), np.float32)
-        self.lib.nifo_hit_positions(float(pose[0]), float(pose[1]), n, origin.ctypes.data, direction.ctypes.data,
+        self.lib.nifo_hit_positions(lattice.ctypes.data if lattice is not None else None, int(nv),
+                                    FLAG_LATTICE_INVERSE if lattice is not None else 0,
+                                    float(pose[0]), float(pose[1]), n, origin.ctypes.data, direction.ctypes.data,
                                     res["voxel_id"].ctypes.data, res["t_in"].ctypes.data, res["t_out"].ctypes.data,
                                     res["distance"].ctypes.data, res["dist_total"].ctypes.data,
                                     hp.ctypes.data, hr.ctypes.data)
@@ -250,7 +265,7 @@ class Oracle:
         return vid, ti, to
 
     def query_multi(self, nv, occ, lattice, bvh, pose, params, origin, direction, max_steps,
-                    occlusion_only=False):
+                    occlusion_only=False, lattice_inverse=False):
         """O11: multi-voxel walk; returns the single-voxel outputs of the accepted (or last) voxel plus
         status / steps / dist_accum (the literal P:61 sum)."""
         origin = _f32(origin); direction = _f32(direction)
@@ -268,7 +283,8 @@ class Oracle:
                                        bvh.handle if bvh is not None else None,
                                        float(pose[0]), float(pose[1]), C.byref(d), table.ctypes.data, arr,
                                        n, origin.ctypes.data, direction.ctypes.data,
-                                       FLAG_OCCLUSION_ONLY if occlusion_only else 0, int(max_steps),
+                                       (FLAG_OCCLUSION_ONLY if occlusion_only else 0) |
+                                       (FLAG_LATTICE_INVERSE if lattice_inverse else 0), int(max_steps),
                                        *[o[k].ctypes.data for k in ("voxel_id", "t_in", "t_out", "occlusion",
                                                                     "distance", "dist_total", "normal", "albedo",
                                                                     "material_logits", "raw_logits", "status",
@@ -278,7 +294,7 @@ class Oracle:
         return o
 
 
-    def walk_trace(self, nv, occ, lattice, bvh, pose, params, origin, direction, max_steps):
+    def walk_trace(self, nv, occ, lattice, bvh, pose, params, origin, direction, max_steps, lattice_inverse=False):
         """O11 trace: (trace_id, trace_z0), each [n, max_steps]; id -1 past the end of a ray's voxel sequence."""
         origin = _f32(origin); direction = _f32(direction)
         n = len(origin)
@@ -289,7 +305,8 @@ class Oracle:
         rc = self.lib.nifo_walk_trace(nv, occ.ctypes.data, lattice.ctypes.data,
                                       bvh.handle if bvh is not None else None, float(pose[0]), float(pose[1]),
                                       C.byref(d), table.ctypes.data, arr, n, origin.ctypes.data,
-                                      direction.ctypes.data, int(max_steps), tid.ctypes.data, tz.ctypes.data)
+                                      direction.ctypes.data, FLAG_LATTICE_INVERSE if lattice_inverse else 0,
+                                      int(max_steps), tid.ctypes.data, tz.ctypes.data)
         if rc != 0:
             raise RuntimeError(f"nifo_walk_trace failed: {rc}")
         return tid, tz

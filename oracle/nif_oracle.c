@@ -48,6 +48,7 @@ typedef float acc_t;
 
 #define NIFO_N_OUT 12
 #define NIFO_FLAG_OCCLUSION_ONLY 1u
+#define NIFO_FLAG_LATTICE_INVERSE 4u /* O7b: voxel-local trilinear inverse from the lattice instead of the closed form */
 #define NIFO_FLAG_DIST_LOG 2u       /* O10b: ReLU + log-transformed distance head (R24) */
 
 int nifo_acc_bytes(void) { return (int)sizeof(acc_t); }
@@ -133,6 +134,66 @@ static void inverse_f32(float theta_max, float k, const float P[3], float out[3]
 void nifo_inverse_f32(float theta_max, float k, int64_t n, const float* P, float* out)
 {
     for (int64_t i = 0; i < n; ++i) inverse_f32(theta_max, k, P + 3 * i, out + 3 * i);
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* O7b  Voxel-local inverse for a deformation given only as a deformed corner lattice        */
+/* ("user-specified deformation"; "within each voxel the deformation field is      */
+/* approximately linear"; R27).  Inside voxel (ix,iy,iz) the deformation is taken to be the   */
+/* trilinear interpolant of its 8 deformed corners q_c, c = dx + 2 dy + 4 dz:                 */
+/*   T(u,v,w) = sum_c q_c * (dx?u:1-u)(dy?v:1-v)(dz?w:1-w),  (u,v,w) in [0,1]^3 the position  */
+/* inside the rest voxel.  T(u,v,w) = P is solved by Newton's method from the voxel centre,   */
+/* NIFO_NEWTON_ITERS iterations, 3x3 system by Cramer's rule, all in fp32 (a singular         */
+/* Jacobian stops the iteration).  Rest point: (2 (i + u) - Nv) / Nv per axis.  Points on the  */
+/* voxel's triangulated faces may land slightly outside [0,1]^3; no clamp here (the encoder    */
+/* clamps the normalised point, R3).                                                          */
+/* ------------------------------------------------------------------------------------ */
+#define NIFO_NEWTON_ITERS 5
+
+static void inverse_trilinear_f32(const float* lattice, int nv, int32_t id, const float P[3], float out[3])
+{
+    int ix = id % nv, iy = (id / nv) % nv, iz = id / (nv * nv);
+    int cell[3] = { ix, iy, iz };
+    size_t np1 = (size_t)nv + 1;
+    float q[8][3];
+    for (int c = 0; c < 8; ++c) {
+        const float* p = lattice + 3 * ((size_t)(ix + (c & 1)) + np1 * ((size_t)(iy + ((c >> 1) & 1)) + np1 * (size_t)(iz + (c >> 2))));
+        q[c][0] = p[0]; q[c][1] = p[1]; q[c][2] = p[2];
+    }
+    float u = 0.5f, v = 0.5f, w = 0.5f;
+    for (int it = 0; it < NIFO_NEWTON_ITERS; ++it) {
+        float T[3], Ju[3], Jv[3], Jw[3], r[3];
+        for (int a = 0; a < 3; ++a) {
+            float d00 = q[1][a] - q[0][a], d10 = q[3][a] - q[2][a], d01 = q[5][a] - q[4][a], d11 = q[7][a] - q[6][a];
+            float c00 = q[0][a] + u * d00, c10 = q[2][a] + u * d10, c01 = q[4][a] + u * d01, c11 = q[6][a] + u * d11;
+            float e0 = c10 - c00, e1 = c11 - c01;
+            float c0 = c00 + v * e0, c1 = c01 + v * e1;
+            T[a] = c0 + w * (c1 - c0);
+            Jw[a] = c1 - c0;
+            Jv[a] = e0 + w * (e1 - e0);
+            float f0 = d00 + v * (d10 - d00), f1 = d01 + v * (d11 - d01);
+            Ju[a] = f0 + w * (f1 - f0);
+            r[a] = P[a] - T[a];
+        }
+        /* Cramer: det[Ju Jv Jw], and the same determinant with one column replaced by r */
+        float cx = Jv[1] * Jw[2] - Jv[2] * Jw[1], cy = Jv[2] * Jw[0] - Jv[0] * Jw[2], cz = Jv[0] * Jw[1] - Jv[1] * Jw[0];
+        float det = Ju[0] * cx + Ju[1] * cy + Ju[2] * cz;
+        if (det == 0.0f) break;
+        float du = (r[0] * cx + r[1] * cy + r[2] * cz) / det;
+        float rx = r[1] * Jw[2] - r[2] * Jw[1], ry = r[2] * Jw[0] - r[0] * Jw[2], rz = r[0] * Jw[1] - r[1] * Jw[0];
+        float dv = (Ju[0] * rx + Ju[1] * ry + Ju[2] * rz) / det;
+        float sx = Jv[1] * r[2] - Jv[2] * r[1], sy = Jv[2] * r[0] - Jv[0] * r[2], sz = Jv[0] * r[1] - Jv[1] * r[0];
+        float dw = (Ju[0] * sx + Ju[1] * sy + Ju[2] * sz) / det;
+        u += du; v += dv; w += dw;
+    }
+    float uvw[3] = { u, v, w };
+    for (int a = 0; a < 3; ++a) out[a] = (2.0f * ((float)cell[a] + uvw[a]) - (float)nv) / (float)nv;
+}
+
+/* exposed for pins: rest point of P[i] taken to lie in voxel id[i] */
+void nifo_inverse_trilinear(const float* lattice, int nv, int64_t n, const int32_t* id, const float* P, float* out)
+{
+    for (int64_t i = 0; i < n; ++i) inverse_trilinear_f32(lattice, nv, id[i], P + 3 * i, out + 3 * i);
 }
 
 /* ------------------------------------------------------------------------------------ */
@@ -713,7 +774,7 @@ void nifo_decode(int64_t n, const float* logits, const float* t_in, const float*
 /* O7-O10 for ONE ray whose voxel (id, ti, to) is known: entry/exit points -> inverse deformation ->
    normalise -> psi(entry) ++ psi(exit) -> MLP -> heads, written to the pointers given (each
    pointing at this ray's slot; optional ones may be NULL). */
-static void nifo_eval_voxel(float theta_max, float bend_k, const nifo_net_desc* nd, const float* table,
+static void nifo_eval_voxel(const float* lattice, int nv, float theta_max, float bend_k, const nifo_net_desc* nd, const float* table,
                             const float* const* weights, const float* o, const float* d, uint32_t flags,
                             int32_t id, float ti, float to,
                             int32_t* vid, float* t_in, float* t_out,
@@ -731,7 +792,8 @@ static void nifo_eval_voxel(float theta_max, float bend_k, const nifo_net_desc* 
         float t = e ? to : ti;
         float P[3], pr[3], xn[3];
         for (int a = 0; a < 3; ++a) P[a] = fmaf(t, d[a], o[a]);
-        inverse_f32(theta_max, bend_k, P, pr);
+        if (flags & NIFO_FLAG_LATTICE_INVERSE) inverse_trilinear_f32(lattice, nv, id, P, pr);
+        else inverse_f32(theta_max, bend_k, P, pr);
         for (int a = 0; a < 3; ++a) {
             float v = (pr[a] + 1.0f) * 0.5f;
             xn[a] = v < 0.0f ? 0.0f : (v > 1.0f ? 1.0f : v);
@@ -797,7 +859,7 @@ int nifo_query(int nv, const uint8_t* occ, const float* lattice, const void* bvh
             if (raw_logits) for (int j = 0; j < NIFO_N_OUT; ++j) raw_logits[NIFO_N_OUT * r + j] = 0.0f;
             continue;
         }
-        nifo_eval_voxel(theta_max, bend_k, nd, table, weights, o, d, flags, vid[r], t_in[r], t_out[r],
+        nifo_eval_voxel(lattice, nv, theta_max, bend_k, nd, table, weights, o, d, flags, vid[r], t_in[r], t_out[r],
                         vid + r, t_in + r, t_out + r, occlusion + r, distance ? distance + r : 0,
                         dist_total ? dist_total + r : 0, normal ? normal + 3 * r : 0, albedo ? albedo + 3 * r : 0,
                         material ? material + 4 * r : 0, raw_logits ? raw_logits + NIFO_N_OUT * r : 0);
@@ -851,7 +913,7 @@ int nifo_query_multi(int nv, const uint8_t* occ, const float* lattice, const voi
             }
             /* evaluate the network on this voxel: reuse the single-voxel pipeline on a one-ray batch whose
                traversal result is forced to (id, ti, to) */
-            nifo_eval_voxel(theta_max, bend_k, nd, table, weights, o, d, flags, id, ti, to,
+            nifo_eval_voxel(lattice, nv, theta_max, bend_k, nd, table, weights, o, d, flags, id, ti, to,
                             vid + r, t_in + r, t_out + r, occlusion + r, distance ? distance + r : 0,
                             dist_total ? dist_total + r : 0, normal ? normal + 3 * r : 0, albedo ? albedo + 3 * r : 0,
                             material ? material + 4 * r : 0, raw_logits ? raw_logits + NIFO_N_OUT * r : 0);
@@ -881,7 +943,7 @@ int nifo_query_multi(int nv, const uint8_t* occ, const float* lattice, const voi
 int nifo_walk_trace(int nv, const uint8_t* occ, const float* lattice, const void* bvh,
                     float theta_max, float bend_k,
                     const nifo_net_desc* nd, const float* table, const float* const* weights,
-                    int64_t n, const float* origin, const float* dir, int max_steps,
+                    int64_t n, const float* origin, const float* dir, uint32_t flags, int max_steps,
                     int32_t* trace_id, float* trace_z0)
 {
     for (int64_t r = 0; r < n; ++r) {
@@ -894,7 +956,7 @@ int nifo_walk_trace(int nv, const uint8_t* occ, const float* lattice, const void
             else nifo_next_voxel_brute(nv, occ, lattice, 1, o, d, &after_t, &after_id, &id, &ti, &to);
             if (id < 0) break;
             int32_t v; float a, b, occl, raw[NIFO_N_OUT];
-            nifo_eval_voxel(theta_max, bend_k, nd, table, weights, o, d, NIFO_FLAG_OCCLUSION_ONLY, id, ti, to,
+            nifo_eval_voxel(lattice, nv, theta_max, bend_k, nd, table, weights, o, d, NIFO_FLAG_OCCLUSION_ONLY | (flags & NIFO_FLAG_LATTICE_INVERSE), id, ti, to,
                             &v, &a, &b, &occl, 0, 0, 0, 0, 0, raw);
             trace_id[r * max_steps + k] = id; trace_z0[r * max_steps + k] = raw[0];
             after_t = ti; after_id = id;
@@ -910,7 +972,8 @@ int nifo_walk_trace(int nv, const uint8_t* occ, const float* lattice, const void
    straight segment between the rest images of the voxel's entry and exit points (the local linear
    approximation of P:43) at the fraction u = clamp(distance / l, 0, 1) of the segment (u = 0 if l = 0).
    Miss: zeros (R18). */
-void nifo_hit_positions(float theta_max, float bend_k, int64_t n, const float* origin, const float* dir,
+void nifo_hit_positions(const float* lattice, int nv, uint32_t flags,
+                        float theta_max, float bend_k, int64_t n, const float* origin, const float* dir,
                         const int32_t* vid, const float* t_in, const float* t_out,
                         const float* distance, const float* dist_total, float* hit_pos, float* hit_rest)
 {
@@ -922,8 +985,13 @@ void nifo_hit_positions(float theta_max, float bend_k, int64_t n, const float* o
             hit_pos[3 * r + a] = fmaf(dist_total[r], d[a], o[a]);
             Pi[a] = fmaf(t_in[r], d[a], o[a]); Po[a] = fmaf(t_out[r], d[a], o[a]);
         }
-        inverse_f32(theta_max, bend_k, Pi, ri);
-        inverse_f32(theta_max, bend_k, Po, ro);
+        if (flags & NIFO_FLAG_LATTICE_INVERSE) {
+            inverse_trilinear_f32(lattice, nv, vid[r], Pi, ri);
+            inverse_trilinear_f32(lattice, nv, vid[r], Po, ro);
+        } else {
+            inverse_f32(theta_max, bend_k, Pi, ri);
+            inverse_f32(theta_max, bend_k, Po, ro);
+        }
         float ell = t_out[r] - t_in[r];
         float u = ell > 0.0f ? distance[r] / ell : 0.0f;
         u = u < 0.0f ? 0.0f : (u > 1.0f ? 1.0f : u);
