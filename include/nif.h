@@ -168,6 +168,17 @@ int nif_bvh_workspace_bytes(int32_t nv, int64_t max_occupied, size_t* bytes);
 int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_deform_params* pose,
                            void* workspace, size_t workspace_bytes, void* stream, nif_bvh** out);
 
+/* The same for a USER-SPECIFIED deformation given as the deformed corner lattice itself:
+ * `lattice_xyz`: DEVICE, (nv+1)^3 x 3 floats, lattice point (i,j,k) at index i + (nv+1)*(j + (nv+1)*k),
+ * copied into the workspace.  No closed-form inverse exists for such a pose, so nif_query maps entry and
+ * exit points back with the voxel-local inverse of the trilinear interpolant of the hit voxel's 8 deformed
+ * corners (R27: Newton, 5 iterations, fp32).  The lattice must not fold over (positive Jacobian);
+ * this is not checked.  nif_bvh_refit_lattice replaces the lattice of an existing BVH (any BVH: a
+ * closed-form one becomes a lattice one).  Both SYNCHRONISE. */
+int nif_build_bvh_from_lattice(const nif_voxel_set* voxels, const float* lattice_xyz,
+                               void* workspace, size_t workspace_bytes, void* stream, nif_bvh** out);
+int nif_bvh_refit_lattice(nif_bvh* bvh, const float* lattice_xyz, void* stream);
+
 /* New pose for the same voxel set: recomputes the deformed corner lattice and every box of the
  * hierarchy in place; the topology (which is the sparse octree of the REST lattice) is reused, so no
  * occupancy pass, scan or allocation happens.  The result is bit-identical to a fresh

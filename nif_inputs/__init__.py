@@ -308,3 +308,22 @@ def shard_range(n: int, rank: int, world: int):
     base, rem = divmod(n, world)
     begin = rank * base + min(rank, rem)
     return begin, begin + base + (1 if rank < rem else 0)
+
+
+def wavy_lattice(nv: int, seed: int, amplitude_voxels: float = 0.35) -> np.ndarray:
+    """A "user-specified deformation" that has no closed-form inverse: the rest corner
+    lattice [(nv+1)^3, 3] (point (i,j,k) at index i + (nv+1)(j + (nv+1)k), coordinates (2i - nv)/nv)
+    displaced by a seeded sum of three smooth sine waves per axis, amplitude `amplitude_voxels` voxel
+    sizes in total (small enough that no voxel folds over).  float32."""
+    rng = np.random.default_rng(seed)
+    g = (2.0 * np.arange(nv + 1, dtype=np.float64) - nv) / nv
+    z, y, x = np.meshgrid(g, g, g, indexing="ij")
+    p = np.stack([x.ravel(), y.ravel(), z.ravel()], axis=1)
+    h = 2.0 / nv
+    disp = np.zeros_like(p)
+    for _ in range(3):
+        k = rng.uniform(1.0, 3.0, size=(3, 3))            # wave vectors (rad per unit length), one per displaced axis
+        ph = rng.uniform(0.0, 2.0 * math.pi, size=3)
+        amp = rng.uniform(0.5, 1.0, size=3) * amplitude_voxels * h / 3.0
+        disp += amp * np.sin(p @ k.T + ph)
+    return np.ascontiguousarray((p + disp).astype(np.float32))

@@ -83,6 +83,9 @@ def lib() -> C.CDLL:
         L.nif_bvh_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_build_deformed_bvh.argtypes = [C.POINTER(_VoxelSet), C.POINTER(_DeformParams), C.c_void_p,
                                              C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
+        L.nif_build_bvh_from_lattice.argtypes = [C.POINTER(_VoxelSet), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p,
+                                                 C.POINTER(C.c_void_p)]
+        L.nif_bvh_refit_lattice.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.nif_bvh_refit.argtypes = [C.c_void_p, C.POINTER(_DeformParams), C.c_void_p]
         L.nif_bvh_get_info.argtypes = [C.c_void_p, C.POINTER(_BvhInfo)]
         L.nif_bvh_get_lattice.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
@@ -157,6 +160,11 @@ class Bvh:
         dp = _DeformParams(float(theta_max), float(bend_k))
         _check(lib().nif_bvh_refit(self.handle, C.byref(dp), _stream_ptr(stream)), "nif_bvh_refit")
 
+    def refit_lattice(self, lattice_xyz: torch.Tensor, stream=None):
+        """nif_bvh_refit_lattice: new user-specified deformed lattice [(nv+1)^3, 3] float32 CUDA (synchronises)."""
+        assert lattice_xyz.is_cuda and lattice_xyz.dtype == torch.float32 and lattice_xyz.is_contiguous()
+        _check(lib().nif_bvh_refit_lattice(self.handle, lattice_xyz.data_ptr(), _stream_ptr(stream)), "nif_bvh_refit_lattice")
+
     def lattice(self) -> torch.Tensor:
         """Copy of the deformed corner lattice, [(nv+1)^3, 3] float32 (for parity tests)."""
         p = C.c_void_p()
@@ -189,6 +197,21 @@ def nif_build_deformed_bvh(nv: int, occupancy: torch.Tensor, theta_max: float, b
     h = C.c_void_p()
     _check(lib().nif_build_deformed_bvh(C.byref(vs), C.byref(dp), ws.data_ptr(), nbytes,
                                         _stream_ptr(stream), C.byref(h)), "nif_build_deformed_bvh")
+    return Bvh(h, ws, occupancy)
+
+
+def nif_build_bvh_from_lattice(nv: int, occupancy: torch.Tensor, lattice_xyz: torch.Tensor,
+                               max_occupied: int | None = None, stream=None) -> Bvh:
+    """User-specified deformation given as the deformed corner lattice [(nv+1)^3, 3] float32 CUDA."""
+    assert occupancy.is_cuda and occupancy.dtype == torch.uint8 and occupancy.is_contiguous()
+    assert lattice_xyz.is_cuda and lattice_xyz.dtype == torch.float32 and lattice_xyz.is_contiguous()
+    assert occupancy.numel() == nv ** 3 and lattice_xyz.numel() == 3 * (nv + 1) ** 3
+    nbytes = nif_bvh_workspace_bytes(nv, nv ** 3 if max_occupied is None else max_occupied)
+    ws = _ws(nbytes)
+    vs = _VoxelSet(nv, occupancy.data_ptr())
+    h = C.c_void_p()
+    _check(lib().nif_build_bvh_from_lattice(C.byref(vs), lattice_xyz.data_ptr(), ws.data_ptr(), nbytes,
+                                            _stream_ptr(stream), C.byref(h)), "nif_build_bvh_from_lattice")
     return Bvh(h, ws, occupancy)
 
 

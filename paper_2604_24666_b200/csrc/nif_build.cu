@@ -64,6 +64,13 @@ __global__ void k_deform_lattice(int nv, double theta_max, double k, float4* __r
     }
 }
 
+// user-supplied deformed lattice ("user-specified deformation"): xyz floats -> the float4 lattice
+__global__ void k_import_lattice(size_t total, const float* __restrict__ xyz, float4* __restrict__ lat)
+{
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x)
+        lat[idx] = make_float4(xyz[3 * idx], xyz[3 * idx + 1], xyz[3 * idx + 2], 0.0f);
+}
+
 // ---- occupancy masks ------------------------------------------------------------------------
 // level 1: one Morton-indexed brick of 2x2x2 voxels; bit c = octant (c&1, (c>>1)&1, c>>2).
 // counters[0] += occupied voxels; counters[1] = max (iy+1) over occupied voxels.
@@ -332,12 +339,14 @@ bool pose_folds_over(const nif_deform_params* pose, int nv, uint32_t top_iy)
     return worst >= 1.0 - 1e-3;
 }
 
-void launch_deform(int nv, const nif_deform_params* pose, float4* lattice, cudaStream_t stream)
+// pose != NULL: closed-form deformation; else copy the user's deformed lattice
+void launch_deform(int nv, const nif_deform_params* pose, const float* user_lattice, float4* lattice, cudaStream_t stream)
 {
     const size_t np1 = (size_t)nv + 1, total = np1 * np1 * np1;
     int blocks = (int)((total + 255) / 256);
     if (blocks > 148 * 32) blocks = 148 * 32;
-    k_deform_lattice<<<blocks, 256, 0, stream>>>(nv, (double)pose->twist_theta_max, (double)pose->bend_k, lattice);
+    if (pose) k_deform_lattice<<<blocks, 256, 0, stream>>>(nv, (double)pose->twist_theta_max, (double)pose->bend_k, lattice);
+    else k_import_lattice<<<blocks, 256, 0, stream>>>(total, user_lattice, lattice);
     nif_count_launch(1);
 }
 
@@ -386,14 +395,13 @@ extern "C" int nif_bvh_workspace_bytes(int32_t nv, int64_t max_occupied, size_t*
     return NIF_OK;
 }
 
-extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_deform_params* pose,
-                                      void* workspace, size_t workspace_bytes, void* stream_,
-                                      nif_bvh** out)
+static int build_common(const nif_voxel_set* voxels, const nif_deform_params* pose, const float* user_lattice,
+                        void* workspace, size_t workspace_bytes, void* stream_, nif_bvh** out)
 {
-    if (!voxels || !pose || !workspace || !out || !voxels->occupancy) return NIF_ERR_INVALID_ARG;
+    if (!voxels || (!pose && !user_lattice) || !workspace || !out || !voxels->occupancy) return NIF_ERR_INVALID_ARG;
     const int nv = voxels->nv;
     if (nv < 2 || nv > 512) return NIF_ERR_INVALID_ARG;
-    if (!isfinite(pose->twist_theta_max) || !isfinite(pose->bend_k)) return NIF_ERR_INVALID_ARG;
+    if (pose && (!isfinite(pose->twist_theta_max) || !isfinite(pose->bend_k))) return NIF_ERR_INVALID_ARG;
     if (((uintptr_t)workspace & 255u) != 0) return NIF_ERR_WORKSPACE;
     if (!device_is_sm100()) return NIF_ERR_UNSUPPORTED;
     cudaStream_t stream = (cudaStream_t)stream_;
@@ -406,7 +414,7 @@ extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_def
     const size_t node_capacity = (workspace_bytes - L.off_nodes) / NODE_BYTES;
 
     NIF_CUDA_TRY(cudaMemsetAsync(counters, 0, 64 * sizeof(uint32_t), stream));
-    launch_deform(nv, pose, lattice, stream);
+    launch_deform(nv, pose, user_lattice, lattice, stream);
     for (int l = 1; l <= L.levels; ++l) {
         const uint32_t c = (uint32_t)L.cells[l];
         uint8_t* mask = (uint8_t*)(ws + L.off_mask[l]);
@@ -427,7 +435,7 @@ extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_def
     NIF_CUDA_TRY(cudaGetLastError());
 
     const uint32_t n_occ = h_counters[0];
-    if (n_occ && pose_folds_over(pose, nv, h_counters[1])) return NIF_ERR_DEFORM_SINGULAR;
+    if (n_occ && pose && pose_folds_over(pose, nv, h_counters[1])) return NIF_ERR_DEFORM_SINGULAR;
     uint32_t base[12] = {0};
     size_t n_nodes = 0;
     for (int l = 1; l <= L.levels; ++l) { base[l] = (uint32_t)n_nodes; n_nodes += h_counters[2 + l]; }
@@ -441,7 +449,8 @@ extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_def
     if (!b) return NIF_ERR_CUDA;
     b->nv = nv; b->n_occupied = (int32_t)n_occ; b->n_nodes = (int32_t)n_nodes; b->depth = L.levels;
     b->root = -1;
-    b->theta_max = pose->twist_theta_max; b->bend_k = pose->bend_k;
+    b->theta_max = pose ? pose->twist_theta_max : 0.0f; b->bend_k = pose ? pose->bend_k : 0.0f;
+    b->local_inverse = pose ? 0 : 1;
     b->lattice = lattice; b->nodes = nodes;
     for (int a = 0; a < 3; ++a) { b->lo[a] = 0.f; b->hi[a] = 0.f; }
     b->ws = ws; b->node_capacity = node_capacity; b->top_iy = h_counters[1];
@@ -454,6 +463,20 @@ extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_def
     return NIF_OK;
 }
 
+extern "C" int nif_build_deformed_bvh(const nif_voxel_set* voxels, const nif_deform_params* pose,
+                                      void* workspace, size_t workspace_bytes, void* stream, nif_bvh** out)
+{
+    if (!pose) return NIF_ERR_INVALID_ARG;
+    return build_common(voxels, pose, nullptr, workspace, workspace_bytes, stream, out);
+}
+
+extern "C" int nif_build_bvh_from_lattice(const nif_voxel_set* voxels, const float* lattice_xyz,
+                                          void* workspace, size_t workspace_bytes, void* stream, nif_bvh** out)
+{
+    if (!lattice_xyz) return NIF_ERR_INVALID_ARG;
+    return build_common(voxels, nullptr, lattice_xyz, workspace, workspace_bytes, stream, out);
+}
+
 // Same voxel set, new pose: the hierarchy's topology is the rest lattice's octree (pose-independent),
 // so only the corner lattice and the boxes are recomputed.
 extern "C" int nif_bvh_refit(nif_bvh* b, const nif_deform_params* pose, void* stream_)
@@ -464,8 +487,21 @@ extern "C" int nif_bvh_refit(nif_bvh* b, const nif_deform_params* pose, void* st
     if (b->n_occupied && pose_folds_over(pose, b->nv, b->top_iy)) return NIF_ERR_DEFORM_SINGULAR;
     cudaStream_t stream = (cudaStream_t)stream_;
     const BuildLayout L = make_layout(b->nv);
-    launch_deform(b->nv, pose, (float4*)(b->ws + L.off_lattice), stream);
-    b->theta_max = pose->twist_theta_max; b->bend_k = pose->bend_k;
+    launch_deform(b->nv, pose, nullptr, (float4*)(b->ws + L.off_lattice), stream);
+    b->theta_max = pose->twist_theta_max; b->bend_k = pose->bend_k; b->local_inverse = 0;
+    if (b->n_occupied) return write_levels(b, L, stream);
+    NIF_CUDA_TRY(cudaStreamSynchronize(stream));
+    return NIF_OK;
+}
+
+extern "C" int nif_bvh_refit_lattice(nif_bvh* b, const float* lattice_xyz, void* stream_)
+{
+    if (!b || !lattice_xyz) return NIF_ERR_INVALID_ARG;
+    if (!device_is_sm100()) return NIF_ERR_UNSUPPORTED;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const BuildLayout L = make_layout(b->nv);
+    launch_deform(b->nv, nullptr, lattice_xyz, (float4*)(b->ws + L.off_lattice), stream);
+    b->theta_max = 0.0f; b->bend_k = 0.0f; b->local_inverse = 1;
     if (b->n_occupied) return write_levels(b, L, stream);
     NIF_CUDA_TRY(cudaStreamSynchronize(stream));
     return NIF_OK;

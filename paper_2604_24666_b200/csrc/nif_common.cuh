@@ -36,6 +36,7 @@ struct nif_bvh {
     int32_t root;          // node index, -1 if the grid is empty
     float lo[3], hi[3];
     float theta_max, bend_k;
+    int32_t local_inverse; // built from a user lattice: map back with the voxel-local inverse (R27)
     const float4* lattice; // device, (nv+1)^3
     const NifNode* nodes;  // device
     // kept for nif_bvh_refit: the topology (masks, offsets, node ranges) is pose-independent

@@ -25,6 +25,85 @@ __device__ __forceinline__ void nif_inverse_deform(float theta_max, float k, flo
     z = -bx * sa + bz * ca;
 }
 
+// (a2) for a deformation given as a corner lattice (R27): voxel-local inverse of the trilinear
+// interpolant of the voxel's 8 deformed corners, Newton from the voxel centre, NIF_NEWTON_ITERS iterations,
+// Cramer's rule, fp32.  `q` = the 8 corners (c = dx + 2 dy + 4 dz).
+#define NIF_NEWTON_ITERS 5
+__device__ __forceinline__ void nif_load_voxel_corners(const float4* __restrict__ lat, int nv, int32_t id, float (&q)[8][3],
+                                                       int (&cell)[3])
+{
+    const uint32_t unv = (uint32_t)nv, uid = (uint32_t)id;
+    const uint32_t ix = uid % unv, iy = (uid / unv) % unv, iz = uid / (unv * unv);
+    cell[0] = (int)ix; cell[1] = (int)iy; cell[2] = (int)iz;
+    const size_t np1 = (size_t)nv + 1;
+    const float4* base = lat + (size_t)ix + np1 * ((size_t)iy + np1 * (size_t)iz);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const float4 v = __ldg(base + (c & 1) + np1 * (size_t)((c >> 1) & 1) + np1 * np1 * (size_t)(c >> 2));
+        q[c][0] = v.x; q[c][1] = v.y; q[c][2] = v.z;
+    }
+}
+__device__ __forceinline__ void nif_inverse_trilinear(const float (&q)[8][3], const int (&cell)[3], int nv,
+                                                      float X, float Y, float Z, float& x, float& y, float& z)
+{
+    const float P[3] = {X, Y, Z};
+    float u = 0.5f, v = 0.5f, w = 0.5f;
+    for (int it = 0; it < NIF_NEWTON_ITERS; ++it) {
+        float Ju[3], Jv[3], Jw[3], r[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const float d00 = q[1][a] - q[0][a], d10 = q[3][a] - q[2][a], d01 = q[5][a] - q[4][a], d11 = q[7][a] - q[6][a];
+            const float c00 = q[0][a] + u * d00, c10 = q[2][a] + u * d10, c01 = q[4][a] + u * d01, c11 = q[6][a] + u * d11;
+            const float e0 = c10 - c00, e1 = c11 - c01;
+            const float c0 = c00 + v * e0, c1 = c01 + v * e1;
+            Jw[a] = c1 - c0;
+            Jv[a] = e0 + w * (e1 - e0);
+            const float f0 = d00 + v * (d10 - d00), f1 = d01 + v * (d11 - d01);
+            Ju[a] = f0 + w * (f1 - f0);
+            r[a] = P[a] - (c0 + w * (c1 - c0));
+        }
+        const float cx = Jv[1] * Jw[2] - Jv[2] * Jw[1], cy = Jv[2] * Jw[0] - Jv[0] * Jw[2], cz = Jv[0] * Jw[1] - Jv[1] * Jw[0];
+        const float det = Ju[0] * cx + Ju[1] * cy + Ju[2] * cz;
+        if (det == 0.0f) break;
+        const float du = (r[0] * cx + r[1] * cy + r[2] * cz) / det;
+        const float rx = r[1] * Jw[2] - r[2] * Jw[1], ry = r[2] * Jw[0] - r[0] * Jw[2], rz = r[0] * Jw[1] - r[1] * Jw[0];
+        const float dv = (Ju[0] * rx + Ju[1] * ry + Ju[2] * rz) / det;
+        const float sx = Jv[1] * r[2] - Jv[2] * r[1], sy = Jv[2] * r[0] - Jv[0] * r[2], sz = Jv[0] * r[1] - Jv[1] * r[0];
+        const float dw = (Ju[0] * sx + Ju[1] * sy + Ju[2] * sz) / det;
+        u += du; v += dv; w += dw;
+    }
+    const float fnv = (float)nv;
+    x = (2.0f * ((float)cell[0] + u) - fnv) / fnv;
+    y = (2.0f * ((float)cell[1] + v) - fnv) / fnv;
+    z = (2.0f * ((float)cell[2] + w) - fnv) / fnv;
+}
+
+// what step (a2) needs: the closed-form pose, or the lattice for the voxel-local inverse
+struct NifMapCtx {
+    float theta_max, bend_k;
+    const float4* lat;        // deformed corner lattice
+    int nv;
+    int local;                // 1: the BVH was built from a user lattice -> voxel-local inverse (R27)
+};
+
+// rest images of a ray's entry and exit points (both lie in voxel `vid`)
+template <bool LOCAL>
+__device__ __forceinline__ void nif_map_back_pair(const NifMapCtx& m, int32_t vid, const float* __restrict__ o,
+                                                  const float* __restrict__ d, float t_in, float t_out, float (&ri)[3], float (&ro)[3])
+{
+    const float Xi = fmaf(t_in, d[0], o[0]), Yi = fmaf(t_in, d[1], o[1]), Zi = fmaf(t_in, d[2], o[2]);
+    const float Xo = fmaf(t_out, d[0], o[0]), Yo = fmaf(t_out, d[1], o[1]), Zo = fmaf(t_out, d[2], o[2]);
+    if constexpr (LOCAL) {
+        float q[8][3]; int cell[3];
+        nif_load_voxel_corners(m.lat, m.nv, vid, q, cell);
+        nif_inverse_trilinear(q, cell, m.nv, Xi, Yi, Zi, ri[0], ri[1], ri[2]);
+        nif_inverse_trilinear(q, cell, m.nv, Xo, Yo, Zo, ro[0], ro[1], ro[2]);
+    } else {
+        nif_inverse_deform(m.theta_max, m.bend_k, Xi, Yi, Zi, ri[0], ri[1], ri[2]);
+        nif_inverse_deform(m.theta_max, m.bend_k, Xo, Yo, Zo, ro[0], ro[1], ro[2]);
+    }
+}
+
 // rest-space point -> normalised grid coordinate in [0,1] ("normalized query point")
 __device__ __forceinline__ float nif_normalise(float p) { return __saturatef((p + 1.0f) * 0.5f); }
 
@@ -130,9 +209,10 @@ __device__ __forceinline__ float nif_sigmoid(float z) { return 1.0f / (1.0f + ex
 struct NifDecodeCtx {
     const float* origin;
     const float* dir;
-    float theta_max, bend_k;
+    NifMapCtx map;
 };
 
+template <bool LOCAL>
 __device__ __forceinline__ void nif_decode_store(const float* __restrict__ z, float t_in, float t_out,
                                                  long long ray, const nif_query_out& out, unsigned flags,
                                                  const NifDecodeCtx& ctx)
@@ -179,13 +259,13 @@ __device__ __forceinline__ void nif_decode_store(const float* __restrict__ z, fl
             out.hit_position[3 * ray + 2] = fmaf(D, dz, oz);
         }
         if (out.hit_position_rest) {
-            float ix, iy, iz, ex, ey, ez;
-            nif_inverse_deform(ctx.theta_max, ctx.bend_k, fmaf(t_in, dx, ox), fmaf(t_in, dy, oy), fmaf(t_in, dz, oz), ix, iy, iz);
-            nif_inverse_deform(ctx.theta_max, ctx.bend_k, fmaf(t_out, dx, ox), fmaf(t_out, dy, oy), fmaf(t_out, dz, oz), ex, ey, ez);
+            const float oo[3] = {ox, oy, oz}, dd[3] = {dx, dy, dz};
+            float ri[3], ro[3];
+            nif_map_back_pair<LOCAL>(ctx.map, LOCAL ? out.voxel_id[ray] : 0, oo, dd, t_in, t_out, ri, ro);
             const float u = ell > 0.0f ? __saturatef(d / ell) : 0.0f;
-            out.hit_position_rest[3 * ray] = fmaf(u, ex - ix, ix);
-            out.hit_position_rest[3 * ray + 1] = fmaf(u, ey - iy, iy);
-            out.hit_position_rest[3 * ray + 2] = fmaf(u, ez - iz, iz);
+            out.hit_position_rest[3 * ray] = fmaf(u, ro[0] - ri[0], ri[0]);
+            out.hit_position_rest[3 * ray + 1] = fmaf(u, ro[1] - ri[1], ri[1]);
+            out.hit_position_rest[3 * ray + 2] = fmaf(u, ro[2] - ri[2], ri[2]);
         }
     }
 }

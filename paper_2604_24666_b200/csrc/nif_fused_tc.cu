@@ -192,6 +192,7 @@ struct TcParams {
     const NifQueryScratch* scratch;
     unsigned int* tile_counter;   // dynamic tile scheduler (scratch header, zeroed per query)
     int enc_mode;                 // NIF_ENC_COMPOSE | NIF_ENC_CONCAT
+    NifMapCtx map;                // (a2): pose, or the lattice for the voxel-local inverse
     const int32_t* hit_list;
     unsigned flags;
 };
@@ -378,7 +379,7 @@ __device__ __forceinline__ void issue_layer_chunk(uint32_t d_tmem, uint32_t act_
                  smem_desc_sw128(w_chunk + (uint32_t)k * 32u), idesc, (uint32_t)((kc | k) != 0));
 }
 
-template <int W, int F, bool CONCAT>
+template <int W, int F, bool CONCAT, bool LOCAL>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_fused_encode_mlp(const TcParams p)
 {
@@ -469,8 +470,15 @@ k_fused_encode_mlp(const TcParams p)
                 nxt_ti = p.out.t_in[nxt_ray]; nxt_to = p.out.t_out[nxt_ray];
                 const float ox = p.origin[3 * nxt_ray], oy = p.origin[3 * nxt_ray + 1], oz = p.origin[3 * nxt_ray + 2];
                 const float dx = p.dir[3 * nxt_ray], dy = p.dir[3 * nxt_ray + 1], dz = p.dir[3 * nxt_ray + 2];
+                if constexpr (LOCAL) {           // deformation given as a lattice: voxel-local inverse (R27)
+                    const float oo[3] = {ox, oy, oz}, dd[3] = {dx, dy, dz};
+                    float ri[3], ro[3];
+                    nif_map_back_pair<true>(p.map, p.out.voxel_id[nxt_ray], oo, dd, nxt_ti, nxt_to, ri, ro);
+                    xi = ri[0]; yi = ri[1]; zi = ri[2]; xo = ro[0]; yo = ro[1]; zo = ro[2];
+                } else {
                 nif_inverse_deform(p.theta_max, p.bend_k, fmaf(nxt_ti, dx, ox), fmaf(nxt_ti, dy, oy), fmaf(nxt_ti, dz, oz), xi, yi, zi);
                 nif_inverse_deform(p.theta_max, p.bend_k, fmaf(nxt_to, dx, ox), fmaf(nxt_to, dy, oy), fmaf(nxt_to, dz, oz), xo, yo, zo);
+                }
             }
             float* rb = ray_buf + ((size_t)b * TC_TILE + r) * 8;
             rb[0] = nif_normalise(xi); rb[1] = nif_normalise(yi); rb[2] = nif_normalise(zi);
@@ -515,7 +523,7 @@ k_fused_encode_mlp(const TcParams p)
                 float z[NIF_N_OUT];
 #pragma unroll
                 for (int a = 0; a < NIF_N_OUT; ++a) z[a] = __uint_as_float(zr[a]);
-                nif_decode_store(z, cur_ti, cur_to, cur_ray, p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.theta_max, p.bend_k});
+                nif_decode_store<LOCAL>(z, cur_ti, cur_to, cur_ray, p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map});
             }
         }
     } else if (warp == TC_MMA_WARP) {
@@ -712,11 +720,11 @@ int tc_pick_stages(int W)
     return 0;
 }
 
-template <int W, int F, bool CONCAT>
+template <int W, int F, bool CONCAT, bool LOCAL>
 int launch_tc(const TcParams& p, uint32_t smem, int blocks, cudaStream_t stream)
 {
-    NIF_CUDA_TRY(cudaFuncSetAttribute(k_fused_encode_mlp<W, F, CONCAT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_fused_encode_mlp<W, F, CONCAT><<<blocks, TC_THREADS, smem, stream>>>(p);
+    NIF_CUDA_TRY(cudaFuncSetAttribute(k_fused_encode_mlp<W, F, CONCAT, LOCAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_fused_encode_mlp<W, F, CONCAT, LOCAL><<<blocks, TC_THREADS, smem, stream>>>(p);
     nif_count_launch(1);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;
@@ -776,6 +784,7 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     p.table = (const __half*)net->table;
     p.w_img = (const uint8_t*)net->w_tc; p.w_bytes = s.w_bytes; p.w1_bytes = s.w1_bytes;
     p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
+    p.map = NifMapCtx{bvh->theta_max, bvh->bend_k, bvh->lattice, bvh->nv, bvh->local_inverse};
     p.origin = rays->origin; p.dir = rays->dir;
     p.out = *out; p.scratch = scratch; p.tile_counter = &scratch->pad[4]; p.hit_list = hit_list; p.flags = flags;
     p.enc_mode = d->enc_mode;
@@ -791,8 +800,9 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     const int blocks = (int)(max_tiles < n_sm ? max_tiles : n_sm);
     // the concatenation variant is its own instantiation so that the composition kernel's code is untouched
 #define NIF_TC_CASE(WW, FF) if (d->width == WW && d->feat == FF) \
-        return d->enc_mode == NIF_ENC_CONCAT ? launch_tc<WW, FF, true>(p, smem, blocks, stream) \
-                                             : launch_tc<WW, FF, false>(p, smem, blocks, stream)
+        return d->enc_mode == NIF_ENC_CONCAT \
+            ? (bvh->local_inverse ? launch_tc<WW, FF, true, true>(p, smem, blocks, stream) : launch_tc<WW, FF, true, false>(p, smem, blocks, stream)) \
+            : (bvh->local_inverse ? launch_tc<WW, FF, false, true>(p, smem, blocks, stream) : launch_tc<WW, FF, false, false>(p, smem, blocks, stream))
     NIF_TC_CASE(32, 2); NIF_TC_CASE(64, 2); NIF_TC_CASE(128, 2);
     NIF_TC_CASE(32, 4); NIF_TC_CASE(64, 4); NIF_TC_CASE(128, 4);
 #undef NIF_TC_CASE

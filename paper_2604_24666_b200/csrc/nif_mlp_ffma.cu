@@ -17,7 +17,7 @@ struct FfmaParams {
     int d_in, hidden_layers, width, n_out;
     const void* table;
     const void* w[NIF_MAX_LAYERS];
-    float theta_max, bend_k;
+    NifMapCtx map;
     const float* origin; const float* dir;
     nif_query_out out;
     const NifQueryScratch* scratch;
@@ -100,11 +100,12 @@ k_encode_mlp_ffma(const FfmaParams p)
             if (h < n_hit) {
                 ray = p.hit_list[h];
                 ti = p.out.t_in[ray]; to = p.out.t_out[ray];
-                const float t = e ? to : ti;
-                const float X = fmaf(t, p.dir[3 * ray], p.origin[3 * ray]);
-                const float Y = fmaf(t, p.dir[3 * ray + 1], p.origin[3 * ray + 1]);
-                const float Z = fmaf(t, p.dir[3 * ray + 2], p.origin[3 * ray + 2]);
-                nif_inverse_deform(p.theta_max, p.bend_k, X, Y, Z, x, y, z);
+                const float oo[3] = {p.origin[3 * ray], p.origin[3 * ray + 1], p.origin[3 * ray + 2]};
+                const float dd[3] = {p.dir[3 * ray], p.dir[3 * ray + 1], p.dir[3 * ray + 2]};
+                float ri[3], ro[3];
+                if (p.map.local) nif_map_back_pair<true>(p.map, p.out.voxel_id[ray], oo, dd, ti, to, ri, ro);
+                else nif_map_back_pair<false>(p.map, 0, oo, dd, ti, to, ri, ro);
+                x = e ? ro[0] : ri[0]; y = e ? ro[1] : ri[1]; z = e ? ro[2] : ri[2];
             }
             xn[(r * 2 + e) * 3 + 0] = nif_normalise(x);
             xn[(r * 2 + e) * 3 + 1] = nif_normalise(y);
@@ -151,7 +152,8 @@ k_encode_mlp_ffma(const FfmaParams p)
             float z[NIF_N_OUT];
 #pragma unroll
             for (int a = 0; a < NIF_N_OUT; ++a) z[a] = a < p.n_out ? nxt[r * 16 + a] : 0.0f;
-            nif_decode_store(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.theta_max, p.bend_k});
+            if (p.map.local) nif_decode_store<true>(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map});
+            else nif_decode_store<false>(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map});
         }
         __syncthreads();
     }
@@ -191,7 +193,7 @@ int nif_launch_ffma(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch*
     p.n_out = (flags & NIF_OCCLUSION_ONLY) ? 1 : NIF_N_OUT;
     p.table = net->table;
     for (int i = 0; i <= net->desc.hidden_layers; ++i) p.w[i] = net->w_plain[i];
-    p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
+    p.map = NifMapCtx{bvh->theta_max, bvh->bend_k, bvh->lattice, bvh->nv, bvh->local_inverse};
     p.origin = rays->origin; p.dir = rays->dir;
     p.out = *out; p.scratch = scratch; p.hit_list = hit_list; p.flags = flags;
     const int S = 1 + 2 * net->enc.bands;
