@@ -199,6 +199,13 @@ __device__ inline void store_node(NifNode* dst, const NifNode& nd)
     for (int i = 0; i < 16; ++i) d[i] = s[i];
 }
 
+// child boxes as stored in a node: one ulp outwards (nif_traverse.cu slab_node); the exact boxes stay in
+// `boxes` for the level above and for the root
+// (at least 1e-20 in absolute terms: next to 0 an ulp is a denormal, and (hi - o) * FLT_MAX must stay huge
+// for a ray parallel to the slab with o exactly on the plane)
+__device__ __forceinline__ float ulp_down(float v) { return isfinite(v) ? fminf(nextafterf(v, -INFINITY), v - 1e-20f) : v; }
+__device__ __forceinline__ float ulp_up(float v) { return isfinite(v) ? fmaxf(nextafterf(v, INFINITY), v + 1e-20f) : v; }
+
 __global__ void k_write_bricks(int nv, uint32_t n_bricks, const uint8_t* __restrict__ mask,
                                const uint32_t* __restrict__ offs, uint32_t node_base,
                                const float4* __restrict__ lat, NifNode* __restrict__ nodes,
@@ -226,7 +233,7 @@ __global__ void k_write_bricks(int nv, uint32_t n_bricks, const uint8_t* __restr
             }
             for (int a = 0; a < 3; ++a) { blo[a] = fminf(blo[a], lo[a]); bhi[a] = fmaxf(bhi[a], hi[a]); }
         }
-        for (int a = 0; a < 3; ++a) { nd.lo[a][c] = lo[a]; nd.hi[a][c] = hi[a]; }
+        for (int a = 0; a < 3; ++a) { nd.lo[a][c] = ulp_down(lo[a]); nd.hi[a][c] = ulp_up(hi[a]); }
         nd.child[c] = id;
     }
     nd.mask = bits; nd.is_brick = 1;
@@ -259,7 +266,7 @@ __global__ void k_write_level(uint32_t n_cells, const uint8_t* __restrict__ mask
             lo[0] = l.x; lo[1] = l.y; lo[2] = l.z; hi[0] = h.x; hi[1] = h.y; hi[2] = h.z;
             for (int a = 0; a < 3; ++a) { blo[a] = fminf(blo[a], lo[a]); bhi[a] = fmaxf(bhi[a], hi[a]); }
         }
-        for (int a = 0; a < 3; ++a) { nd.lo[a][c] = lo[a]; nd.hi[a][c] = hi[a]; }
+        for (int a = 0; a < 3; ++a) { nd.lo[a][c] = ulp_down(lo[a]); nd.hi[a][c] = ulp_up(hi[a]); }
         nd.child[c] = id;
     }
     (void)child_mask;

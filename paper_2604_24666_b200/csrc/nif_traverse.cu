@@ -41,6 +41,34 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
     return (tmin <= tmax) && (tmax >= 0.0f);
 }
 
+// Child boxes of a hierarchy node only PRUNE (a voxel's own interval comes from voxel_hit), so their test
+// may be cheaper as long as it stays conservative: the build stores them inflated by one ulp outwards
+// (nif_build.cu) and the ray carries inverses clamped to +-FLT_MAX, so a ray parallel to a slab and exactly
+// on the voxel's boundary plane lies strictly inside the inflated slab and 0 * inv is 0, never NaN -- the
+// NaN handling of axis_interval (a third of the node step's instructions) is not needed.  Same operation
+// sequence otherwise, so monotone rounding keeps every enclosed voxel's interval inside the node's.
+__device__ __forceinline__ bool slab_node(float lx, float ly, float lz, float hx, float hy, float hz,
+                                          const Ray& r, float& bn)
+{
+    const float x0 = __fmul_rn(__fsub_rn(lx, r.ox), r.ix), x1 = __fmul_rn(__fsub_rn(hx, r.ox), r.ix);
+    const float y0 = __fmul_rn(__fsub_rn(ly, r.oy), r.iy), y1 = __fmul_rn(__fsub_rn(hy, r.oy), r.iy);
+    const float z0 = __fmul_rn(__fsub_rn(lz, r.oz), r.iz), z1 = __fmul_rn(__fsub_rn(hz, r.oz), r.iz);
+    const float tmin = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fminf(z0, z1));
+    const float tmax = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fmaxf(z0, z1));
+    bn = fmaxf(tmin, 0.0f);
+    return (tmin <= tmax) && (tmax >= 0.0f);
+}
+
+// r.ix/iy/iz are the CLAMPED inverses (node tests); the exact ones (+-inf for a zero component), which the
+// root box and the voxel's own box need (R10), are recomputed where used
+__device__ __forceinline__ Ray exact_inverses(const Ray& r)
+{
+    Ray e = r;
+    e.ix = __fdiv_rn(1.0f, r.dx); e.iy = __fdiv_rn(1.0f, r.dy); e.iz = __fdiv_rn(1.0f, r.dz);
+    return e;
+}
+__device__ __forceinline__ float clamp_inverse(float inv) { return fminf(fmaxf(inv, -3.402823466e38f), 3.402823466e38f); }
+
 struct V3 { float x, y, z; };
 
 __device__ __forceinline__ V3 vsub(V3 a, V3 b)
@@ -101,7 +129,7 @@ __device__ __forceinline__ bool voxel_hit(const float4* __restrict__ lat, int nv
         lz = fminf(lz, q[c].z); hz = fmaxf(hz, q[c].z);
     }
     float bn, bf;
-    if (!slab(lx, ly, lz, hx, hy, hz, r, bn, bf)) return false;
+    if (!slab(lx, ly, lz, hx, hy, hz, exact_inverses(r), bn, bf)) return false;
     const V3 o{r.ox, r.oy, r.oz}, d{r.dx, r.dy, r.dz};
     float tlo = INFINITY, thi = -INFINITY;
     bool any = false;
@@ -242,7 +270,11 @@ k_traverse_persistent(const TravParams p)
                 r.ix = __fdiv_rn(1.0f, r.dx); r.iy = __fdiv_rn(1.0f, r.dy); r.iz = __fdiv_rn(1.0f, r.dz);
                 best_id = -1; best_in = INFINITY; best_out = INFINITY; sp = 0;
                 float bn, bf;
-                if (p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf)) {
+                const bool root_hit = p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf);
+                if constexpr (!AFTER) {       // successor rounds keep the exact inverses: they also prune on the far end
+                    r.ix = clamp_inverse(r.ix); r.iy = clamp_inverse(r.iy); r.iz = clamp_inverse(r.iz);
+                }
+                if (root_hit) {
                     stack[sp++] = make_uint2((uint32_t)p.root, __float_as_uint(bn));
                 } else {
                     retire_ray(p, ray, -1, INFINITY, INFINITY);
@@ -290,11 +322,15 @@ k_traverse_persistent(const TravParams p)
                 for (int c = 0; c < 8; ++c) {
                     key[c] = 0xffffffffu;
                     if (__any_sync(0xffffffffu, (meta.x >> c) & 1u)) {       // coherent warps skip absent octants
-                        float cn, cf;
+                        float cn, cf = INFINITY;
                         // AFTER: every voxel below has t_in <= its box's far end <= cf (boxes nest, R10), so a
                         // child that ends before after_t holds no successor
-                        const bool ok = slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf) &&
-                                        ((meta.x >> c) & 1u) && !(cn > best_in) && !(AFTER && cf < after_t);
+                        bool ok;
+                        if constexpr (AFTER)
+                            ok = slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf);
+                        else
+                            ok = slab_node(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn);
+                        ok = ok && ((meta.x >> c) & 1u) && !(cn > best_in) && !(AFTER && cf < after_t);
                         // cn >= 0: its bit pattern orders like an integer; the 3 low mantissa bits make
                         // room for the octant (t_near only gets smaller: pruning stays conservative).  ~
                         // turns the ascending network into "farthest first"; rejected children sort last.
@@ -364,7 +400,9 @@ k_traverse_simple(const TravParams p)
     uint2 stack[STACK_MAX];
     int sp = 0;
     float bn, bf;
-    if (p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf))
+    const bool root_hit = p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf);
+    r.ix = clamp_inverse(r.ix); r.iy = clamp_inverse(r.iy); r.iz = clamp_inverse(r.iz);
+    if (root_hit)
         stack[sp++] = make_uint2((uint32_t)p.root, __float_as_uint(bn));
     while (sp > 0) {
         const uint2 e = stack[--sp];
@@ -400,8 +438,8 @@ k_traverse_simple(const TravParams p)
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
             if (!((meta.x >> c) & 1u)) continue;
-            float cn, cf;
-            if (slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf) &&
+            float cn;
+            if (slab_node(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn) &&
                 !(cn > best_in) && sp < STACK_MAX) {
                 int q = sp++;
                 while (q > sp0 && __uint_as_float(stack[q - 1].y) < cn) { stack[q] = stack[q - 1]; --q; }

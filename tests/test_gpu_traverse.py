@@ -23,9 +23,9 @@ def P():
     return parity
 
 
-def _trav(H, case):
+def _trav(H, case, flags=0):
     import paper_2604_24666_b200 as nif
-    return H.run_gpu(case, flags=nif.NIF_TRAVERSE_ONLY, raw_logits=False)
+    return H.run_gpu(case, flags=nif.NIF_TRAVERSE_ONLY | flags, raw_logits=False)
 
 
 @pytest.mark.parametrize("cfg_id,pose_index", [(0, 0), (1, 0), (2, 3), (4, 0)])
@@ -183,3 +183,41 @@ def test_both_traversal_kernels_agree_bit_for_bit(oracle, H, P, cfg_id, pose_ind
     side = H.OracleSide(oracle, case)
     idx = np.arange(0, len(case.origin), max(1, len(case.origin) // 4000))
     P.assert_traversal(P.compare_traversal(H.subset(res["incoherent"], idx), side.query(idx, traverse_only=True)))
+
+
+def test_axis_parallel_rays_in_lattice_planes(oracle, H, P):
+    """Degenerate rays for the node test (inverse direction +-inf, origin exactly on box planes): rays
+    parallel to one or two axes whose origins lie exactly on lattice planes of an identity-pose grid,
+    both signs of direction and of zero.  Ids and t must still equal the brute-force definition."""
+    nv = 8
+    rng = np.random.default_rng(5)
+    occ = (rng.random(nv ** 3) < 0.6).astype(np.uint8)
+    cfg = I.scaled(I.get_config(0), nv=nv)
+    g = (2.0 * np.arange(nv + 1) - nv) / nv
+    os_, ds_ = [], []
+    for axis in range(3):
+        for sign in (1.0, -1.0):
+            for zero in (0.0, -0.0):
+                for a in g:
+                    for b in list(g[::2]) + [0.123, -0.456]:
+                        o = np.zeros(3); d = np.full(3, zero)
+                        o[axis] = -3.0 * sign; d[axis] = sign
+                        o[(axis + 1) % 3] = a; o[(axis + 2) % 3] = b
+                        os_.append(o.copy()); ds_.append(d.copy())
+                        # parallel to one axis only: tilt within the plane of the second axis
+                        d2 = d.copy(); d2[(axis + 2) % 3] = 0.25 * sign
+                        d2 /= np.linalg.norm(d2)
+                        os_.append(o.copy()); ds_.append(d2)
+    o = np.array(os_, np.float32); d = np.array(ds_, np.float32)
+    case = H.make_case(0, with_net=False, cfg=cfg, occ=occ, pose=[0.0, 0.0])
+    case.origin, case.direction = o, d
+    case.origin_d, case.direction_d = torch.from_numpy(o).cuda(), torch.from_numpy(d).cuda()
+    lat = oracle.deform_lattice(nv, 0.0, 0.0)
+    vid, ti, to = oracle.traverse_brute(nv, occ, lat, o, d)
+    ref = {"voxel_id": vid, "t_in": ti, "t_out": to}
+    for fl in (8, 16):                                   # NIF_TRAVERSE_COHERENT, NIF_TRAVERSE_INCOHERENT: both kernels
+        gpu = _trav(H, case, flags=fl)
+        m = P.compare_traversal(gpu, ref)
+        P.assert_traversal(m)
+        assert m["t_in_bit_mismatch"] == 0 and m["t_out_bit_mismatch"] == 0, m
+    assert (vid >= 0).sum() > 1000
