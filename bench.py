@@ -267,13 +267,23 @@ def run_ours(args) -> None:
         refit_ms.append(e0.elapsed_time(e1))
     n_per_pose = cfg.rays_per_pose
     n_total = n_per_pose * cfg.n_poses
+    batched = cfg.n_poses > 1 and args.poses == "batched" and not args.walk
+    if batched:                                        # one nif_query_poses over the rays of all poses (B:9)
+        all_o = torch.cat([p["o"] for p in poses]); all_d = torch.cat([p["d"] for p in poses])
+        all_pid = torch.cat([torch.full((n_per_pose,), i, dtype=torch.int32, device=dev) for i in range(cfg.n_poses)])
+        all_bvh = [p["bvh"] for p in poses]
+        out_all = nif.alloc_outputs(n_total, device=dev)
+        ws_all = None
     out = nif.alloc_outputs(n_per_pose, device=dev)
     walk_out = nif.alloc_walk_outputs(n_per_pose, device=dev) if args.walk else None
     ws = None
     ws_multi = None
 
     def step():
-        nonlocal ws, ws_multi
+        nonlocal ws, ws_multi, ws_all
+        if batched:
+            ws_all = nif.nif_query_poses(all_bvh, net, all_o, all_d, all_pid, out_all, workspace=ws_all, flags=flags)
+            return
         for p in poses:
             if args.walk:                              # multi-voxel walk, --walk K rounds
                 ws_multi = nif.nif_query_multi(p["bvh"], net, p["o"], p["d"], out, walk_out, args.walk,
@@ -317,6 +327,7 @@ def run_ours(args) -> None:
         elapsed_ms = float(t.item())
     ms_per_step = elapsed_ms / args.steps
     value = world * n_total / (ms_per_step * 1e-3) / 1e6
+    launches_per_query = 1 if batched else cfg.n_poses     # per-kernel times below are per query launch
 
     walk_stats = None
     if args.walk:
@@ -372,7 +383,7 @@ def run_ours(args) -> None:
     nq = max(prof["n_queries"], 1)
     net_ms = prof["network_ms"] / nq                    # average launch duration, CUDA events
     trav_ms = prof["traverse_ms"] / nq
-    hits_per_launch = n_hit / cfg.n_poses
+    hits_per_launch = n_hit / launches_per_query
     table_bytes = params.table_storage().nbytes
     l2_resident = table_bytes <= (64 << 20)              # 126 MB L2: a 32 MiB table stays resident, 512 MiB does not
     probe_bytes = (32 << 20) if l2_resident else (256 << 20)
@@ -399,11 +410,11 @@ def run_ours(args) -> None:
                 "sector_worst_case": {"achieved": gather_gbs, "frac": gather_gbs / probe["gbps"],
                                       "what": "every lane's gather counted as its own 32 B sector (SURVEY 8(d).2 worst case); "
                                               "exceeds 1 when the 32 rays of a warp share sectors"},
-                "avg_launch_ms": net_ms, "share_of_step": net_ms * cfg.n_poses / ms_per_step,
+                "avg_launch_ms": net_ms, "share_of_step": net_ms * launches_per_query / ms_per_step,
                 "tensor": {"bound": "tensor", "achieved": tensor_tfs, "peak": peaks["tf_sustained"],
                            "unit": "TFLOP/s", "frac": tensor_tfs / peaks["tf_sustained"],
                            "peak_source": f"{peaks['source']} bf16 sustained (fp16 same pipe)"},
-                "hbm": {"bound": "hbm", "achieved": (n_per_pose * (work["hbm_bytes_per_ray_in"] + work["hbm_bytes_per_ray_out"]))
+                "hbm": {"bound": "hbm", "achieved": ((n_total / launches_per_query) * (work["hbm_bytes_per_ray_in"] + work["hbm_bytes_per_ray_out"]))
                         / ((net_ms + trav_ms) * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "peak_source": f"{peaks['source']} copy bandwidth"}}
     roofline["hbm"]["frac"] = roofline["hbm"]["achieved"] / peaks["hbm_gbs"]
@@ -414,7 +425,8 @@ def run_ours(args) -> None:
                     "the real network / event-timed kernel duration", "avg_launch_ms": mlp_probe,
             "achieved": tf, "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": tf / peaks["tf_burst"],
             "peak_source": f"{peaks['source']} bf16 burst (fp16 same pipe)"}
-    kernels = {"traverse_ms": trav_ms, "encode_mlp_ms": net_ms, "traverse_share": trav_ms * cfg.n_poses / ms_per_step,
+    kernels = {"traverse_ms": trav_ms, "encode_mlp_ms": net_ms, "traverse_share": trav_ms * launches_per_query / ms_per_step,
+               "queries_per_step": launches_per_query,
                "bvh_build_ms_per_pose": float(np.median(build_ms)),
                "bvh_refit_ms_per_pose": float(np.median(refit_ms))}
 
@@ -427,6 +439,7 @@ def run_ours(args) -> None:
                        "hit_rays_per_step_per_gpu": n_hit, "hit_fraction": n_hit / n_total,
                        "l2": "no flush: per-step working set (rays 24 B + outputs 60 B per ray + 32 MiB table) "
                              "exceeds the 126 MB L2; the hash table is meant to stay L2-resident",
+                       "poses": ("one nif_query_poses over all poses" if batched else "one nif_query per pose"),
                        "parallelism": f"dp{world} (independent frames per rank, no collective)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "nif_query_host (pinned host buffers, chunked, 3 streams)", "steps": e2e_steps},
@@ -457,6 +470,8 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--enc", default="compose", choices=["compose", "concat"],
                     help="hybrid-encoding reading: the paper's composition (default, headline) or concatenation")
+    ap.add_argument("--poses", default="batched", choices=["batched", "loop"],
+                    help="multi-pose configs: one nif_query_poses per step (default) or one nif_query per pose")
     ap.add_argument("--walk", type=int, default=0, help="time nif_query_multi with this max_steps instead of nif_query "
                                                         "(SURVEY 8(f) f1; not the headline; use --params varpres)")
     args = ap.parse_args()

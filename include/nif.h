@@ -225,6 +225,18 @@ int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
               const nif_query_out* out, void* workspace, size_t workspace_bytes,
               unsigned flags, void* stream);
 
+/* Several poses of one object in one query (B:9 "8 poses ... One BVH per pose ... Network ... shared across
+ * all poses"): ray r is traced against bvhs[pose_id[r]].  `bvhs`: HOST array of n_poses (1..64) BVHs of the
+ * same grid size and the same kind (all closed-form or all lattice poses); `pose_id`: DEVICE, rays->n entries
+ * in [0, n_poses).  Everything else as nif_query (same outputs, same flags except NIF_PROBE_SKIP_GATHER).
+ * Hit rays are grouped by the REST-space voxel they hit across poses, which is what the shared hash grid is
+ * indexed by, so one batched call is faster than n_poses separate ones.  Workspace:
+ * nif_query_poses_workspace_bytes(rays->n).  Enqueue only. */
+int nif_query_poses_workspace_bytes(int64_t n, size_t* bytes);
+int nif_query_poses(const nif_bvh* const* bvhs, int32_t n_poses, const nif_net* net,
+                    const nif_ray_batch* rays, const int32_t* pose_id, const nif_query_out* out,
+                    void* workspace, size_t workspace_bytes, unsigned flags, void* stream);
+
 /* -------- evaluation-time multi-voxel walk (R22, R23) ------------------- */
 
 /* Outcome of a walk, per ray. */

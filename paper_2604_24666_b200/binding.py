@@ -99,6 +99,9 @@ def lib() -> C.CDLL:
         L.nif_query_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_query.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut),
                                 C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
+        L.nif_query_poses_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
+        L.nif_query_poses.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_void_p, C.POINTER(_RayBatch), C.c_void_p,
+                                      C.POINTER(_QueryOut), C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
         L.nif_query_multi_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_query_multi.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut),
                                       C.POINTER(_WalkOut), C.c_int32, C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
@@ -298,6 +301,30 @@ def nif_query(bvh: Bvh, net: Net | None, origin: torch.Tensor, direction: torch.
     q = _out_struct(out)
     _check(lib().nif_query(bvh.handle, net.handle if net is not None else None, C.byref(rb), C.byref(q),
                            workspace.data_ptr(), workspace.numel(), flags, _stream_ptr(stream)), "nif_query")
+    return workspace
+
+
+def nif_query_poses_workspace_bytes(n: int) -> int:
+    b = C.c_size_t()
+    _check(lib().nif_query_poses_workspace_bytes(n, C.byref(b)), "nif_query_poses_workspace_bytes")
+    return b.value
+
+
+def nif_query_poses(bvhs: list, net: Net | None, origin: torch.Tensor, direction: torch.Tensor, pose_id: torch.Tensor,
+                    out: dict, workspace: torch.Tensor | None = None, flags: int = 0, stream=None) -> torch.Tensor:
+    """One query over rays of several poses: ray r is traced against bvhs[pose_id[r]] (include/nif.h)."""
+    n = origin.shape[0]
+    assert origin.is_cuda and direction.is_cuda and origin.dtype == torch.float32
+    assert origin.is_contiguous() and direction.is_contiguous() and direction.shape[0] == n
+    assert pose_id.is_cuda and pose_id.dtype == torch.int32 and pose_id.is_contiguous() and pose_id.numel() == n
+    if workspace is None:
+        workspace = _ws(nif_query_poses_workspace_bytes(n))
+    rb = _RayBatch(n, origin.data_ptr(), direction.data_ptr())
+    q = _out_struct(out)
+    handles = (C.c_void_p * len(bvhs))(*[b.handle for b in bvhs])
+    _check(lib().nif_query_poses(handles, len(bvhs), net.handle if net is not None else None, C.byref(rb),
+                                 pose_id.data_ptr(), C.byref(q), workspace.data_ptr(), workspace.numel(), flags,
+                                 _stream_ptr(stream)), "nif_query_poses")
     return workspace
 
 

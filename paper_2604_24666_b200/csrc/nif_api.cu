@@ -243,6 +243,65 @@ extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_b
     return rc;
 }
 
+// Several poses of one object in ONE query: every ray names its pose (SURVEY 8(f) f2, B:9 "one BVH per pose ...
+// network shared across all poses").  Hit rays are binned by rest-space voxel across poses, so the encode tiles
+// mix rays of all poses that hit the same voxel: they look up the same table cells.
+extern "C" int nif_query_poses_workspace_bytes(int64_t n, size_t* bytes)
+{
+    size_t q = 0;
+    int rc = nif_query_workspace_bytes(n, &q);
+    if (rc != NIF_OK) return rc;
+    *bytes = align_up(q, 256) + align_up(sizeof(NifPoseDesc) * NIF_MAX_POSES, 256);
+    return NIF_OK;
+}
+
+extern "C" int nif_query_poses(const nif_bvh* const* bvhs, int32_t n_poses, const nif_net* net,
+                               const nif_ray_batch* rays, const int32_t* pose_id, const nif_query_out* out,
+                               void* workspace, size_t workspace_bytes, unsigned flags, void* stream_)
+{
+    if (!bvhs || n_poses < 1 || n_poses > NIF_MAX_POSES || !pose_id) return NIF_ERR_INVALID_ARG;
+    for (int i = 0; i < n_poses; ++i) {
+        if (!bvhs[i]) return NIF_ERR_INVALID_ARG;
+        if (bvhs[i]->nv != bvhs[0]->nv || bvhs[i]->local_inverse != bvhs[0]->local_inverse) return NIF_ERR_INVALID_ARG;
+    }
+    int rc = validate_query(bvhs[0], net, rays, out, flags);
+    if (rc != NIF_OK) return rc;
+    if (flags & NIF_PROBE_SKIP_GATHER) return NIF_ERR_INVALID_ARG;
+    if (rays->n == 0) return NIF_OK;
+    size_t need = 0, qbytes = 0;
+    nif_query_poses_workspace_bytes(rays->n, &need);
+    nif_query_workspace_bytes(rays->n, &qbytes);
+    if (!workspace || ((uintptr_t)workspace & 255u) != 0 || workspace_bytes < need) return NIF_ERR_WORKSPACE;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    NifQueryWs ws;
+    nif_query_ws_layout(bvhs[0], rays->n, workspace, &ws);
+    NifPoseDesc* d_desc = (NifPoseDesc*)((char*)workspace + align_up(qbytes, 256));
+    NifPoseDesc h_desc[NIF_MAX_POSES];
+    memset(h_desc, 0, sizeof(h_desc));
+    for (int i = 0; i < n_poses; ++i) {
+        const nif_bvh* b = bvhs[i];
+        h_desc[i].nodes = b->nodes; h_desc[i].lat = b->lattice; h_desc[i].root = b->root;
+        for (int a = 0; a < 3; ++a) { h_desc[i].lo[a] = b->lo[a]; h_desc[i].hi[a] = b->hi[a]; }
+        h_desc[i].theta_max = b->theta_max; h_desc[i].bend_k = b->bend_k; h_desc[i].local_inverse = b->local_inverse;
+    }
+    // pageable source: the copy is staged before the call returns, so the stack array may go out of scope
+    NIF_CUDA_TRY(cudaMemcpyAsync(d_desc, h_desc, sizeof(NifPoseDesc) * (size_t)n_poses, cudaMemcpyHostToDevice, stream));
+    NifPoseBatch batch{d_desc, pose_id, n_poses};
+    const bool traverse_only = (flags & NIF_TRAVERSE_ONLY) != 0;
+    NIF_CUDA_TRY(cudaMemsetAsync(workspace, 0, sizeof(NifQueryScratch) + (traverse_only ? 0 : (size_t)ws.n_bins * 4), stream));
+    const int prof = nif_prof_begin(stream);
+    // the coherence vote looks at ray geometry only; its "extent" comes from the first pose
+    rc = nif_launch_traverse(bvhs[0], rays, out, &ws, flags, nullptr, stream, &batch);
+    if (rc == NIF_OK && !traverse_only) rc = nif_launch_bin_hits(bvhs[0], rays, out, &ws, nullptr, stream);
+    nif_prof_mark(prof, 1, stream);
+    if (rc != NIF_OK || traverse_only) return rc;
+    const bool use_tc = net->desc.dtype == NIF_F16 && net->tc_supported && !(flags & NIF_ENGINE_FFMA);
+    if (use_tc) rc = nif_launch_fused_tc(bvhs[0], net, rays, out, ws.scratch, ws.hit_list, flags, stream, &batch);
+    else rc = nif_launch_ffma(bvhs[0], net, rays, out, ws.scratch, ws.hit_list, flags, stream, &batch);
+    nif_prof_mark(prof, 2, stream);
+    return rc;
+}
+
 extern "C" int nif_query_last_hit_count(const void* workspace, void* stream_, int64_t* n_hit)
 {
     if (!workspace || !n_hit) return NIF_ERR_INVALID_ARG;

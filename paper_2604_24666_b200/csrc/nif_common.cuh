@@ -88,6 +88,25 @@ struct NifQueryWs {                    // pointers into the caller's workspace
     int bin_shift, nvb;                // bin = (ix >> s) + nvb * ((iy >> s) + nvb * (iz >> s))
 };
 
+// nif_query_poses: what the kernels need of one pose's BVH (device array, one entry per pose)
+#define NIF_MAX_POSES 64
+struct NifPoseDesc {
+    const NifNode* nodes;
+    const float4* lat;
+    float lo[3], hi[3];                // root box
+    int32_t root;
+    float theta_max, bend_k;
+    int32_t local_inverse;
+    int32_t pad[2];
+};
+static_assert(sizeof(NifPoseDesc) == 64, "pose descriptor is 64 bytes");
+
+struct NifPoseBatch {                  // NULL pointers outside nif_query_poses
+    const NifPoseDesc* poses;          // device
+    const int32_t* pose_id;            // device, per ray
+    int n_poses;
+};
+
 // one round of the multi-voxel walk (nif_walk.cu): round 0 is the plain nearest-voxel query over all
 // rays; rounds >= 1 run over `ray_list` (rays still walking) and look for each ray's next voxel
 struct NifWalkRound {
@@ -107,16 +126,19 @@ extern "C" void nif_count_launch(int n);
 
 // launchers implemented in the individual .cu files
 int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        const NifQueryWs* ws, unsigned flags, const NifWalkRound* walk, cudaStream_t stream);
+                        const NifQueryWs* ws, unsigned flags, const NifWalkRound* walk, cudaStream_t stream,
+                        const NifPoseBatch* batch = nullptr);
 int nif_launch_bin_hits(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
                         const NifQueryWs* ws, const NifWalkRound* walk, cudaStream_t stream);
 void nif_query_ws_layout(const nif_bvh* bvh, int64_t n, void* workspace, NifQueryWs* ws);
 int nif_launch_ffma(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                     const nif_query_out* out, const NifQueryScratch* scratch,
-                    const int32_t* hit_list, unsigned flags, cudaStream_t stream);
+                    const int32_t* hit_list, unsigned flags, cudaStream_t stream,
+                    const NifPoseBatch* batch = nullptr);
 int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                         const nif_query_out* out, NifQueryScratch* scratch,
-                        const int32_t* hit_list, unsigned flags, cudaStream_t stream);
+                        const int32_t* hit_list, unsigned flags, cudaStream_t stream,
+                        const NifPoseBatch* batch = nullptr);
 int nif_tc_pack_weights(nif_net* net, cudaStream_t stream);
 int nif_tc_supported(const nif_net_desc* d);
 

@@ -86,6 +86,17 @@ struct NifMapCtx {
     int local;                // 1: the BVH was built from a user lattice -> voxel-local inverse (R27)
 };
 
+// nif_query_poses: the pose of this ray (closed-form parameters, or its lattice) replaces the batch-wide one
+__device__ __forceinline__ NifMapCtx nif_ray_map(const NifMapCtx& base, const NifPoseBatch& b, long long ray)
+{
+    NifMapCtx m = base;
+    if (b.pose_id) {
+        const NifPoseDesc* pd = b.poses + b.pose_id[ray];
+        m.theta_max = pd->theta_max; m.bend_k = pd->bend_k; m.lat = pd->lat;
+    }
+    return m;
+}
+
 // rest images of a ray's entry and exit points (both lie in voxel `vid`)
 template <bool LOCAL>
 __device__ __forceinline__ void nif_map_back_pair(const NifMapCtx& m, int32_t vid, const float* __restrict__ o,
@@ -210,6 +221,7 @@ struct NifDecodeCtx {
     const float* origin;
     const float* dir;
     NifMapCtx map;
+    NifPoseBatch batch;
 };
 
 template <bool LOCAL>
@@ -261,7 +273,7 @@ __device__ __forceinline__ void nif_decode_store(const float* __restrict__ z, fl
         if (out.hit_position_rest) {
             const float oo[3] = {ox, oy, oz}, dd[3] = {dx, dy, dz};
             float ri[3], ro[3];
-            nif_map_back_pair<LOCAL>(ctx.map, LOCAL ? out.voxel_id[ray] : 0, oo, dd, t_in, t_out, ri, ro);
+            nif_map_back_pair<LOCAL>(nif_ray_map(ctx.map, ctx.batch, ray), LOCAL ? out.voxel_id[ray] : 0, oo, dd, t_in, t_out, ri, ro);
             const float u = ell > 0.0f ? __saturatef(d / ell) : 0.0f;
             out.hit_position_rest[3 * ray] = fmaf(u, ro[0] - ri[0], ri[0]);
             out.hit_position_rest[3 * ray + 1] = fmaf(u, ro[1] - ri[1], ri[1]);

@@ -193,6 +193,7 @@ struct TcParams {
     unsigned int* tile_counter;   // dynamic tile scheduler (scratch header, zeroed per query)
     int enc_mode;                 // NIF_ENC_COMPOSE | NIF_ENC_CONCAT
     NifMapCtx map;                // (a2): pose, or the lattice for the voxel-local inverse
+    NifPoseBatch batch;           // nif_query_poses: per-ray pose (pose_id == NULL otherwise)
     const int32_t* hit_list;
     unsigned flags;
 };
@@ -473,11 +474,16 @@ k_fused_encode_mlp(const TcParams p)
                 if constexpr (LOCAL) {           // deformation given as a lattice: voxel-local inverse (R27)
                     const float oo[3] = {ox, oy, oz}, dd[3] = {dx, dy, dz};
                     float ri[3], ro[3];
-                    nif_map_back_pair<true>(p.map, p.out.voxel_id[nxt_ray], oo, dd, nxt_ti, nxt_to, ri, ro);
+                    nif_map_back_pair<true>(nif_ray_map(p.map, p.batch, nxt_ray), p.out.voxel_id[nxt_ray], oo, dd, nxt_ti, nxt_to, ri, ro);
                     xi = ri[0]; yi = ri[1]; zi = ri[2]; xo = ro[0]; yo = ro[1]; zo = ro[2];
                 } else {
-                nif_inverse_deform(p.theta_max, p.bend_k, fmaf(nxt_ti, dx, ox), fmaf(nxt_ti, dy, oy), fmaf(nxt_ti, dz, oz), xi, yi, zi);
-                nif_inverse_deform(p.theta_max, p.bend_k, fmaf(nxt_to, dx, ox), fmaf(nxt_to, dy, oy), fmaf(nxt_to, dz, oz), xo, yo, zo);
+                float th = p.theta_max, bk = p.bend_k;
+                if (p.batch.pose_id) {           // nif_query_poses: this ray's pose
+                    const NifPoseDesc* pd = p.batch.poses + p.batch.pose_id[nxt_ray];
+                    th = pd->theta_max; bk = pd->bend_k;
+                }
+                nif_inverse_deform(th, bk, fmaf(nxt_ti, dx, ox), fmaf(nxt_ti, dy, oy), fmaf(nxt_ti, dz, oz), xi, yi, zi);
+                nif_inverse_deform(th, bk, fmaf(nxt_to, dx, ox), fmaf(nxt_to, dy, oy), fmaf(nxt_to, dz, oz), xo, yo, zo);
                 }
             }
             float* rb = ray_buf + ((size_t)b * TC_TILE + r) * 8;
@@ -523,7 +529,7 @@ k_fused_encode_mlp(const TcParams p)
                 float z[NIF_N_OUT];
 #pragma unroll
                 for (int a = 0; a < NIF_N_OUT; ++a) z[a] = __uint_as_float(zr[a]);
-                nif_decode_store<LOCAL>(z, cur_ti, cur_to, cur_ray, p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map});
+                nif_decode_store<LOCAL>(z, cur_ti, cur_to, cur_ray, p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map, p.batch});
             }
         }
     } else if (warp == TC_MMA_WARP) {
@@ -772,7 +778,8 @@ int nif_tc_pack_weights(nif_net* net, cudaStream_t stream)
 }
 
 int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays, const nif_query_out* out,
-                        NifQueryScratch* scratch, const int32_t* hit_list, unsigned flags, cudaStream_t stream)
+                        NifQueryScratch* scratch, const int32_t* hit_list, unsigned flags, cudaStream_t stream,
+                        const NifPoseBatch* batch)
 {
     if (rays->n == 0) return NIF_OK;
     const nif_net_desc* d = &net->desc;
@@ -785,6 +792,7 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     p.w_img = (const uint8_t*)net->w_tc; p.w_bytes = s.w_bytes; p.w1_bytes = s.w1_bytes;
     p.theta_max = bvh->theta_max; p.bend_k = bvh->bend_k;
     p.map = NifMapCtx{bvh->theta_max, bvh->bend_k, bvh->lattice, bvh->nv, bvh->local_inverse};
+    p.batch = batch ? *batch : NifPoseBatch{nullptr, nullptr, 0};
     p.origin = rays->origin; p.dir = rays->dir;
     p.out = *out; p.scratch = scratch; p.tile_counter = &scratch->pad[4]; p.hit_list = hit_list; p.flags = flags;
     p.enc_mode = d->enc_mode;

@@ -18,6 +18,7 @@ struct FfmaParams {
     const void* table;
     const void* w[NIF_MAX_LAYERS];
     NifMapCtx map;
+    NifPoseBatch batch;
     const float* origin; const float* dir;
     nif_query_out out;
     const NifQueryScratch* scratch;
@@ -103,8 +104,9 @@ k_encode_mlp_ffma(const FfmaParams p)
                 const float oo[3] = {p.origin[3 * ray], p.origin[3 * ray + 1], p.origin[3 * ray + 2]};
                 const float dd[3] = {p.dir[3 * ray], p.dir[3 * ray + 1], p.dir[3 * ray + 2]};
                 float ri[3], ro[3];
-                if (p.map.local) nif_map_back_pair<true>(p.map, p.out.voxel_id[ray], oo, dd, ti, to, ri, ro);
-                else nif_map_back_pair<false>(p.map, 0, oo, dd, ti, to, ri, ro);
+                const NifMapCtx m = nif_ray_map(p.map, p.batch, ray);
+                if (p.map.local) nif_map_back_pair<true>(m, p.out.voxel_id[ray], oo, dd, ti, to, ri, ro);
+                else nif_map_back_pair<false>(m, 0, oo, dd, ti, to, ri, ro);
                 x = e ? ro[0] : ri[0]; y = e ? ro[1] : ri[1]; z = e ? ro[2] : ri[2];
             }
             xn[(r * 2 + e) * 3 + 0] = nif_normalise(x);
@@ -152,8 +154,8 @@ k_encode_mlp_ffma(const FfmaParams p)
             float z[NIF_N_OUT];
 #pragma unroll
             for (int a = 0; a < NIF_N_OUT; ++a) z[a] = a < p.n_out ? nxt[r * 16 + a] : 0.0f;
-            if (p.map.local) nif_decode_store<true>(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map});
-            else nif_decode_store<false>(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map});
+            if (p.map.local) nif_decode_store<true>(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map, p.batch});
+            else nif_decode_store<false>(z, tseg[2 * r], tseg[2 * r + 1], ray_of[r], p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map, p.batch});
         }
         __syncthreads();
     }
@@ -184,10 +186,11 @@ int launch_t(const FfmaParams& p, int feat, size_t smem, int blocks, cudaStream_
 
 int nif_launch_ffma(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                     const nif_query_out* out, const NifQueryScratch* scratch,
-                    const int32_t* hit_list, unsigned flags, cudaStream_t stream)
+                    const int32_t* hit_list, unsigned flags, cudaStream_t stream, const NifPoseBatch* batch)
 {
     if (rays->n == 0) return NIF_OK;
     FfmaParams p;
+    p.batch = batch ? *batch : NifPoseBatch{nullptr, nullptr, 0};
     p.enc = net->enc;
     p.d_in = net->d_in; p.hidden_layers = net->desc.hidden_layers; p.width = net->desc.width;
     p.n_out = (flags & NIF_OCCLUSION_ONLY) ? 1 : NIF_N_OUT;

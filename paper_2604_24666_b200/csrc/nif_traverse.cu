@@ -183,7 +183,36 @@ struct TravParams {
     const int32_t* ray_list;                  // NULL: rays 0..n-1
     const unsigned int* n_list;               // device count of ray_list
     float* walk_dist_accum;                   // NULL outside a walk; a ray that runs out of voxels gets 0
+    NifPoseBatch batch;                       // nif_query_poses: per-ray pose (MULTI kernels)
 };
+
+// MULTI kernels: the pose descriptors staged in shared memory, a pose index per lane
+template <bool MULTI> struct PoseView {
+    const NifPoseDesc* s;                     // shared-memory copy
+    __device__ __forceinline__ const NifNode* nodes(const TravParams& p, int pose) const { return MULTI ? s[pose].nodes : p.nodes; }
+    __device__ __forceinline__ const float4* lat(const TravParams& p, int pose) const { return MULTI ? s[pose].lat : p.lat; }
+    __device__ __forceinline__ int root(const TravParams& p, int pose) const { return MULTI ? s[pose].root : p.root; }
+    __device__ __forceinline__ bool root_hit(const TravParams& p, int pose, const Ray& r, float& bn) const
+    {
+        float bf;
+        if (MULTI) {
+            const NifPoseDesc& d = s[pose];
+            return d.root >= 0 && slab(d.lo[0], d.lo[1], d.lo[2], d.hi[0], d.hi[1], d.hi[2], r, bn, bf);
+        }
+        return p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf);
+    }
+};
+template <bool MULTI>
+__device__ __forceinline__ PoseView<MULTI> stage_poses(const TravParams& p, NifPoseDesc* s_pose)
+{
+    if (MULTI) {
+        const int n_words = p.batch.n_poses * (int)(sizeof(NifPoseDesc) / 4);
+        for (int i = threadIdx.x; i < n_words; i += blockDim.x)
+            reinterpret_cast<uint32_t*>(s_pose)[i] = reinterpret_cast<const uint32_t*>(p.batch.poses)[i];
+        __syncthreads();
+    }
+    return PoseView<MULTI>{s_pose};
+}
 
 // successor bound of the walk: only voxels whose (t_in, id) is lexicographically greater than the
 // voxel the ray evaluated last are candidates (R22)
@@ -233,16 +262,18 @@ __device__ __forceinline__ void retire_ray(const TravParams& p, long long ray, i
 // then all of them run the expensive 12-triangle voxel test together; finished lanes are refilled
 // from a global counter once enough of them are idle.  Incoherent rays (config 3) otherwise leave
 // 4 of 32 lanes active on average.
-template <bool AFTER>
+template <bool AFTER, bool MULTI>
 __global__ void __launch_bounds__(TRAV_BLOCK, TRAV_BLOCKS_PER_SM)
 k_traverse_persistent(const TravParams p)
 {
     if (!AFTER && *p.coherent_flag != 0u) return;         // k_traverse_simple takes this batch
+    __shared__ NifPoseDesc s_pose[MULTI ? NIF_MAX_POSES : 1];
+    const PoseView<MULTI> pv = stage_poses<MULTI>(p, s_pose);
+    int pose = 0;
     const long long n_rays = p.ray_list ? (long long)*p.n_list : p.n;
     float after_t = -INFINITY;                            // AFTER: successor bound (R22)
     int32_t after_id = -1;
     const int lane = threadIdx.x & 31;
-    const NifNode* __restrict__ nodes = p.nodes;
     uint2 stack[STACK_MAX];
     int sp = 0;
     long long ray = -1;                                   // -1: lane has no ray
@@ -265,17 +296,18 @@ k_traverse_persistent(const TravParams p)
             if (ray < 0 && cand < n_rays) {
                 ray = p.ray_list ? (long long)p.ray_list[cand] : cand;
                 if (AFTER) { after_t = p.out.t_in[ray]; after_id = p.out.voxel_id[ray]; }
+                if (MULTI) pose = p.batch.pose_id[ray];
                 r.ox = p.origin[3 * ray]; r.oy = p.origin[3 * ray + 1]; r.oz = p.origin[3 * ray + 2];
                 r.dx = p.dir[3 * ray]; r.dy = p.dir[3 * ray + 1]; r.dz = p.dir[3 * ray + 2];
                 r.ix = __fdiv_rn(1.0f, r.dx); r.iy = __fdiv_rn(1.0f, r.dy); r.iz = __fdiv_rn(1.0f, r.dz);
                 best_id = -1; best_in = INFINITY; best_out = INFINITY; sp = 0;
-                float bn, bf;
-                const bool root_hit = p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf);
+                float bn;
+                const bool root_hit = pv.root_hit(p, pose, r, bn);
                 if constexpr (!AFTER) {       // successor rounds keep the exact inverses: they also prune on the far end
                     r.ix = clamp_inverse(r.ix); r.iy = clamp_inverse(r.iy); r.iz = clamp_inverse(r.iz);
                 }
                 if (root_hit) {
-                    stack[sp++] = make_uint2((uint32_t)p.root, __float_as_uint(bn));
+                    stack[sp++] = make_uint2((uint32_t)pv.root(p, pose), __float_as_uint(bn));
                 } else {
                     retire_ray(p, ray, -1, INFINITY, INFINITY);
                     ray = -1;
@@ -298,7 +330,7 @@ k_traverse_persistent(const TravParams p)
                 uint4 meta = make_uint4(0u, 0u, 0u, 0u);                     // mask, is_brick, base, -
                 if (inner) {
                     const uint2 e = stack[--sp];
-                    const NifNode* nd = nodes + e.x;
+                    const NifNode* nd = pv.nodes(p, pose) + e.x;
                     const float4* f4 = reinterpret_cast<const float4*>(nd);
 #pragma unroll
                     for (int a = 0; a < 3; ++a) {
@@ -366,7 +398,7 @@ k_traverse_persistent(const TravParams p)
         if (ray >= 0 && sp > 0) {
             const uint32_t id = stack[--sp].x & ~LEAF_FLAG;
             float ti, to;
-            if (voxel_hit(p.lat, p.nv, id, r, ti, to) && (!AFTER || after_bound(ti, (int32_t)id, after_t, after_id))) {
+            if (voxel_hit(pv.lat(p, pose), p.nv, id, r, ti, to) && (!AFTER || after_bound(ti, (int32_t)id, after_t, after_id))) {
                 if (ti < best_in || (ti == best_in && (int32_t)id < best_id)) {
                     best_id = (int32_t)id; best_in = ti; best_out = to;
                 }
@@ -385,12 +417,16 @@ k_traverse_persistent(const TravParams p)
 // One thread per ray, static assignment: the right shape for coherent batches (camera rays), where
 // the 32 rays of a warp walk the same nodes and the loads of a node broadcast.  Absent octants are
 // skipped, hit children are insertion-sorted (farthest first).
+template <bool MULTI>
 __global__ void __launch_bounds__(TRAV_BLOCK)
 k_traverse_simple(const TravParams p)
 {
     if (*p.coherent_flag == 0u) return;                   // k_traverse_persistent takes this batch
+    __shared__ NifPoseDesc s_pose[MULTI ? NIF_MAX_POSES : 1];
+    const PoseView<MULTI> pv = stage_poses<MULTI>(p, s_pose);
     const long long ray = (long long)blockIdx.x * TRAV_BLOCK + threadIdx.x;
     if (ray >= p.n) return;
+    const int pose = MULTI ? p.batch.pose_id[ray] : 0;
     Ray r;
     int32_t best_id = -1;
     float best_in = INFINITY, best_out = INFINITY;
@@ -399,25 +435,25 @@ k_traverse_simple(const TravParams p)
     r.ix = __fdiv_rn(1.0f, r.dx); r.iy = __fdiv_rn(1.0f, r.dy); r.iz = __fdiv_rn(1.0f, r.dz);
     uint2 stack[STACK_MAX];
     int sp = 0;
-    float bn, bf;
-    const bool root_hit = p.root >= 0 && slab(p.rlx, p.rly, p.rlz, p.rhx, p.rhy, p.rhz, r, bn, bf);
+    float bn;
+    const bool root_hit = pv.root_hit(p, pose, r, bn);
     r.ix = clamp_inverse(r.ix); r.iy = clamp_inverse(r.iy); r.iz = clamp_inverse(r.iz);
     if (root_hit)
-        stack[sp++] = make_uint2((uint32_t)p.root, __float_as_uint(bn));
+        stack[sp++] = make_uint2((uint32_t)pv.root(p, pose), __float_as_uint(bn));
     while (sp > 0) {
         const uint2 e = stack[--sp];
         if (__uint_as_float(e.y) > best_in) continue;          // strictly later: cannot win a tie either (R12)
         if (e.x & LEAF_FLAG) {
             const uint32_t id = e.x & ~LEAF_FLAG;
             float ti, to;
-            if (voxel_hit(p.lat, p.nv, id, r, ti, to)) {
+            if (voxel_hit(pv.lat(p, pose), p.nv, id, r, ti, to)) {
                 if (ti < best_in || (ti == best_in && (int32_t)id < best_id)) {
                     best_id = (int32_t)id; best_in = ti; best_out = to;
                 }
             }
             continue;
         }
-        const NifNode* nd = p.nodes + e.x;
+        const NifNode* nd = pv.nodes(p, pose) + e.x;
         const float4* f4 = reinterpret_cast<const float4*>(nd);
         float lo[3][8], hi[3][8];
 #pragma unroll
@@ -541,7 +577,8 @@ k_scatter_hits(long long n, int nv, int bin_shift, int nvb, const int32_t* __res
 }  // namespace
 
 int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
-                        const NifQueryWs* ws, unsigned flags, const NifWalkRound* walk, cudaStream_t stream)
+                        const NifQueryWs* ws, unsigned flags, const NifWalkRound* walk, cudaStream_t stream,
+                        const NifPoseBatch* batch)
 {
     if (rays->n == 0) return NIF_OK;
     static int n_sm = 0;
@@ -561,12 +598,13 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
     p.ray_list = walk && walk->round > 0 ? walk->ray_list : nullptr;
     p.n_list = walk ? walk->n_list : nullptr;
     p.walk_dist_accum = walk ? walk->dist_accum : nullptr;
+    p.batch = batch ? *batch : NifPoseBatch{nullptr, nullptr, 0};
     p.coherent_flag = &ws->scratch->pad[0];
     const long long want = (rays->n + TRAV_BLOCK - 1) / TRAV_BLOCK;
     const long long cap = (long long)n_sm * TRAV_BLOCKS_PER_SM;
     if (p.ray_list) {
         // walk rounds >= 1: the live rays are in voxel-bin order, not pixel order -> persistent kernel
-        k_traverse_persistent<true><<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
+        k_traverse_persistent<true, false><<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
         nif_count_launch(1);
         NIF_CUDA_TRY(cudaGetLastError());
         return NIF_OK;
@@ -578,8 +616,13 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
     for (int a = 0; a < 3; ++a) extent = fmaxf(extent, bvh->hi[a] - bvh->lo[a]);
     k_ray_coherence<<<(n_groups * 32 + 255) / 256, 256, 0, stream>>>(
         (long long)rays->n, rays->origin, rays->dir, extent, n_groups, flags, &ws->scratch->pad[1], &ws->scratch->pad[0]);
-    k_traverse_simple<<<(unsigned)want, TRAV_BLOCK, 0, stream>>>(p);
-    k_traverse_persistent<false><<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
+    if (batch) {
+        k_traverse_simple<true><<<(unsigned)want, TRAV_BLOCK, 0, stream>>>(p);
+        k_traverse_persistent<false, true><<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
+    } else {
+        k_traverse_simple<false><<<(unsigned)want, TRAV_BLOCK, 0, stream>>>(p);
+        k_traverse_persistent<false, false><<<(unsigned)(want < cap ? want : cap), TRAV_BLOCK, 0, stream>>>(p);
+    }
     nif_count_launch(3);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;
