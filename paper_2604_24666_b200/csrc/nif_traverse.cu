@@ -417,8 +417,11 @@ k_traverse_persistent(const TravParams p)
 // One thread per ray, static assignment: the right shape for coherent batches (camera rays), where
 // the 32 rays of a warp walk the same nodes and the loads of a node broadcast.  Absent octants are
 // skipped, hit children are insertion-sorted (farthest first).
+#ifndef NIF_TRAV_SIMPLE_MINB
+#define NIF_TRAV_SIMPLE_MINB 6      // 80 registers, 6 blocks per SM: cfg 1 0.186 -> 0.177 ms (8: 0.182, 10: 0.209)
+#endif
 template <bool MULTI>
-__global__ void __launch_bounds__(TRAV_BLOCK)
+__global__ void __launch_bounds__(TRAV_BLOCK, NIF_TRAV_SIMPLE_MINB)
 k_traverse_simple(const TravParams p)
 {
     if (*p.coherent_flag == 0u) return;                   // k_traverse_persistent takes this batch
