@@ -17,9 +17,12 @@
 //               L levels of that sample are interpolated (8 table gathers each, fp32, two batches of
 //               loads in flight) and written as fp16 into the canonical K-major SWIZZLE_128B A chunk
 //               of the stage, 16 bytes per store.
-// Hidden/output weights sit in shared memory for the whole kernel as pre-swizzled B-operand images.
-// The layer-1 accumulator is double-buffered in TMEM so the gathers of tile t+1 overlap the MLP tail
-// of tile t.
+// Hidden/output weight chunks stream through a 2-slot ring (warp 5, second lane) in the order the row
+// warps consume them.  The layer-1 accumulator is double-buffered in TMEM so the gathers of tile t+1
+// overlap the MLP tail of tile t.  Tiles are drawn from a global counter (dynamic scheduling).
+// Template parameters: W, F; CONCAT = concatenation reading of the hybrid encoding (R1; phi items + gamma
+// scalar items); LOCAL = voxel-local trilinear inverse for lattice-supplied deformations (R27).  Variants
+// are separate instantiations: the composition kernel's register allocation is fragile.
 #include "nif_encode.cuh"
 
 #include <type_traits>
