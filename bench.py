@@ -464,7 +464,7 @@ def main() -> None:
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: the headline)")
     ap.add_argument("--params", default="uniform0.1", choices=["uniform0.1", "varpres"])
     ap.add_argument("--engine", default="auto", choices=["auto", "ffma"])
-    ap.add_argument("--chunk", type=int, default=1 << 19, help="rays per staging chunk of nif_query_host")
+    ap.add_argument("--chunk", type=int, default=1 << 20, help="rays per staging chunk of nif_query_host")
     ap.add_argument("--ref-sample", type=int, default=32768, help="rays per step of --impl reference")
     ap.add_argument("--probe-table", action="store_true", help="run the gather probe over the real table")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -378,8 +378,14 @@ extern "C" int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage*
     const bool heads = !(flags & NIF_TRAVERSE_ONLY);
     const bool full = heads && !(flags & NIF_OCCLUSION_ONLY);
     int chunk_idx = 0;
-    for (int64_t begin = 0; begin < rays->n; begin += st->chunk, ++chunk_idx) {
-        const int64_t m = (rays->n - begin < st->chunk) ? rays->n - begin : st->chunk;
+    // the device->host copies (60 B per ray) are the bottleneck of the pipeline, so they should start as
+    // early as possible: the first chunks are short (1/8, 1/4, 1/2 of the slot size), then full ones
+    int64_t m = 0;
+    for (int64_t begin = 0; begin < rays->n; begin += m, ++chunk_idx) {
+        int64_t want = st->chunk;
+        if (chunk_idx < 3 && rays->n > st->chunk) want = st->chunk >> (3 - chunk_idx);
+        if (want < 1) want = 1;
+        m = (rays->n - begin < want) ? rays->n - begin : want;
         const int slot = chunk_idx % NSLOT;
         cudaStream_t stream = st->stream[slot];
         char* d = st->dev[slot];
