@@ -116,10 +116,10 @@ def test_host_buffer_entry_matches_device_entry(H, nif):
 
 
 FULL = [  # cfg, pose, sampled rays for traversal parity, sampled hit rays for network parity
-    (1, 0, 1 << 15, 3000),
-    (2, 5, 1 << 14, 1500),
-    (3, 6, 1 << 14, 1500),
-    (4, 0, 1 << 14, 600),
+    (1, 0, 1 << 15, 6000),
+    (2, 5, 1 << 14, 5000),
+    (3, 6, 1 << 14, 5000),
+    (4, 0, 1 << 14, 3000),
 ]
 
 

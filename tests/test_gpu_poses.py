@@ -120,3 +120,33 @@ def test_query_poses_argument_validation(H, nif):
     single = H.run_gpu(a)
     assert np.array_equal(out["voxel_id"].cpu().numpy(), single["voxel_id"])
     assert np.array_equal(out["dist_total"].cpu().numpy(), single["dist_total"])
+
+
+def test_full_size_config2_batched_equals_per_pose(oracle, H, P, nif):
+    """BASELINE.json configs[2] at full size in the launch configuration bench.py times (one nif_query_poses
+    over 8 x 2^20 rays): bit-identical, ray for ray, to one nif_query per pose; a seeded sample of one pose
+    is recomputed by the oracle."""
+    cfg = I.get_config(2)
+    cases = [H.make_case(2, pose_index=pi, with_net=(pi == 0)) for pi in range(cfg.n_poses)]
+    for c in cases[1:]:
+        c.net = cases[0].net
+    n = cfg.rays_per_pose
+    o = torch.cat([c.origin_d for c in cases]); d = torch.cat([c.direction_d for c in cases])
+    pid = torch.cat([torch.full((n,), k, dtype=torch.int32, device="cuda") for k in range(cfg.n_poses)])
+    out = nif.alloc_outputs(n * cfg.n_poses)
+    nif.nif_query_poses([c.bvh for c in cases], cases[0].net, o, d, pid, out)
+    torch.cuda.synchronize()
+    single = nif.alloc_outputs(n)
+    for k, c in enumerate(cases):
+        nif.nif_query(c.bvh, c.net, c.origin_d, c.direction_d, single)
+        torch.cuda.synchronize()
+        for key in ("voxel_id", "t_in", "t_out", "occlusion", "dist_total", "normal", "material_logits"):
+            assert torch.equal(out[key][k * n:(k + 1) * n], single[key]), (k, key)
+    k = 5
+    rng = np.random.default_rng(2)
+    hit = np.nonzero(out["voxel_id"][k * n:(k + 1) * n].cpu().numpy() >= 0)[0]
+    idx = np.sort(rng.choice(hit, 8000, replace=False))      # the 99.9 % argmax gate needs thousands of hits
+    ref = H.OracleSide(oracle, cases[k]).query(idx)
+    got = {key: v[k * n:(k + 1) * n].cpu().numpy()[idx] for key, v in out.items()}
+    P.assert_traversal(P.compare_traversal(got, ref))
+    P.assert_network(P.compare_network(got, ref, fp16=True), fp16=True)
