@@ -437,8 +437,9 @@ def run_ours(args) -> None:
             "data": "synthetic",
             "config": {"workload": workload_name(cfg), "params": args.params, "rays_per_step_per_gpu": n_total,
                        "hit_rays_per_step_per_gpu": n_hit, "hit_fraction": n_hit / n_total,
-                       "l2": "no flush: per-step working set (rays 24 B + outputs 60 B per ray + 32 MiB table) "
-                             "exceeds the 126 MB L2; the hash table is meant to stay L2-resident",
+                       "l2": f"no flush: per-step working set (rays 24 B + outputs 60 B per ray + {params.table_storage().nbytes >> 20} MiB table) "
+                             "exceeds the 126 MB L2" + ("; the hash table is meant to stay L2-resident between frames"
+                                                         if params.table_storage().nbytes <= (64 << 20) else ""),
                        "poses": ("one nif_query_poses over all poses" if batched else "one nif_query per pose"),
                        "parallelism": f"dp{world} (independent frames per rank, no collective)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
