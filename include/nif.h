@@ -19,6 +19,8 @@
  *     buffers of a nif_stage.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  nif_query only
  *     enqueues work and returns; calls documented as "synchronises" wait for the stream.
+ *     The enqueue-only calls (nif_query, nif_query_multi, nif_query_poses) allocate nothing and
+ *     can be captured in a CUDA graph and replayed (rays and outputs are read/written at replay).
  *   - Return value: NIF_OK (0) or a negative nif_status.  On error no output is written.
  *     No exceptions, no abort(), nothing printed.
  *   - There is no CPU fallback: on a device that is not compute capability 10.x every entry
