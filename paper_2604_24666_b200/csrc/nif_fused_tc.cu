@@ -722,6 +722,9 @@ constexpr uint32_t TC_L1_FRIENDLY_SMEM = 164u * 1024u;    // above this carve-ou
 // ring depth: the deepest that keeps the footprint L1-friendly, else the deepest that fits at all
 int tc_pick_stages(int W)
 {
+    // W = 128 is validated with the 4-stage ring only (200 KB, always available on sm_100); a forced 2- or
+    // 3-stage ring failed at launch in an experiment and was not investigated, so it is never chosen
+    if (W == 128) return tc_smem_layout(TC_MAX_STAGES, W).total <= TC_MAX_SMEM ? TC_MAX_STAGES : 0;
     for (int st = TC_MAX_STAGES; st >= 3; --st)
         if (tc_smem_layout(st, W).total <= TC_L1_FRIENDLY_SMEM) return st;
     for (int st = TC_MAX_STAGES; st >= 2; --st)
