@@ -222,7 +222,8 @@ int nif_query_workspace_bytes(int64_t n, size_t* bytes);
 /* Enqueues the whole hot path on `stream` and returns without synchronising.
  * `workspace`: DEVICE, 256-byte aligned, >= nif_query_workspace_bytes(rays->n); contents are
  * scratch (hit-ray compaction list and counters) and may be reused by the next call on the
- * same stream.  Several poses (B:9) = one nif_bvh and one nif_query per pose sharing one net. */
+ * same stream.  Several poses (B:9) = one nif_bvh per pose sharing one net, and either one nif_query
+ * per pose or one nif_query_poses for all of them. */
 int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
               const nif_query_out* out, void* workspace, size_t workspace_bytes,
               unsigned flags, void* stream);
@@ -275,14 +276,15 @@ int nif_query_multi(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch*
 
 /* -------- end-to-end with HOST buffers ---------------------------------------------------- */
 
-/* Staging for nif_query_host: device buffers for `chunk_rays` rays x 2 (double buffer), three
- * streams.  chunk_rays >= 1. */
+/* Staging for nif_query_host: three slots of device buffers for `chunk_rays` rays each (inputs,
+ * outputs, query workspace), one stream per slot.  chunk_rays >= 1. */
 int nif_stage_create(int64_t chunk_rays, nif_stage** out);
 void nif_stage_destroy(nif_stage* stage);
 
 /* Same query with HOST pointers in `rays` and `out` (pinned memory recommended; pageable
  * works but copies synchronously).  Splits the batch into chunks, overlapping the host->device
- * copy of chunk i+1, the kernels of chunk i and the device->host copy of chunk i-1.
+ * copy of chunk i+1, the kernels of chunk i and the device->host copy of chunk i-1 (the first
+ * chunks are shorter than chunk_rays so that the device->host stream starts early).
  * SYNCHRONISES: on return every output is in host memory. */
 int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
                    const nif_ray_batch* rays_host, const nif_query_out* out_host, unsigned flags);
@@ -301,7 +303,7 @@ int nif_query_last_hit_count(const void* workspace, void* stream, int64_t* n_hit
 int nif_profile_enable(int on);
 int nif_profile_read(double* traverse_ms, double* network_ms, int64_t* n_queries);
 
-/* Random-sector gather probe: the denominator of the gather roofline (DESIGN.md section 9).
+/* Random-sector gather probe: the denominator of the gather roofline (DESIGN.md section 8).
  * All SMs issue independent 4-byte loads at pseudo-random 32-byte sectors of the DEVICE buffer
  * `buf` (`bytes` rounded down to a power-of-two number of sectors); `iters` batches of 8 loads
  * per thread, 512-thread blocks.  `smem_bytes` of (untouched) dynamic shared memory per block
