@@ -717,19 +717,14 @@ TcShape tc_shape(const nif_net_desc* d)
 }
 
 constexpr uint32_t TC_MAX_SMEM = 227u * 1024u;
-constexpr uint32_t TC_L1_FRIENDLY_SMEM = 164u * 1024u;    // above this carve-out the L1 is too small for the gathers
 
-// ring depth: the deepest that keeps the footprint L1-friendly, else the deepest that fits at all
+// ring depth: always the full 4-stage ring (W = 32 / 64: 118 / 139 KB, inside the L1-friendly 164 KB carve-out of
+// DESIGN.md 7.3; W = 128: 200 KB).  Shallower rings were measured slower (7.7) and a forced 3-stage ring at
+// W = 128 failed at launch on full-size config 4 in an experiment that was not investigated further, so no other
+// depth is ever selected; a device without enough shared memory gets the FFMA engine instead.
 int tc_pick_stages(int W)
 {
-    // W = 128 is validated with the 4-stage ring only (200 KB, always available on sm_100); a forced 2- or
-    // 3-stage ring failed at launch in an experiment and was not investigated, so it is never chosen
-    if (W == 128) return tc_smem_layout(TC_MAX_STAGES, W).total <= TC_MAX_SMEM ? TC_MAX_STAGES : 0;
-    for (int st = TC_MAX_STAGES; st >= 3; --st)
-        if (tc_smem_layout(st, W).total <= TC_L1_FRIENDLY_SMEM) return st;
-    for (int st = TC_MAX_STAGES; st >= 2; --st)
-        if (tc_smem_layout(st, W).total <= TC_MAX_SMEM) return st;
-    return 0;
+    return tc_smem_layout(TC_MAX_STAGES, W).total <= TC_MAX_SMEM ? TC_MAX_STAGES : 0;
 }
 
 template <int W, int F, bool CONCAT, bool LOCAL>
