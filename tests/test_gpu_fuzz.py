@@ -63,3 +63,45 @@ def test_random_scenes_bit_exact(oracle, seed):
             assert np.array_equal(g["t_out"][hit].view(np.int32), to[hit].view(np.int32)), (it, kind, fl)
         done += 1
     assert done >= 30
+
+
+def test_random_scenes_walk_successor_sequence(oracle):
+    """The successor traversal of nif_query_multi on random grids and poses: with a network that never accepts,
+    the number of voxels walked and the last voxel equal the oracle's successor chain."""
+    import harness as H
+    import paper_2604_24666_b200 as nif
+    import test_gpu_walk as W
+    rng = np.random.default_rng(3)
+    done = 0
+    for it in range(24):
+        nv = int(rng.choice([3, 4, 6, 8, 12, 16]))
+        occ = (rng.random(nv ** 3) < rng.uniform(0.2, 1.0)).astype(np.uint8)
+        if not occ.any():
+            occ[0] = 1
+        theta = float(rng.uniform(-2.0, 2.0)); k = float(rng.uniform(-0.8, 0.8))
+        cfg = I.scaled(I.get_config(0), nv=nv)
+        try:
+            case = H.make_case(0, cfg=cfg, occ=occ, pose=[theta, k], n_rays=1200)
+        except nif.NifError as e:
+            assert e.status == -3
+            continue
+        case = W._net_with(H, case, "never_accept")
+        K = int(rng.choice([3, 8, 30]))
+        gpu = W.run_walk(nif, case, K)
+        lat = oracle.deform_lattice(nv, theta, k); bvh = oracle.bvh_build(nv, occ, lat)
+        o, d = case.origin, case.direction
+        n = len(o)
+        at = np.full(n, -np.inf, np.float32); ai = np.full(n, -1, np.int32)
+        count = np.zeros(n, np.int32); last = np.full(n, -1, np.int32)
+        for _ in range(K):
+            v, ti, _ = bvh.next_voxel(o, d, at, ai)
+            live = v >= 0
+            if not live.any():
+                break
+            count += live; last = np.where(live, v, last)
+            at = np.where(live, ti, at); ai = np.where(live, v, ai)
+        capped = count >= K
+        assert np.array_equal(gpu["steps"], count), (it, nv, theta, k, K)
+        assert np.array_equal(gpu["voxel_id"][capped], last[capped]) and (gpu["voxel_id"][~capped] == -1).all()
+        done += 1
+    assert done >= 16
