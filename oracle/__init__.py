@@ -21,6 +21,7 @@ _CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared", 
 FLAG_OCCLUSION_ONLY = 1
 FLAG_DIST_LOG = 2
 FLAG_LATTICE_INVERSE = 4
+FLAG_ACT_F16 = 8
 N_OUT = 12
 
 
@@ -31,7 +32,7 @@ def build(force: bool = False) -> dict:
         so = _HERE / name
         if force or not so.exists() or so.stat().st_mtime < _SRC.stat().st_mtime:
             tmp = so.with_suffix(f".tmp{os.getpid()}.so")
-            subprocess.check_call(["gcc", *_CFLAGS, *extra, str(_SRC), "-o", str(tmp), "-lm"])
+            subprocess.check_call(["gcc", *_CFLAGS, *extra, str(_SRC), "-o", str(tmp), "-lquadmath", "-lm"])
             os.replace(tmp, so)
         out[name] = so
     return out
@@ -67,6 +68,8 @@ class Oracle:
         L.nifo_traverse_brute.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 5
         L.nifo_forward_f64.argtypes = [C.c_double, C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
         L.nifo_deform_lattice.argtypes = [C.c_int, C.c_float, C.c_float, C.c_void_p]
+        L.nifo_deform_lattice_counted.argtypes = [C.c_int, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
+        L.nifo_forward_exact_f32.argtypes = [C.c_float, C.c_float, C.c_int64, C.c_void_p, C.c_void_p]
         L.nifo_inverse_f32.argtypes = [C.c_float, C.c_float, C.c_int64, C.c_void_p, C.c_void_p]
         L.nifo_voxel_hit.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p]
@@ -75,6 +78,7 @@ class Oracle:
         L.nifo_encode.argtypes = [C.POINTER(_NetDesc), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         L.nifo_mlp.argtypes = [C.POINTER(_NetDesc), C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_void_p]
         L.nifo_decode.argtypes = [C.c_int64] + [C.c_void_p] * 9
+        L.nifo_round_f16.argtypes = [C.c_int64, C.c_void_p, C.c_void_p]
         L.nifo_query.restype = C.c_int
         L.nifo_query.argtypes = ([C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float,
                                   C.POINTER(_NetDesc), C.c_void_p, C.c_void_p, C.c_int64,
@@ -101,9 +105,18 @@ class Oracle:
         self.lib.nifo_forward_f64(float(theta_max), float(k), len(p), p.ctypes.data, out.ctypes.data)
         return out
 
-    def deform_lattice(self, nv, theta_max, k):
+    def deform_lattice(self, nv, theta_max, k, count_exact=False):
+        """O2x: correctly rounded fp32 lattice (fp64 evaluation, binary128 where the rounding is in doubt)."""
         out = np.empty(((nv + 1) ** 3, 3), dtype=np.float32)
-        self.lib.nifo_deform_lattice(int(nv), float(theta_max), float(k), out.ctypes.data)
+        cnt = C.c_int64(0)
+        self.lib.nifo_deform_lattice_counted(int(nv), float(theta_max), float(k), out.ctypes.data, C.byref(cnt))
+        return (out, cnt.value) if count_exact else out
+
+    def forward_exact_f32(self, theta_max, k, p):
+        """O2x definition: binary128 evaluation of the closed form, rounded once to fp32."""
+        p = np.ascontiguousarray(p, dtype=np.float64).reshape(-1, 3)
+        out = np.empty(p.shape, dtype=np.float32)
+        self.lib.nifo_forward_exact_f32(float(theta_max), float(k), len(p), p.ctypes.data, out.ctypes.data)
         return out
 
     def inverse_trilinear(self, lattice, nv, voxel_id, P):
@@ -184,6 +197,13 @@ class Oracle:
         self.lib.nifo_mlp(C.byref(d), arr, x.shape[1], len(x), x.ctypes.data, out.ctypes.data)
         return out
 
+    def round_f16(self, x):
+        """O9b: IEEE binary16 round-to-nearest-even of each value, as float32"""
+        x = _f32(x)
+        out = np.empty_like(x)
+        self.lib.nifo_round_f16(x.size, x.ctypes.data, out.ctypes.data)
+        return out
+
     def decode(self, logits, t_in, t_out):
         logits = _f32(logits); t_in = _f32(t_in); t_out = _f32(t_out)
         n = len(logits)
@@ -206,8 +226,8 @@ class Oracle:
 
     def query(self, nv, occ, lattice, bvh, pose, params, origin, direction,
               occlusion_only=False, traverse_only=False, dist_log=False, hit_positions=False,
-              lattice_inverse=False):
-        """Whole pipeline.  bvh=None -> brute-force definition."""
+              lattice_inverse=False, act_f16=False):
+        """Whole pipeline.  bvh=None -> brute-force definition.  act_f16: O9b (fp16 activations, B:8)."""
         origin = _f32(origin); direction = _f32(direction)
         n = len(origin)
         sh = params.shape
@@ -228,7 +248,7 @@ class Oracle:
                                  float(pose[0]), float(pose[1]), C.byref(d), table.ctypes.data, arr,
                                  n, origin.ctypes.data, direction.ctypes.data,
                                  (FLAG_OCCLUSION_ONLY if occlusion_only else 0) | (FLAG_DIST_LOG if dist_log else 0) |
-                                 (FLAG_LATTICE_INVERSE if lattice_inverse else 0),
+                                 (FLAG_LATTICE_INVERSE if lattice_inverse else 0) | (FLAG_ACT_F16 if act_f16 else 0),
                                  g("voxel_id"), g("t_in"), g("t_out"), g("occlusion"), g("distance"),
                                  g("dist_total"), g("normal"), g("albedo"), g("material_logits"),
                                  g("raw_logits"))

@@ -21,11 +21,14 @@
  * Parity pins (tests/test_oracle_*.py, -m "not gpu"):
  *   O2/O7 deformation    : printed values (tests/golden/deform_worked.txt), identity pose,
  *                          inverse(forward(x)) = x
+ *   O2x exact lattice    : binary128 evaluation == mpmath at 60 digits rounded to fp32; the fp64
+ *                          fast path + fallback == the binary128 evaluation on every lattice point
  *   O4/O5 voxel hit      : slab closed form on the identity pose, reversed-ray invariant
  *   O6 nearest voxel     : BVH == brute force, bit-exact
  *   O8 encode            : hand-computed toy table (tests/golden/hash_toy.txt), constant and
  *                          affine tables, torch grid_sample on dense levels, numpy sin/cos
  *   O9 MLP               : torch fp64 linear+relu chain
+ *   O9b fp16 activations : round_f16 == numpy float16 conversion; numpy float16 chain
  *   O10 decode           : closed forms / invariants
  *   end-to-end accuracy against a trained model: PARITY UNPINNED (no weights/objects exist).
  */
@@ -50,6 +53,7 @@ typedef float acc_t;
 #define NIFO_FLAG_OCCLUSION_ONLY 1u
 #define NIFO_FLAG_LATTICE_INVERSE 4u /* O7b: voxel-local trilinear inverse from the lattice instead of the closed form */
 #define NIFO_FLAG_DIST_LOG 2u       /* O10b: ReLU + log-transformed distance head (R24) */
+#define NIFO_FLAG_ACT_F16 8u        /* O9b: MLP input features and hidden activations rounded to fp16 (B:8) */
 
 int nifo_acc_bytes(void) { return (int)sizeof(acc_t); }
 
@@ -85,11 +89,76 @@ void nifo_forward_f64(double theta_max, double k, int64_t n, const double* p, do
     for (int64_t i = 0; i < n; ++i) forward_f64(theta_max, k, p + 3 * i, out + 3 * i);
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* O2x  The deformed lattice is the CORRECTLY ROUNDED fp32 value of the real-valued closed    */
+/* form (R7, R28): inputs are the fp64 rest coordinate (2i-nv)/nv (one fp64          */
+/* division, exact for power-of-two nv) and the pose parameters theta_max, k (fp32, exact in   */
+/* fp64); the formula of forward_f64 is then a real function of those, and the lattice entry    */
+/* is RN_fp32 of its value.  Hit ids must be bit-exact between two implementations            */
+/* (BASELINE.json:5), and a lattice entry that differs in its last bit can move a grazing ray    */
+/* to another voxel, so "each side's fp64 libm, rounded once" (round 1) is not a definition:    */
+/* two libms differ in the last fp64 bit about once in 1e7 values and that flips an fp32         */
+/* rounding.  The definition written out: forward_q evaluates the same formula in binary128      */
+/* (__float128, libquadmath sinq/cosq: 113-bit significand, error < 2^-100 here) and rounds      */
+/* ONCE to fp32.  nifo_deform_lattice reaches the same result faster: it evaluates in fp64,      */
+/* whose absolute error is far below NIFO_LATTICE_E for coordinates of magnitude < 8, and falls  */
+/* back to forward_q only where the fp64 value lies within NIFO_LATTICE_E of a midpoint between  */
+/* two adjacent fp32 numbers (where the fp64 error could change the rounding).  Pin:              */
+/* tests/test_oracle_lattice.py compares it bit for bit with forward_q on every point, and        */
+/* forward_q with mpmath at 60 digits.                                                            */
+/* ------------------------------------------------------------------------------------ */
+#include <quadmath.h>
+
+static void forward_q(float theta_max_f, float k_f, const double p[3], __float128 out[3])
+{
+    __float128 theta_max = (__float128)theta_max_f, k = (__float128)k_f;
+    __float128 x = (__float128)p[0], y = (__float128)p[1], z = (__float128)p[2];
+    __float128 one = (__float128)1.0, two = (__float128)2.0;
+    __float128 a = theta_max * (y + one) / two;
+    __float128 ca = cosq(a), sa = sinq(a);
+    __float128 tx = x * ca + z * sa;
+    __float128 ty = y;
+    __float128 tz = -x * sa + z * ca;
+    if (fabs((double)k_f) < 1e-6) {
+        out[0] = tx; out[1] = ty; out[2] = tz;
+    } else {
+        __float128 al = k * tx;
+        __float128 sh = sinq(al / two);
+        out[0] = (one - k * ty) * sinq(al) / k;
+        out[1] = ty * cosq(al) + two * sh * sh / k;
+        out[2] = tz;
+    }
+}
+
+/* exposed for pins: the definition, n points -> n x 3 floats (binary128 evaluation, one rounding) */
+void nifo_forward_exact_f32(float theta_max, float k, int64_t n, const double* p, float* out)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        __float128 q[3];
+        forward_q(theta_max, k, p + 3 * i, q);
+        for (int a = 0; a < 3; ++a) out[3 * i + a] = (float)q[a];
+    }
+}
+
+#define NIFO_LATTICE_E 9.094947017729282e-13      /* 2^-40: >= 1000 fp64 ulps of any |coordinate| < 8 */
+
+/* 1 if rounding the fp64 value v (absolute error <= NIFO_LATTICE_E) to fp32 could go either way */
+static int rounding_ambiguous(double v)
+{
+    float f = (float)v;
+    if (!isfinite(f)) return 1;
+    double lo = 0.5 * ((double)f + (double)nextafterf(f, -INFINITY));   /* midpoints to both neighbours: exact in fp64 */
+    double hi = 0.5 * ((double)f + (double)nextafterf(f, INFINITY));
+    return fabs(v - lo) <= NIFO_LATTICE_E || fabs(v - hi) <= NIFO_LATTICE_E;
+}
+
 /* lattice point (i,j,k), 0<=i,j,k<=nv, rest position ((2i-nv)/nv, ...) evaluated in fp64 (O1).
-   Output index (i + (nv+1)(j + (nv+1)k))*3. */
-void nifo_deform_lattice(int nv, float theta_max, float bend_k, float* lattice)
+   Output index (i + (nv+1)(j + (nv+1)k))*3.  Returns through *n_exact (optional) how many points
+   needed the binary128 evaluation. */
+void nifo_deform_lattice_counted(int nv, float theta_max, float bend_k, float* lattice, int64_t* n_exact)
 {
     int np1 = nv + 1;
+    int64_t cnt = 0;
     for (int k = 0; k <= nv; ++k)
         for (int j = 0; j <= nv; ++j)
             for (int i = 0; i <= nv; ++i) {
@@ -99,8 +168,21 @@ void nifo_deform_lattice(int nv, float theta_max, float bend_k, float* lattice)
                 p[2] = (2.0 * k - nv) / nv;
                 forward_f64((double)theta_max, (double)bend_k, p, q);
                 float* o = lattice + 3 * ((size_t)i + (size_t)np1 * ((size_t)j + (size_t)np1 * k));
-                o[0] = (float)q[0]; o[1] = (float)q[1]; o[2] = (float)q[2];
+                if (rounding_ambiguous(q[0]) || rounding_ambiguous(q[1]) || rounding_ambiguous(q[2])) {
+                    __float128 e[3];
+                    forward_q(theta_max, bend_k, p, e);
+                    o[0] = (float)e[0]; o[1] = (float)e[1]; o[2] = (float)e[2];
+                    ++cnt;
+                } else {
+                    o[0] = (float)q[0]; o[1] = (float)q[1]; o[2] = (float)q[2];
+                }
             }
+    if (n_exact) *n_exact = cnt;
+}
+
+void nifo_deform_lattice(int nv, float theta_max, float bend_k, float* lattice)
+{
+    nifo_deform_lattice_counted(nv, theta_max, bend_k, lattice, 0);
 }
 
 /* ------------------------------------------------------------------------------------ */
@@ -695,8 +777,34 @@ void nifo_encode(const nifo_net_desc* nd, const float* table, int64_t n, const f
 /* perceptron").  a0 = input; a_i = ReLU(W_i a_{i-1}), i=1..H; z = W_{H+1} a_H.  No biases, */
 /* linear output (R16).  weights[i]: row-major (fan_out, fan_in).                          */
 /* ------------------------------------------------------------------------------------ */
+/* O9b  BASELINE.json config 1 (B:8) fixes the precision of the fp16 networks: "fp16 weights and
+   activations, fp32 accumulate".  round_f16 is IEEE binary16 round-to-nearest-even of one value
+   (11-bit significand: quantum 2^(e-10) in the binade 2^e, fixed quantum 2^-24 below 2^-14,
+   overflow above 65504 to infinity), returned as a float.  With act_f16 the MLP input features and
+   every hidden activation (after ReLU) are rounded that way; products and sums stay in acc_t.  The
+   default (act_f16 = 0) keeps activations in acc_t: the "fp32 oracle" of the north star.  The
+   rounded mode exists because an argmax is an integer decided by floating point, and such a decision
+   is to be taken in the same precision on both sides (the material argmax gate of DESIGN.md 3).
+   Pin: tests/test_oracle_network.py compares round_f16 with numpy's float16 conversion. */
+static float round_f16(float v)
+{
+    if (!(fabsf(v) < INFINITY) || v == 0.0f) return v;      /* inf, NaN, +-0 */
+    int e;
+    (void)frexpf(v, &e);                                    /* |v| = m 2^e, m in [0.5, 1) */
+    int q = e - 11;                                         /* quantum exponent */
+    if (q < -24) q = -24;
+    float r = ldexpf(nearbyintf(ldexpf(v, -q)), q);         /* default rounding mode: ties to even */
+    if (fabsf(r) > 65504.0f) r = copysignf(INFINITY, v);
+    return r;
+}
+
+void nifo_round_f16(int64_t n, const float* in, float* out)
+{
+    for (int64_t i = 0; i < n; ++i) out[i] = round_f16(in[i]);
+}
+
 static void mlp_forward(const nifo_net_desc* nd, const float* const* weights, int d_in,
-                        const acc_t* input, int n_out, acc_t* z, acc_t* buf0, acc_t* buf1)
+                        const acc_t* input, int n_out, acc_t* z, acc_t* buf0, acc_t* buf1, int act_f16)
 {
     const acc_t* cur = input; int cur_n = d_in;
     acc_t* bufs[2] = { buf0, buf1 };
@@ -707,6 +815,7 @@ static void mlp_forward(const nifo_net_desc* nd, const float* const* weights, in
             acc_t acc = 0;
             for (int k = 0; k < cur_n; ++k) acc += (acc_t)W[(size_t)o * cur_n + k] * cur[k];
             nxt[o] = acc > 0 ? acc : 0;
+            if (act_f16) nxt[o] = (acc_t)round_f16((float)nxt[o]);
         }
         cur = nxt; cur_n = nd->width;
     }
@@ -728,7 +837,7 @@ void nifo_mlp(const nifo_net_desc* nd, const float* const* weights, int d_in, in
     for (int64_t i = 0; i < n; ++i) {
         acc_t z[NIFO_N_OUT];
         for (int j = 0; j < d_in; ++j) in[j] = (acc_t)input[(size_t)i * d_in + j];
-        mlp_forward(nd, weights, d_in, in, NIFO_N_OUT, z, b0, b1);
+        mlp_forward(nd, weights, d_in, in, NIFO_N_OUT, z, b0, b1, 0);
         for (int j = 0; j < NIFO_N_OUT; ++j) logits[(size_t)i * NIFO_N_OUT + j] = (float)z[j];
     }
     free(in); free(b0); free(b1);
@@ -803,7 +912,9 @@ static void nifo_eval_voxel(const float* lattice, int nv, float theta_max, float
     acc_t z[NIFO_N_OUT];
     float zf[NIFO_N_OUT];
     for (int j = 0; j < NIFO_N_OUT; ++j) z[j] = 0;
-    mlp_forward(nd, weights, d_in, in, n_out, z, b0, b1);
+    if (flags & NIFO_FLAG_ACT_F16)
+        for (int j = 0; j < d_in; ++j) in[j] = (acc_t)round_f16((float)in[j]);
+    mlp_forward(nd, weights, d_in, in, n_out, z, b0, b1, (flags & NIFO_FLAG_ACT_F16) != 0);
     for (int j = 0; j < NIFO_N_OUT; ++j) zf[j] = (float)z[j];
     if (raw_logits) for (int j = 0; j < NIFO_N_OUT; ++j) raw_logits[j] = zf[j];
     if (flags & NIFO_FLAG_OCCLUSION_ONLY) {

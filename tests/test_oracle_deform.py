@@ -115,3 +115,57 @@ def test_lattice_is_forward_of_rest_lattice_rounded_once(oracle):
     # the float pose parameters are widened exactly to double
     want = oracle.forward_f64(np.float32(th), np.float32(k), rest).astype(np.float32)
     assert np.array_equal(lat, want)
+
+
+# ---- O2x: the lattice is the CORRECTLY ROUNDED fp32 value of the closed form (R28) ----
+def _mp_round_f32(v):
+    """nearest float32 to the mpmath number v, decided in mpmath arithmetic (no double rounding)"""
+    import mpmath as mp
+    f = np.float32(float(v))
+    cands = [f, np.nextafter(f, np.float32(-np.inf)), np.nextafter(f, np.float32(np.inf))]
+    return min(cands, key=lambda c: abs(mp.mpf(float(c)) - v))
+
+
+def _mp_forward(th, k, p):
+    """the closed form of B:7/B:8 (twist about +y, circular-arc bend about z) at 60 digits, in the
+    textbook arc form X = (1/k - y) sin(kx), Y = 1/k - (1/k - y) cos(kx) -- not the oracle's
+    cancellation-free rearrangement"""
+    import mpmath as mp
+    mp.mp.dps = 60
+    th, k = mp.mpf(float(np.float32(th))), mp.mpf(float(np.float32(k)))
+    x, y, z = (mp.mpf(float(c)) for c in p)
+    a = th * (y + 1) / 2
+    tx, ty, tz = x * mp.cos(a) + z * mp.sin(a), y, -x * mp.sin(a) + z * mp.cos(a)
+    if abs(k) < mp.mpf("1e-6"):
+        return tx, ty, tz
+    R = 1 / k
+    return (R - ty) * mp.sin(k * tx), R - (R - ty) * mp.cos(k * tx), tz
+
+
+@pytest.mark.parametrize("pose", POSES)
+def test_exact_forward_is_the_correctly_rounded_closed_form(oracle, pose):
+    th, k = pose
+    p = _points(300, k, 5)
+    got = oracle.forward_exact_f32(th, k, p)
+    for i in range(len(p)):
+        want = [_mp_round_f32(v) for v in _mp_forward(th, k, p[i])]
+        assert [float(g) for g in got[i]] == [float(w) for w in want], (i, p[i])
+
+
+@pytest.mark.parametrize("nv,pose", [(16, (1.0, 0.0)), (12, (0.7, 0.5)), (32, (math.pi, 1.2)), (24, (1.3, 0.02755911))])
+def test_lattice_equals_exact_forward_on_every_point(oracle, nv, pose):
+    # the fp64 fast path with its binary128 fallback must give the definition's bits everywhere
+    lat, n_exact = oracle.deform_lattice(nv, *pose, count_exact=True)
+    g = (2.0 * np.arange(nv + 1) - nv) / nv
+    z, y, x = np.meshgrid(g, g, g, indexing="ij")
+    p = np.stack([x.ravel(), y.ravel(), z.ravel()], axis=1)
+    want = oracle.forward_exact_f32(pose[0], pose[1], p)
+    assert np.array_equal(lat.view(np.int32), want.view(np.int32))
+    assert n_exact < 0.15 * len(p)            # the fallback is the exception (exact zeros such as the y = 0 plane, near-midpoint values)
+
+
+def test_fp64_rounding_alone_is_not_the_definition(oracle):
+    # why O2x exists: plain fp64 evaluation rounded to fp32 differs from the correctly rounded value on a
+    # few entries of a large lattice, or at least needs the fallback there
+    lat, n_exact = oracle.deform_lattice(64, 0.0, 0.8, count_exact=True)
+    assert n_exact > 0

@@ -123,3 +123,44 @@ def test_fp32_oracle_is_within_1e5_of_fp64_accumulation(oracle, oracle64):
         assert np.abs(a["raw_logits"] - b["raw_logits"]).max() <= 1e-5 * zr
         for k in ("occlusion", "albedo", "normal"):
             assert np.abs(a[k] - b[k]).max() <= 1e-5, k
+
+
+# ---- O9b: fp16 activations (B:8 "fp16 weights and activations, fp32 accumulate") -------------------
+def test_round_f16_equals_numpy_float16_conversion(oracle):
+    rng = np.random.default_rng(9)
+    x = np.concatenate([
+        rng.standard_normal(200_000).astype(np.float32) * 10.0 ** rng.uniform(-9, 5, 200_000).astype(np.float32),
+        np.array([0.0, -0.0, 1.0, -1.0, 65504.0, 65519.99, 65520.0, 70000.0, -65520.0, 2.0 ** -14, 2.0 ** -24,
+                  2.0 ** -25, 1.5 * 2.0 ** -25, 2.0 ** -26, np.inf, -np.inf, 1.0 + 2.0 ** -11, 1.0 + 3 * 2.0 ** -11,
+                  1.0 + 2.0 ** -11 + 2.0 ** -20, 2049.0, 2051.0], np.float32),
+        np.arange(0, 70000, 0.37, dtype=np.float32) * 2.0 ** -20])       # ties and subnormal halves
+    with np.errstate(over="ignore"):
+        want = x.astype(np.float16).astype(np.float32)
+    got = oracle.round_f16(x)
+    assert np.array_equal(got.view(np.int32), want.view(np.int32))
+
+
+def test_act_f16_mode_rounds_where_the_precision_contract_says(oracle):
+    # the rounded mode equals the plain MLP applied to an fp16-rounded input with every hidden activation
+    # rounded: checked through a numpy float16 chain with fp64 accumulation (sums differ at 1e-6, not 1e-3)
+    cfg, occ, pose, lat, bvh, o, d, P = _setup(oracle, 1, 400, "varpres")
+    a = oracle.query(cfg.nv, occ, lat, bvh, pose, P, o, d)
+    b = oracle.query(cfg.nv, occ, lat, bvh, pose, P, o, d, act_f16=True)
+    hit = a["voxel_id"] >= 0
+    assert hit.sum() > 30
+    assert np.array_equal(a["voxel_id"], b["voxel_id"]) and np.array_equal(a["t_in"], b["t_in"])
+    rest = oracle.rest_endpoints(float(pose[0]), float(pose[1]), o[hit], d[hit], a["voxel_id"][hit], a["t_in"][hit], a["t_out"][hit])
+    xn = np.clip((rest + 1.0) * 0.5, 0.0, 1.0).astype(np.float32)
+    feats = np.concatenate([oracle.encode(P, xn[:, 0]), oracle.encode(P, xn[:, 1])], axis=1)
+    act = feats.astype(np.float16).astype(np.float64)
+    for w in P.weights[:-1]:
+        act = np.maximum(act @ w.astype(np.float64).T, 0.0).astype(np.float16).astype(np.float64)
+    z = act @ P.weights[-1].astype(np.float64).T
+    rms = np.sqrt((z ** 2).mean())
+    # fp32 vs fp64 sums differ by ~1e-7: almost every logit agrees to 1e-5 rms; where a sum sits on an fp16
+    # rounding boundary one hidden activation moves by one fp16 ulp, a logit error of ~1e-3 rms at most
+    err = np.abs(b["raw_logits"][hit] - z) / rms
+    assert np.median(err) <= 1e-6 and (err > 1e-5).mean() < 0.05 and err.max() <= 3e-3, (np.median(err), (err > 1e-5).mean(), err.max())
+    # and the two modes differ by fp16 noise: well above fp32 rounding, well inside the logit gate
+    diff = np.abs(a["raw_logits"][hit] - b["raw_logits"][hit]).max() / rms
+    assert 1e-5 < diff < 5e-3, diff
