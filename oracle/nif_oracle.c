@@ -100,7 +100,7 @@ void nifo_forward_f64(double theta_max, double k, int64_t n, const double* p, do
 /* two libms differ in the last fp64 bit about once in 1e7 values and that flips an fp32         */
 /* rounding.  The definition written out: forward_q evaluates the same formula in binary128      */
 /* (__float128, libquadmath sinq/cosq: 113-bit significand, error < 2^-100 here) and rounds      */
-/* ONCE to fp32.  nifo_deform_lattice reaches the same result faster: it evaluates in fp64,      */
+/* ONCE to fp32 (a zero result is stored as +0).  nifo_deform_lattice reaches the same result faster: it evaluates in fp64,      */
 /* whose absolute error is far below NIFO_LATTICE_E for coordinates of magnitude < 8, and falls  */
 /* back to forward_q only where the fp64 value lies within NIFO_LATTICE_E of a midpoint between  */
 /* two adjacent fp32 numbers (where the fp64 error could change the rounding).  Pin:              */
@@ -136,7 +136,10 @@ void nifo_forward_exact_f32(float theta_max, float k, int64_t n, const double* p
     for (int64_t i = 0; i < n; ++i) {
         __float128 q[3];
         forward_q(theta_max, k, p + 3 * i, q);
-        for (int a = 0; a < 3; ++a) out[3 * i + a] = (float)q[a];
+        for (int a = 0; a < 3; ++a) {
+            out[3 * i + a] = (float)q[a];
+            if (out[3 * i + a] == 0.0f) out[3 * i + a] = 0.0f;   /* +0, never -0 (R28) */
+        }
     }
 }
 
@@ -176,6 +179,8 @@ void nifo_deform_lattice_counted(int nv, float theta_max, float bend_k, float* l
                 } else {
                     o[0] = (float)q[0]; o[1] = (float)q[1]; o[2] = (float)q[2];
                 }
+                for (int a = 0; a < 3; ++a)
+                    if (o[a] == 0.0f) o[a] = 0.0f;           /* a zero coordinate is stored as +0 (R28) */
             }
     if (n_exact) *n_exact = cnt;
 }

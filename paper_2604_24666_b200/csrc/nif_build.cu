@@ -32,11 +32,130 @@ __host__ __device__ inline uint32_t compact3(uint32_t x)
     return x;
 }
 
-// ---- O1/O2: rest lattice -> deformed lattice, fp64, one rounding to fp32 (R7) -------
-// Explicit _rn intrinsics: no fma contraction, so the operation sequence is the one DESIGN.md
-// states (twist about +y by theta_max (y+1)/2, then circular-arc bend about z).
-__global__ void k_deform_lattice(int nv, double theta_max, double k, float4* __restrict__ lat)
+// ---- O1/O2: rest lattice -> deformed lattice (R7, R28) ---------------------------------
+// The lattice entry is the CORRECTLY ROUNDED fp32 value of the closed form (twist about +y by
+// theta_max (y+1)/2, then circular-arc bend about z), a real function of the fp64 rest coordinate
+// (2i-nv)/nv and the fp32 pose parameters: hit ids must be bit-exact against an independent
+// implementation (B:5), and a last-bit difference of a corner can move a grazing ray to another voxel.
+// Fast path: fp64 with CUDA's sincos (absolute error far below LATTICE_E for |coordinate| < 8), rounded
+// once.  Where that value lies within LATTICE_E of the midpoint of two adjacent fp32 numbers -- where the
+// fp64 error could change the rounding; exact zeros included -- the point is re-evaluated in
+// double-double arithmetic (~105 bits: error-free sums and fma products, Taylor series for sin/cos after
+// a three-word pi/2 reduction) and rounded from the (hi, lo) pair without double rounding.
+struct dd { double hi, lo; };
+
+__device__ __forceinline__ dd dd_quick(double a, double b)       // |a| >= |b| or a == 0
 {
+    const double s = __dadd_rn(a, b);
+    return dd{s, __dsub_rn(b, __dsub_rn(s, a))};
+}
+__device__ __forceinline__ dd dd_two_sum(double a, double b)
+{
+    const double s = __dadd_rn(a, b), bb = __dsub_rn(s, a);
+    return dd{s, __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb))};
+}
+__device__ __forceinline__ dd dd_two_prod(double a, double b)
+{
+    const double p = __dmul_rn(a, b);
+    return dd{p, __fma_rn(a, b, -p)};
+}
+__device__ __forceinline__ dd dd_from(double a) { return dd{a, 0.0}; }
+__device__ __forceinline__ dd dd_neg(dd a) { return dd{-a.hi, -a.lo}; }
+__device__ __forceinline__ dd dd_add(dd a, dd b)
+{
+    dd s = dd_two_sum(a.hi, b.hi);
+    const dd t = dd_two_sum(a.lo, b.lo);
+    s = dd_quick(s.hi, __dadd_rn(s.lo, t.hi));
+    return dd_quick(s.hi, __dadd_rn(s.lo, t.lo));
+}
+__device__ __forceinline__ dd dd_sub(dd a, dd b) { return dd_add(a, dd_neg(b)); }
+__device__ __forceinline__ dd dd_mul(dd a, dd b)
+{
+    if (a.hi == 0.0 || b.hi == 0.0) return dd{__dmul_rn(a.hi, b.hi), 0.0};       // keeps exact (signed) zeros
+    const dd p = dd_two_prod(a.hi, b.hi);
+    return dd_quick(p.hi, __dadd_rn(p.lo, __dadd_rn(__dmul_rn(a.hi, b.lo), __dmul_rn(a.lo, b.hi))));
+}
+__device__ __forceinline__ dd dd_div(dd a, dd b)
+{
+    if (a.hi == 0.0) return dd{__ddiv_rn(a.hi, b.hi), 0.0};
+    const double q1 = __ddiv_rn(a.hi, b.hi);
+    dd r = dd_sub(a, dd_mul(dd_from(q1), b));
+    const double q2 = __ddiv_rn(r.hi, b.hi);
+    r = dd_sub(r, dd_mul(dd_from(q2), b));
+    const double q3 = __ddiv_rn(r.hi, b.hi);
+    return dd_add(dd_quick(q1, q2), dd_from(q3));
+}
+// sin and cos of a double-double argument (|a| up to a few hundred)
+__device__ void dd_sincos(dd a, dd& s_out, dd& c_out)
+{
+    const double kq = rint(__dmul_rn(a.hi, 0.6366197723675814));               // nearest multiple of pi/2
+    dd r = a;
+    if (kq != 0.0) {
+        r = dd_sub(r, dd_two_prod(kq, 1.5707963267948966));                     // pi/2 in three words
+        r = dd_sub(r, dd_two_prod(kq, 6.123233995736766e-17));
+        r = dd_sub(r, dd_two_prod(kq, -1.4973849048591698e-33));
+    }
+    const dd r2 = dd_mul(r, r);
+    dd s = r, c = dd_from(1.0), ts = r, tc = dd_from(1.0);
+    for (int n = 1; n <= 16; ++n) {                                             // |r| <= pi/4: r^33/33! < 2^-130
+        tc = dd_div(dd_mul(tc, r2), dd_from((double)((2 * n - 1) * (2 * n))));
+        ts = dd_div(dd_mul(ts, r2), dd_from((double)((2 * n) * (2 * n + 1))));
+        if (n & 1) { c = dd_sub(c, tc); s = dd_sub(s, ts); }
+        else { c = dd_add(c, tc); s = dd_add(s, ts); }
+    }
+    const int quad = (int)((long long)kq & 3LL);
+    if (quad == 0) { s_out = s; c_out = c; }
+    else if (quad == 1) { s_out = c; c_out = dd_neg(s); }
+    else if (quad == 2) { s_out = dd_neg(s); c_out = dd_neg(c); }
+    else { s_out = dd_neg(c); c_out = s; }
+}
+// RN_fp32(hi + lo) without double rounding: hi alone decides unless it sits exactly on an fp32 midpoint
+__device__ __forceinline__ float dd_round_f32(dd v)
+{
+    const float f = __double2float_rn(v.hi);
+    if ((double)f == v.hi || !isfinite(f)) return f;
+    const float below = (double)f < v.hi ? f : nextafterf(f, -INFINITY);
+    const float above = (double)f < v.hi ? nextafterf(f, INFINITY) : f;
+    const double mid = 0.5 * ((double)below + (double)above);
+    if (v.hi < mid) return below;
+    if (v.hi > mid) return above;
+    return v.lo > 0.0 ? above : (v.lo < 0.0 ? below : f);
+}
+__device__ void deform_point_dd(double x, double y, double z, float theta_max, float k, float& X, float& Y, float& Z)
+{
+    const dd a = dd_div(dd_mul(dd_from((double)theta_max), dd_two_sum(y, 1.0)), dd_from(2.0));
+    dd sa, ca;
+    dd_sincos(a, sa, ca);
+    const dd dx = dd_from(x), dz = dd_from(z);
+    const dd tx = dd_add(dd_mul(dx, ca), dd_mul(dz, sa));
+    const dd ty = dd_from(y);
+    const dd tz = dd_add(dd_mul(dd_neg(dx), sa), dd_mul(dz, ca));
+    if (fabs((double)k) < 1e-6) { X = dd_round_f32(tx); Y = dd_round_f32(ty); Z = dd_round_f32(tz); return; }
+    const dd kd = dd_from((double)k);
+    const dd al = dd_mul(kd, tx);
+    dd sal, cal, sh, ch;
+    dd_sincos(al, sal, cal);
+    dd_sincos(dd_div(al, dd_from(2.0)), sh, ch);
+    X = dd_round_f32(dd_div(dd_mul(dd_sub(dd_from(1.0), dd_mul(kd, ty)), sal), kd));
+    Y = dd_round_f32(dd_add(dd_mul(ty, cal), dd_div(dd_mul(dd_from(2.0), dd_mul(sh, sh)), kd)));
+    Z = dd_round_f32(tz);
+}
+
+constexpr double LATTICE_E = 9.094947017729282e-13;      // 2^-40
+
+// could an error of LATTICE_E change the fp32 rounding of v ?
+__device__ __forceinline__ bool rounding_in_doubt(double v)
+{
+    const float f = __double2float_rn(v);
+    if (!isfinite(f)) return true;
+    const double lo = 0.5 * ((double)f + (double)nextafterf(f, -INFINITY));
+    const double hi = 0.5 * ((double)f + (double)nextafterf(f, INFINITY));
+    return fabs(v - lo) <= LATTICE_E || fabs(v - hi) <= LATTICE_E;
+}
+
+__global__ void k_deform_lattice(int nv, float theta_max_f, float k_f, float4* __restrict__ lat)
+{
+    const double theta_max = (double)theta_max_f, k = (double)k_f;
     const size_t np1 = (size_t)nv + 1;
     const size_t total = np1 * np1 * np1;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
@@ -60,7 +179,11 @@ __global__ void k_deform_lattice(int nv, double theta_max, double k, float4* __r
             X = __ddiv_rn(__dmul_rn(__dsub_rn(1.0, __dmul_rn(k, ty)), sal), k);
             Y = __dadd_rn(__dmul_rn(ty, cal), __ddiv_rn(__dmul_rn(__dmul_rn(2.0, sh), sh), k));
         }
-        lat[idx] = make_float4((float)X, (float)Y, (float)Z, 0.0f);
+        float fx = (float)X, fy = (float)Y, fz = (float)Z;
+        if (rounding_in_doubt(X) || rounding_in_doubt(Y) || rounding_in_doubt(Z))
+            deform_point_dd(x, y, z, theta_max_f, k_f, fx, fy, fz);
+        // a zero coordinate is stored as +0 (R28): -0 + 0 = +0 under round-to-nearest
+        lat[idx] = make_float4(__fadd_rn(fx, 0.0f), __fadd_rn(fy, 0.0f), __fadd_rn(fz, 0.0f), 0.0f);
     }
 }
 
@@ -352,7 +475,7 @@ void launch_deform(int nv, const nif_deform_params* pose, const float* user_latt
     const size_t np1 = (size_t)nv + 1, total = np1 * np1 * np1;
     int blocks = (int)((total + 255) / 256);
     if (blocks > 148 * 32) blocks = 148 * 32;
-    if (pose) k_deform_lattice<<<blocks, 256, 0, stream>>>(nv, (double)pose->twist_theta_max, (double)pose->bend_k, lattice);
+    if (pose) k_deform_lattice<<<blocks, 256, 0, stream>>>(nv, pose->twist_theta_max, pose->bend_k, lattice);
     else k_import_lattice<<<blocks, 256, 0, stream>>>(total, user_lattice, lattice);
     nif_count_launch(1);
 }

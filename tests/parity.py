@@ -3,7 +3,10 @@
 Tolerances (BASELINE.json:5 north star; derivations in DESIGN.md section 8):
   voxel ids and hit/miss flags   bit-exact
   t_in, t_out                    |d| <= 1e-5 |ref|  (expected bit-equal; mismatches are counted)
-  occlusion, albedo, normal      max abs error <= 2e-2
+  occlusion, albedo              max abs error <= 2e-2
+  unit normal                    max abs error <= 2e-2 where the normalisation is well-conditioned (|z_n| >= 0.3 rms(z),
+                                 >= 95 % of hit rays); everywhere: |dn| <= 2 |dz_n| / |z_n| (every normal error is
+                                 explained by the gated logit error) and the decode arithmetic itself to 1e-5 (R29)
   distance                       s = sigmoid(z1): |d| <= tol; d: |d| <= tol*l + 1e-5 (t_in+t_out);
                                  D = t_in + d: relative <= tol;  tol = 1e-2 (fp16 MLP) / 1e-5 (fp32)
   material argmax                agreement >= 99.9 % of hit rays
@@ -54,6 +57,22 @@ def compare_network(gpu: dict, ref: dict, fp16: bool, occlusion_only: bool = Fal
     m["tol"] = tol
     for k in ("albedo", "normal"):
         m[k + "_max_abs"] = float(np.abs(gpu[k][hit] - ref[k][hit]).max())
+    if "raw_logits" in gpu and gpu["raw_logits"] is not None:
+        # the unit normal z/|z| is ill-conditioned where the normal logits nearly vanish (random weights do
+        # that, a trained head does not): |dn| <= 2 |dz| / |z|.  Views: the error where |z| >= 0.3 rms
+        # (conditioned: the 2e-2 tolerance must hold), how many rays exceed 2e-2 at all, whether every
+        # error is explained by the logit error (first-order bound), and the decode arithmetic itself
+        # (GPU normal against the normalised GPU logits, fp64)
+        zr = ref["raw_logits"][hit][:, 2:5].astype(np.float64); zg = gpu["raw_logits"][hit][:, 2:5].astype(np.float64)
+        nr = np.linalg.norm(zr, axis=1); dz = np.linalg.norm(zg - zr, axis=1)
+        dn = np.abs(gpu["normal"][hit] - ref["normal"][hit]).max(axis=1)
+        cond = nr >= 0.3 * m["logit_rms"]
+        m["normal_conditioned_frac"] = float(cond.mean())
+        m["normal_conditioned_max_abs"] = float(dn[cond].max()) if cond.any() else 0.0
+        m["normal_over_2e-2_count"] = int((dn > 2e-2).sum())
+        m["normal_err_over_first_order_bound"] = float((dn / (2.0 * dz / np.maximum(nr, 1e-30) + 1e-6)).max())
+        ng = zg / np.sqrt(np.maximum((zg * zg).sum(1, keepdims=True), 1e-24))
+        m["normal_decode_max_abs"] = float(np.abs(gpu["normal"][hit] - ng).max())
     ti = ref["t_in"][hit].astype(np.float64); to = ref["t_out"][hit].astype(np.float64)
     ell = to - ti
     d_ref = ref["distance"][hit].astype(np.float64); d_gpu = gpu["distance"][hit].astype(np.float64)
@@ -72,14 +91,19 @@ def compare_network(gpu: dict, ref: dict, fp16: bool, occlusion_only: bool = Fal
     return m
 
 
-def assert_network(m: dict, fp16: bool, occlusion_only: bool = False):
+def assert_network(m: dict, fp16: bool, occlusion_only: bool = False, logit_tol: float | None = None):
     assert m["miss_all_zero"], m
     assert m["occlusion_max_abs"] <= 2e-2, m
     if "logit_max_abs_over_rms" in m:
-        assert m["logit_max_abs_over_rms"] <= (5e-3 if fp16 else 5e-5), m
+        assert m["logit_max_abs_over_rms"] <= (logit_tol or (5e-3 if fp16 else 5e-5)), m
     if occlusion_only:
         return
-    assert m["albedo_max_abs"] <= 2e-2 and m["normal_max_abs"] <= 2e-2, m
+    assert m["albedo_max_abs"] <= 2e-2, m
+    if "normal_conditioned_max_abs" in m:        # see compare_network; R29
+        assert m["normal_conditioned_max_abs"] <= 2e-2 and m["normal_conditioned_frac"] >= 0.95, m
+        assert m["normal_err_over_first_order_bound"] <= 1.0 and m["normal_decode_max_abs"] <= 1e-5, m
+    else:
+        assert m["normal_max_abs"] <= 2e-2, m
     assert m["s_max_abs"] <= m["tol"], m
     assert m["distance_max_over_bound"] <= 1.0, m
     assert m["dist_total_max_rel"] <= m["tol"], m
