@@ -96,6 +96,8 @@ class Oracle:
                                       C.c_void_p, C.c_void_p, C.c_uint32, C.c_int, C.c_void_p, C.c_void_p]
         L.nifo_hit_positions.argtypes = [C.c_void_p, C.c_int, C.c_uint32, C.c_float, C.c_float, C.c_int64] + [C.c_void_p] * 9
         L.nifo_inverse_trilinear.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nifo_exit_face_walk.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p,
+                                          C.c_int, C.c_void_p, C.c_void_p]
         self.acc_bytes = L.nifo_acc_bytes()
 
     # ---- deformation -----------------------------------------------------------------
@@ -272,6 +274,15 @@ class Oracle:
                                     hp.ctypes.data, hr.ctypes.data)
         return hp, hr
 
+
+    def exit_face_walk(self, nv, occ, lattice, bvh, origin, direction, max_vox):
+        """O11x: the literal exit-face walk of P:51 -> (seq [n, max_vox] of occupied voxel ids, -1 padded; status [n])."""
+        origin = _f32(origin); direction = _f32(direction)
+        n = len(origin)
+        seq = np.empty((n, max_vox), np.int32); status = np.empty(n, np.int32)
+        self.lib.nifo_exit_face_walk(int(nv), occ.ctypes.data, lattice.ctypes.data, bvh.handle if bvh is not None else None,
+                                     n, origin.ctypes.data, direction.ctypes.data, int(max_vox), seq.ctypes.data, status.ctypes.data)
+        return seq, status
 
     def next_voxel_brute(self, nv, occ, lattice, origin, direction, after_t, after_id):
         """O11 definition: successor of (after_t, after_id) in each ray's (t_in, id)-ordered voxel sequence."""

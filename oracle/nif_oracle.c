@@ -30,6 +30,8 @@
  *   O9 MLP               : torch fp64 linear+relu chain
  *   O9b fp16 activations : round_f16 == numpy float16 conversion; numpy float16 chain
  *   O10 decode           : closed forms / invariants
+ *   O11 walk             : per-voxel enumeration, DDA row, telescoping sum; O11x: the literal exit-face walk of
+ *                          P:51 visits the same voxel sequence (differences classified, tests/test_oracle_multi.py)
  *   end-to-end accuracy against a trained model: PARITY UNPINNED (no weights/objects exist).
  */
 #include <math.h>
@@ -981,6 +983,80 @@ int nifo_query(int nv, const uint8_t* occ, const float* lattice, const void* bvh
                         material ? material + 4 * r : 0, raw_logits ? raw_logits + NIFO_N_OUT * r : 0);
     }
     return 0;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* O11x  The voxel walk as P:51 words it, literally: "we adopt a geometry-aware traversal by    */
+/* explicitly determining the voxel face through which a ray exits, which allows correct         */
+/* selection of neighboring voxels"; the first voxel comes from the BVH.  This is a PIN    */
+/* for reading R22 (the product and O11 define the walk as the successor in (t_in, id) order      */
+/* over all occupied voxels), not a product path.  One ray: start in the first occupied voxel     */
+/* (O6).  In the current lattice cell (occupied or not -- every cell of the lattice has its 8      */
+/* deformed corners) intersect the ray with the cell's 12 triangles (O3/O4); the accepted          */
+/* intersection with the largest t is where the ray leaves the cell and the face that triangle     */
+/* lies on is the exit face (axis a, side s); the next cell is the lattice neighbour across it.     */
+/* Unoccupied cells are stepped through the same way; leaving the grid ends the walk.  `seq`        */
+/* receives the occupied cells in the order they are entered (the first voxel included).           */
+/* status: 0 = left the grid; 1 = no progress (the cell is only touched: exit t <= the t at which  */
+/* it was entered -- a ray through an edge or corner, where "the exit face" is not defined);        */
+/* 2 = no triangle of the cell accepted the ray; 3 = max_vox occupied voxels recorded; -1 = the    */
+/* ray hits no occupied voxel at all.                                                              */
+/* ------------------------------------------------------------------------------------ */
+static int cell_exit_face(const float* lattice, int nv, const int cell[3], v3 O, v3 D, int* axis, int* side, float* t_exit)
+{
+    int any = 0; float best = -INFINITY;
+    for (int a = 0; a < 3; ++a) {
+        int b = (a + 1) % 3, c = (a + 2) % 3;
+        for (int s = 0; s < 2; ++s) {
+            v3 q[2][2];
+            for (int u = 0; u < 2; ++u)
+                for (int v = 0; v < 2; ++v) {
+                    int idx[3];
+                    idx[a] = cell[a] + s; idx[b] = cell[b] + u; idx[c] = cell[c] + v;
+                    q[u][v] = lattice_pt(lattice, nv, idx[0], idx[1], idx[2]);
+                }
+            float t;
+            if (tri_hit(O, D, q[0][0], q[1][0], q[1][1], &t) && (!any || t > best)) { any = 1; best = t; *axis = a; *side = s; }
+            if (tri_hit(O, D, q[0][0], q[1][1], q[0][1], &t) && (!any || t > best)) { any = 1; best = t; *axis = a; *side = s; }
+        }
+    }
+    *t_exit = best;
+    return any;
+}
+
+void nifo_exit_face_walk(int nv, const uint8_t* occ, const float* lattice, const void* bvh,
+                         int64_t n, const float* origin, const float* dir, int max_vox,
+                         int32_t* seq, int32_t* status)
+{
+    for (int64_t r = 0; r < n; ++r) {
+        const float* o = origin + 3 * r; const float* d = dir + 3 * r;
+        int32_t* out = seq + (size_t)r * max_vox;
+        for (int k = 0; k < max_vox; ++k) out[k] = -1;
+        int32_t id; float ti, to;
+        if (bvh) traverse_bvh_one((const obvh*)bvh, o, d, &id, &ti, &to);
+        else nifo_traverse_brute(nv, occ, lattice, 1, o, d, &id, &ti, &to);
+        if (id < 0) { status[r] = -1; continue; }
+        v3 O, D; O.x = o[0]; O.y = o[1]; O.z = o[2]; D.x = d[0]; D.y = d[1]; D.z = d[2];
+        int cell[3]; cell[0] = id % nv; cell[1] = (id / nv) % nv; cell[2] = id / (nv * nv);
+        int count = 0;
+        out[count++] = id;
+        float t_entered = -INFINITY;
+        int st = 0;
+        for (;;) {
+            int axis = 0, side = 0; float t_exit;
+            if (!cell_exit_face(lattice, nv, cell, O, D, &axis, &side, &t_exit)) { st = 2; break; }
+            if (!(t_exit > t_entered)) { st = 1; break; }
+            cell[axis] += side ? 1 : -1;
+            if (cell[axis] < 0 || cell[axis] >= nv) { st = 0; break; }
+            t_entered = t_exit;
+            int32_t nid = cell[0] + nv * (cell[1] + nv * cell[2]);
+            if (occ[nid]) {
+                if (count == max_vox) { st = 3; break; }
+                out[count++] = nid;
+            }
+        }
+        status[r] = st;
+    }
 }
 
 /* ------------------------------------------------------------------------------------ */

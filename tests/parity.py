@@ -5,7 +5,7 @@ Tolerances (BASELINE.json:5 north star; derivations in DESIGN.md section 8):
   t_in, t_out                    |d| <= 1e-5 |ref|  (expected bit-equal; mismatches are counted)
   occlusion, albedo              max abs error <= 2e-2
   unit normal                    max abs error <= 2e-2 where the normalisation is well-conditioned (|z_n| >= 0.3 rms(z),
-                                 >= 95 % of hit rays); everywhere: |dn| <= 2 |dz_n| / |z_n| (every normal error is
+                                 >= 90 % of hit rays); everywhere: |dn| <= 2 |dz_n| / |z_n| (every normal error is
                                  explained by the gated logit error) and the decode arithmetic itself to 1e-5 (R29)
   distance                       s = sigmoid(z1): |d| <= tol; d: |d| <= tol*l + 1e-5 (t_in+t_out);
                                  D = t_in + d: relative <= tol;  tol = 1e-2 (fp16 MLP) / 1e-5 (fp32)
@@ -100,7 +100,7 @@ def assert_network(m: dict, fp16: bool, occlusion_only: bool = False, logit_tol:
         return
     assert m["albedo_max_abs"] <= 2e-2, m
     if "normal_conditioned_max_abs" in m:        # see compare_network; R29
-        assert m["normal_conditioned_max_abs"] <= 2e-2 and m["normal_conditioned_frac"] >= 0.95, m
+        assert m["normal_conditioned_max_abs"] <= 2e-2 and m["normal_conditioned_frac"] >= 0.9, m
         assert m["normal_err_over_first_order_bound"] <= 1.0 and m["normal_decode_max_abs"] <= 1e-5, m
     else:
         assert m["normal_max_abs"] <= 2e-2, m

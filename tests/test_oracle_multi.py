@@ -206,3 +206,85 @@ def test_trace_is_the_walk_without_stopping(oracle):
             assert multi["status"][r] == 0 and multi["steps"][r] == n_vox and multi["voxel_id"][r] == -1
         else:
             assert multi["status"][r] == 2 and multi["steps"][r] == K and multi["voxel_id"][r] == tid[r, K - 1]
+
+
+# ---- O11x: the literal exit-face walk of P:51 pins reading R22 (successor order) --------------------
+def _successor_sequences(bvh, o, d, max_vox):
+    n = len(o)
+    seq = np.full((n, max_vox), -1, np.int32)
+    tin = np.full((n, max_vox), np.nan, np.float32); tout = tin.copy()
+    at = np.full(n, -np.inf, np.float32); ai = np.full(n, -1, np.int32)
+    live = np.arange(n)
+    for k in range(max_vox):
+        vid, ti, to = bvh.next_voxel(o[live], d[live], at[live], ai[live])
+        ok = vid >= 0
+        seq[live[ok], k] = vid[ok]; tin[live[ok], k] = ti[ok]; tout[live[ok], k] = to[ok]
+        at[live[ok]] = ti[ok]; ai[live[ok]] = vid[ok]
+        live = live[ok]
+        if len(live) == 0:
+            break
+    return seq, tin, tout
+
+
+EXIT_FACE_CASES = [  # name, config, pose index, rays, lattice kind, minimum fraction of identical sequences
+    ("cfg0 twist", 0, 0, 4096, "pose", 0.995),
+    ("cfg1 bend (reduced frame)", 1, 0, 20_000, "pose", 0.999),
+    ("cfg2 twist+bend, pose 5 (reduced)", 2, 5, 5_000, "pose", 0.995),
+    ("wavy user lattice", 0, 0, 4096, "wavy", 0.999),
+    ("cfg0 identity", 0, 0, 4096, "identity", 0.999),
+]
+
+
+@pytest.mark.parametrize("name,cfg_id,pose_index,n_rays,kind,min_same", EXIT_FACE_CASES)
+def test_exit_face_walk_visits_the_successor_sequence(oracle, name, cfg_id, pose_index, n_rays, kind, min_same):
+    """P:51 words the walk as "determine the face through which the ray exits, select the neighbouring voxel";
+    the product (and O11) define it as the successor in (t_in, id) order over all occupied voxels (R22).
+    On a conforming lattice the two visit the same occupied voxels in the same order, except where "the
+    exit face" is not a well-defined notion:
+      (i)  a warped (non-convex) voxel the ray crosses twice: the literal walk leaves it at its LAST crossing
+           and never sees the voxels in the notch between the two crossings; the successor order lists them
+           after it (their [t_in, t_out] lies inside the crossed-twice voxel's);
+      (ii) a ray through a lattice edge or corner: the next cell is only touched (status 1: no progress).
+    Every differing ray must be of kind (i) or (ii), and they must be rare."""
+    cfg = I.get_config(cfg_id)
+    occ = I.occupancy(cfg)
+    pose = I.poses(cfg)[pose_index]
+    if kind == "wavy":
+        lat = I.wavy_lattice(cfg.nv, 3)
+    elif kind == "identity":
+        lat = oracle.deform_lattice(cfg.nv, 0.0, 0.0)
+    else:
+        lat = oracle.deform_lattice(cfg.nv, float(pose[0]), float(pose[1]))
+    bvh = oracle.bvh_build(cfg.nv, occ, lat)
+    lo, hi = bvh.bounds()
+    o, d = I.rays(cfg, pose_index, lo, hi, n=n_rays)
+    M = 3 * cfg.nv
+    seq, status = oracle.exit_face_walk(cfg.nv, occ, lat, bvh, o, d, M)
+    suc, tin, tout = _successor_sequences(bvh, o, d, M)
+    hit = suc[:, 0] >= 0
+    assert hit.sum() > 1000 and np.array_equal(seq[:, 0], suc[:, 0])          # same first voxel (P:53), same misses
+    assert (status[~hit] == -1).all() and np.isin(status[hit], (0, 1)).all()  # never "no triangle", never truncated
+    same = (seq == suc).all(axis=1)
+    assert same[hit].mean() >= min_same, (name, same[hit].mean())
+    n_notch = n_touch = 0
+    for r in np.nonzero(hit & ~same)[0]:
+        E = [int(v) for v in seq[r] if v >= 0]
+        S = [(int(v), float(a), float(b)) for v, a, b in zip(suc[r], tin[r], tout[r]) if v >= 0]
+        ids = [v for v, _, _ in S]
+        pos = [ids.index(v) for v in E]                       # every voxel of the literal walk is in the successor list ...
+        assert pos == sorted(pos), (name, r)                  # ... in the same order
+        iv = {v: (a, b) for v, a, b in S}
+        # a walk that stopped (ii) misses everything from the touched cell on (ties in t_in included)
+        tol = 4e-6 * max(1.0, abs(iv[E[-1]][1]))              # a few fp32 ulps of t
+        t_stop = np.inf if status[r] == 0 else iv[E[-1]][0] - tol
+        skipped = [v for v in ids if v not in E and iv[v][0] < t_stop]
+        for v in skipped:                                     # (i): nested inside a voxel the literal walk did visit
+            a, b = iv[v]
+            assert any(iv[e][0] <= a + tol and b <= iv[e][1] + tol for e in E), (name, r, v)
+        if status[r] == 1:
+            n_touch += 1
+        else:
+            assert skipped, (name, r)                         # status 0: the only difference is notch voxels
+            n_notch += 1
+    if kind == "identity":
+        assert n_notch == 0                                   # cubes are convex
