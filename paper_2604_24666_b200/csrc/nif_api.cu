@@ -14,6 +14,21 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline size_t elem_bytes(int dtype) { return dtype == NIF_F16 ? 2 : 4; }
 }  // namespace
 
+int nif_sm_count()
+{
+    static std::atomic<int> cache[64];                        // 0 = not asked yet
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return -1; }
+    if (dev >= 0 && dev < 64) {
+        const int c = cache[dev].load(std::memory_order_relaxed);
+        if (c > 0) return c;
+    }
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { (void)cudaGetLastError(); return -1; }
+    if (dev >= 0 && dev < 64) cache[dev].store(n, std::memory_order_relaxed);
+    return n;
+}
+
 extern "C" void nif_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 extern "C" int64_t nif_kernel_launch_count(void) { return (int64_t)g_launches.load(); }
 

@@ -143,6 +143,8 @@ int nif_tc_pack_weights(nif_net* net, cudaStream_t stream);
 int nif_tc_supported(const nif_net_desc* d);
 
 extern "C" int nif_device_supported(void);
+// multiprocessor count of the CURRENT device (cached per device ordinal); <= 0 on error
+int nif_sm_count();
 
 // per-kernel event timing hooks (nif_probe.cu); slot < 0 = profiling off
 int nif_prof_begin(cudaStream_t stream);

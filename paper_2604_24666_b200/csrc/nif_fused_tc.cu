@@ -3,26 +3,36 @@
 // tcgen05 tensor cores -> head decode, per tile of 128 hit rays, with no
 // intermediate HBM round trip.
 //
-// Warp roles (one CTA per SM, TC_THREADS threads):
-//   warps 0-3   "row" warps: thread r owns ray r of the tile.  They prepare the NEXT tile's rest-space
-//               endpoints (a2), then drain the layer-1 accumulator from TMEM (tcgen05.ld), run the
-//               hidden and output layers (ReLU -> fp16 -> swizzled smem A operand -> tcgen05.mma,
-//               issued by thread 0) and decode/store the heads (a5).
-//   warp 4      allocates TMEM; one lane issues the layer-1 MMAs chunk by chunk as ring stages fill
-//               (full/empty mbarriers), commits to the accumulator barrier.
-//   warp 5      one lane streams the layer-1 weight chunk of every ring stage from L2 with
-//               cp.async.bulk (W1 is NOT kept resident: a small shared-memory footprint leaves the L1
-//               large enough to keep the gathers' misses in flight).
-//   warps 6..   gather warps: lane = ray, one work item = (32-ray group, endpoint, PE sample); the
-//               L levels of that sample are interpolated (8 table gathers each, fp32, two batches of
-//               loads in flight) and written as fp16 into the canonical K-major SWIZZLE_128B A chunk
-//               of the stage, 16 bytes per store.
-// Hidden/output weight chunks stream through a 2-slot ring (warp 5, second lane) in the order the row
-// warps consume them.  The layer-1 accumulator is double-buffered in TMEM so the gathers of tile t+1
-// overlap the MLP tail of tile t.  Tiles are drawn from a global counter (dynamic scheduling).
-// Template parameters: W, F; CONCAT = concatenation reading of the hybrid encoding (R1; phi items + gamma
-// scalar items); LOCAL = voxel-local trilinear inverse for lattice-supplied deformations (R27).  Variants
-// are separate instantiations: the composition kernel's register allocation is fragile.
+// Data flow of one tile (UMMA M = 128 rays, thread/TMEM lane r = ray r of the tile):
+//   * every A operand lives in TENSOR MEMORY: the gather warps write the layer-1 features with
+//     tcgen05.st (fp16 pairs, 32 columns per 64-feature K chunk, a ring of chunk slots), the tail
+//     warps write the hidden activations the same way, and the MMAs are issued in the A-from-TMEM
+//     form.  Shared memory holds only B operands (weights) and ray info, which keeps the L1 data
+//     cache large for the table gathers and needs no proxy fences;
+//   * layer-1 weights stay resident in shared memory when they fit the budget (config 1-3: 104 KB),
+//     otherwise their K chunks stream through a ring (config 4: 416 KB); hidden/output weights are
+//     resident for W <= 64 and stream through a 2-slot ring for W = 128;
+//   * accumulators: layer 1 double-buffered (tile t+1 accumulates while tile t is in its tail), one
+//     hidden/output accumulator per tail group (W = 128: aliased onto the drained layer-1 buffer).
+//
+// Warp roles (one CTA per SM, 28 warps; setmaxnreg moves registers from the small roles to the
+// gather warps, whose loop needs 80):
+//   warps 0-3 / 4-7  tail groups 0 / 1, alternating tiles: drain the layer-1 accumulator (tcgen05.ld),
+//                    ReLU -> fp16 -> tcgen05.st as the next A operand, one thread issues the hidden /
+//                    output layer MMAs, finally decode and store the heads (a5).  Two groups keep two
+//                    tiles' dependent layer chains in flight.
+//   warp 8           lane 0 issues the layer-1 MMAs chunk by chunk as ring slots fill.
+//   warp 9           lane 0 loads the resident weights once and streams layer-1 chunks when they are
+//                    not resident; lane 1 streams hidden/output chunks (W = 128).
+//   warps 10-11      "prep": draw tile ids from the global counter, fetch the tile's rays through
+//                    hit_list and map entry/exit points back to rest space (a2) -> ray_buf (3 deep).
+//   warps 12-27      gather warps: lane = ray of row group (warp % 4); one work item = (endpoint, PE
+//                    sample): the L levels of that sample are interpolated (8 table gathers each, fp32,
+//                    two batches of loads in flight) and written as fp16 into the chunk slot (a3).
+// Template parameters: W, F; CONCAT = concatenation reading of the hybrid encoding (R1); LOCAL =
+// voxel-local trilinear inverse for lattice-supplied deformations (R27); PROBE = the gathers are
+// replaced by a constant A operand (the MLP-only probe of bench.py; its own instantiation, the product
+// kernels carry no probe branch).
 #include "nif_encode.cuh"
 
 #include <type_traits>
@@ -30,18 +40,21 @@
 namespace {
 
 constexpr int TC_TILE = 128;                 // rays per tile = UMMA M
-constexpr int TC_ROW_WARPS = 4;
-#ifndef NIF_TC_GATHER_WARPS
-#define NIF_TC_GATHER_WARPS 16
-#endif
-constexpr int TC_GATHER_WARPS = NIF_TC_GATHER_WARPS;
-constexpr int TC_MMA_WARP = TC_ROW_WARPS;    // warp index 4
-constexpr int TC_TMA_WARP = TC_ROW_WARPS + 1;  // warp index 5: streams the layer-1 weight chunks
-constexpr int TC_THREADS = 32 * (TC_ROW_WARPS + 2 + TC_GATHER_WARPS);
-constexpr int TC_MAX_STAGES = 4;             // ring depth (runtime 2..4); one stage = A chunk (128 x 64) + W1 chunk (W x 64)
-constexpr int TC_HSLOTS = 2;                 // ring of hidden/output-layer weight chunks (W x 64 each)
-constexpr int TC_A_CHUNK_BYTES = TC_TILE * 128;
+constexpr int TC_TAIL_WARPS = 8;             // two groups of 4
+constexpr int TC_MMA_WARP = 8;
+constexpr int TC_LOAD_WARP = 9;
+constexpr int TC_PREP_WARP0 = 10;            // warps 10, 11
+constexpr int TC_PREP_THREADS = 64;
+constexpr int TC_GATHER_WARP0 = 12;
+constexpr int TC_GATHER_WARPS = 16;
+constexpr int TC_THREADS = 32 * (TC_GATHER_WARP0 + TC_GATHER_WARPS);      // 896
+constexpr int TC_RAY_BUFS = 3;               // ray_buf depth: prep runs up to two tiles ahead of the tails
+constexpr int TC_RAY_FIELDS = 9;             // xi yi zi xo yo zo t_in t_out ray
+constexpr int TC_MAX_A_SLOTS = 8;            // layer-1 A chunk slots in TMEM (32 columns each)
+constexpr int TC_MAX_W1_SLOTS = 8;           // layer-1 weight chunk slots when W1 streams
+constexpr int TC_HSLOTS = 2;                 // hidden/output weight chunk ring (W = 128)
 constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded to the UMMA minimum)
+constexpr int TC_REGS_MISC = 40, TC_REGS_GATHER = 80;   // launch: 72 x 28 warps; setmaxnreg only redistributes what a dec released: 8 x 72 + 4 x 40 + 16 x 80 = 28 x 72
 
 // ---- PTX wrappers -----------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -70,10 +83,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
             "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
     } while (!done);
 }
-// wait for the role warps whose waits are long (a whole tile of gathers): try_wait with a suspend-time
-// hint parks the thread in hardware until the phase completes or the hint expires, so the wait takes
-// (almost) no issue slots from the gather warps and still wakes up as soon as the barrier flips
-__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, unsigned hint_ns)
+// wait for the role warps whose waits are long: try_wait with a suspend-time hint parks the thread in
+// hardware until the phase completes or the hint expires, so the wait takes (almost) no issue slots
+// from the gather warps and still wakes up as soon as the barrier flips
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, unsigned hint_ns = 20000)
 {
     uint32_t done;
     do {
@@ -86,7 +99,6 @@ __device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, u
     } while (!done);
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
@@ -105,16 +117,19 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols)
 {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
 }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
-// D[tmem] (+)= A[smem] * B[smem]^T, fp16 operands, fp32 accumulate, M = 128
-__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+// D[tmem] (+)= A[tmem] * B[smem]^T, fp16 operands, fp32 accumulate, M = 128.  A: lane = row, 16-bit
+// elements packed two per 32-bit column (K = 16 -> 8 columns); B: K-major SWIZZLE_128B descriptor.
+__device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
 {
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
-        "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 // all previously issued MMAs of this thread arrive on `bar` when they complete (implies fence::before_thread_sync)
 __device__ __forceinline__ void umma_commit(uint32_t bar)
@@ -158,12 +173,25 @@ __device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t* v)
         : "r"(taddr) : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+// registers -> TMEM: this warp's 32 lanes x 4 / 16 consecutive 32-bit columns
+__device__ __forceinline__ void tmem_st_32x4(uint32_t taddr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
 {
-    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
-__device__ __forceinline__ void row_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st_32x16(uint32_t taddr, const uint32_t* v)
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ void named_bar_sync(int id, int threads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
 
 __device__ __forceinline__ uint32_t pack_half2(float a, float b)
 {
@@ -177,6 +205,16 @@ __host__ __device__ __forceinline__ uint32_t sw128_off(uint32_t row, uint32_t un
     return row * 128u + ((unit ^ (row & 7u)) << 4);
 }
 
+// ---- optional per-tile timestamps (compile with -DNIF_TC_TRACE; _work/ scripts read them) ---------
+#ifdef NIF_TC_TRACE
+__device__ unsigned int* g_tc_trace = nullptr;        // [cta][NIF_TC_TRACE_TILES][32] clock() samples
+#define NIF_TC_TRACE_TILES 24
+#define TC_TRACE(j, slot) do { if (g_tc_trace && (j) < NIF_TC_TRACE_TILES) \
+        g_tc_trace[((size_t)blockIdx.x * NIF_TC_TRACE_TILES + (size_t)(j)) * 32 + (slot)] = (unsigned int)clock(); } while (0)
+#else
+#define TC_TRACE(j, slot) do { } while (0)
+#endif
+
 // ---- kernel parameters -------------------------------------------------------------------------
 struct TcParams {
     NifEnc enc;
@@ -187,7 +225,8 @@ struct TcParams {
     const __half* table;
     const uint8_t* w_img;         // B-operand images: W1 chunks | hidden layers 2..H | output layer
     uint32_t w_bytes, w1_bytes;
-    int stages;                   // ring depth, 2..TC_MAX_STAGES
+    int w1_slots;                 // layer-1 weight chunk slots in shared memory
+    int w1_resident;              // 1: w1_slots == n_chunks, loaded once; 0: ring
     float theta_max, bend_k;
     const float* origin;
     const float* dir;
@@ -201,25 +240,33 @@ struct TcParams {
     unsigned flags;
 };
 
+// shared memory: [hidden/output weights][layer-1 weight slots][ray_buf][barriers, tile ids, level constants]
 struct TcSmemLayout {
-    uint32_t w_img, a_ring, act, ray_buf, bars, total;
+    uint32_t w_hid, w1, ray_buf, bars, total;
 };
-__host__ __device__ inline TcSmemLayout tc_smem_layout(int stages, int W)
+__host__ __device__ inline uint32_t tc_hid_bytes(int W, int hidden_layers)
+{
+    const uint32_t KC = (uint32_t)(W + 63) / 64;
+    if (W > 64) return TC_HSLOTS * (uint32_t)W * 128u;                                   // ring
+    return (uint32_t)(hidden_layers - 1) * KC * (uint32_t)W * 128u + KC * TC_NOUT_PAD * 128u;   // resident
+}
+__host__ __device__ inline TcSmemLayout tc_smem_layout(int W, int hidden_layers, int w1_slots)
 {
     TcSmemLayout L;
     uint32_t off = 0;
-    L.w_img = off;   off += TC_HSLOTS * (uint32_t)W * 128u;          // hidden/output weight chunk ring
-    L.a_ring = off;  off += (uint32_t)stages * (TC_A_CHUNK_BYTES + (uint32_t)W * 128u);   // stage = A chunk | W1 chunk
-    L.act = off;     off += (uint32_t)((W + 63) / 64) * TC_A_CHUNK_BYTES;
-    L.ray_buf = off; off += 2u * TC_TILE * 8u * sizeof(float);
-    L.bars = off;    off += 512;
+    L.w_hid = off;   off += (tc_hid_bytes(W, hidden_layers) + 1023u) & ~1023u;
+    L.w1 = off;      off += (uint32_t)w1_slots * (uint32_t)W * 128u;
+    L.ray_buf = off; off += (uint32_t)TC_RAY_BUFS * TC_RAY_FIELDS * TC_TILE * 4u;
+    L.bars = off;    off += 1024;
     L.total = off + 1024;                       // slack for the manual 1024-byte alignment
     return L;
 }
 
-enum { BAR_FULL = 0, BAR_EMPTY = TC_MAX_STAGES, BAR_ACC_FULL = 2 * TC_MAX_STAGES, BAR_ACC_EMPTY = BAR_ACC_FULL + 2,
-       BAR_RAY_FULL = BAR_ACC_EMPTY + 2, BAR_RAY_EMPTY = BAR_RAY_FULL + 2, BAR_HID = BAR_RAY_EMPTY + 2,
-       BAR_HFULL = BAR_HID + 1, BAR_HEMPTY = BAR_HFULL + TC_HSLOTS, BAR_COUNT = BAR_HEMPTY + TC_HSLOTS };
+enum { BAR_A_FULL = 0, BAR_A_EMPTY = BAR_A_FULL + TC_MAX_A_SLOTS, BAR_W1_FULL = BAR_A_EMPTY + TC_MAX_A_SLOTS,
+       BAR_W1_EMPTY = BAR_W1_FULL + TC_MAX_W1_SLOTS, BAR_ACC_FULL = BAR_W1_EMPTY + TC_MAX_W1_SLOTS,
+       BAR_ACC_EMPTY = BAR_ACC_FULL + 2, BAR_RAY_FULL = BAR_ACC_EMPTY + 2, BAR_RAY_EMPTY = BAR_RAY_FULL + TC_RAY_BUFS,
+       BAR_HID = BAR_RAY_EMPTY + TC_RAY_BUFS, BAR_HFULL = BAR_HID + 2, BAR_HEMPTY = BAR_HFULL + TC_HSLOTS,
+       BAR_WRES = BAR_HEMPTY + TC_HSLOTS, BAR_COUNT = BAR_WRES + 1 };
 
 // ---- (a3) gathers of one sample, software-pipelined in batches of 8/F levels (16 loads of 4 B for
 // F = 2, 8 loads of 8 B for F = 4).  issue() computes the 8 table indices of each level of the batch
@@ -346,79 +393,76 @@ struct GatherBatch {
     }
 };
 
-// drains W fp32 accumulator columns of this thread's row from TMEM, applies ReLU, rounds to fp16
-// and writes them as the next layer's A operand (K-major SWIZZLE_128B, chunks of 64 columns)
+// drains N32*32 fp32 accumulator columns of this thread's row from TMEM, applies ReLU, rounds to fp16
+// and writes them back to TMEM as the next layer's A operand (two fp16 per 32-bit column)
 template <int W>
-__device__ __forceinline__ void drain_relu_to_act(uint32_t taddr_row, uint32_t act_base, uint32_t row)
+__device__ __forceinline__ void drain_relu_to_act(uint32_t tm_src_row, uint32_t tm_act_row)
 {
-    __syncwarp();                                          // tcgen05.ld is .sync.aligned
+    __syncwarp();                                          // tcgen05.ld / .st are .sync.aligned
 #pragma unroll
     for (int cg = 0; cg < W / 32; ++cg) {
-        uint32_t v[32];
-        tmem_ld_32x32(taddr_row + (uint32_t)(cg * 32), v);
+        uint32_t v[32], h[16];
+        tmem_ld_32x32(tm_src_row + (uint32_t)(cg * 32), v);
         tmem_ld_wait();
-        const uint32_t chunk = act_base + (uint32_t)((cg * 32) / 64) * TC_A_CHUNK_BYTES;
-        const uint32_t unit0 = (uint32_t)(((cg * 32) % 64) / 8);
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            uint32_t h[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                h[i] = pack_half2(fmaxf(__uint_as_float(v[8 * u + 2 * i]), 0.0f),
-                                  fmaxf(__uint_as_float(v[8 * u + 2 * i + 1]), 0.0f));
-            st_shared_v4(chunk + sw128_off(row, unit0 + (uint32_t)u), h[0], h[1], h[2], h[3]);
-        }
+        for (int i = 0; i < 16; ++i)
+            h[i] = pack_half2(fmaxf(__uint_as_float(v[2 * i]), 0.0f), fmaxf(__uint_as_float(v[2 * i + 1]), 0.0f));
+        tmem_st_32x16(tm_act_row + (uint32_t)(cg * 16), h);
     }
+    tmem_st_wait();
 }
 
-// issues D[128 x N] (+)= act[:, 64 kc .. 64 kc + 63] * Wchunk[N x 64]^T for one K chunk (one thread)
-template <int W>
-__device__ __forceinline__ void issue_layer_chunk(uint32_t d_tmem, uint32_t act_base, uint32_t w_chunk, int N, int kc)
-{
-    constexpr int K16 = (W < 64 ? W : 64) / 16;            // UMMA K steps per chunk
-    const uint32_t idesc = idesc_f16(TC_TILE, N);
-#pragma unroll
-    for (int k = 0; k < K16; ++k)
-        umma_f16(d_tmem, smem_desc_sw128(act_base + (uint32_t)kc * TC_A_CHUNK_BYTES + (uint32_t)k * 32u),
-                 smem_desc_sw128(w_chunk + (uint32_t)k * 32u), idesc, (uint32_t)((kc | k) != 0));
-}
-
-template <int W, int F, bool CONCAT, bool LOCAL>
+template <int W, int F, bool CONCAT, bool LOCAL, bool PROBE>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_fused_encode_mlp(const TcParams p)
 {
+    constexpr bool ALIAS = (W == 128);                     // hidden/output accumulator = the drained layer-1 buffer
+    constexpr int NG = (W == 128) ? 1 : 2;                 // tail groups
+    constexpr int KC = (W + 63) / 64;                      // K chunks of a hidden layer
+    constexpr int K16 = (W < 64 ? W : 64) / 16;            // UMMA K steps per hidden chunk
+    constexpr uint32_t HCHUNK = (uint32_t)W * 128u;        // one weight chunk: W rows x 64 fp16
+    constexpr uint32_t OUTCHUNK = TC_NOUT_PAD * 128u;
+    constexpr uint32_t ACT_COLS = W / 2;
+    constexpr uint32_t C_HID = 2u * W;
+    constexpr uint32_t C_ACT = ALIAS ? 2u * W : 2u * W + NG * W;
+    constexpr uint32_t C_RING = C_ACT + NG * ACT_COLS;
+    constexpr int A_SLOTS = (512 - (int)C_RING) / 32 < TC_MAX_A_SLOTS ? (512 - (int)C_RING) / 32 : TC_MAX_A_SLOTS;
+    constexpr uint32_t TMEM_COLS = 512;
+    static_assert(A_SLOTS >= 4, "layer-1 A ring too short");
+
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    const TcSmemLayout SL = tc_smem_layout(p.stages, W);
-    const uint32_t TC_STAGES = (uint32_t)p.stages;
-    constexpr uint32_t HCHUNK = (uint32_t)W * 128u;                            // hidden-layer weight chunk (W x 64 fp16)
-    constexpr uint32_t STAGE_BYTES = TC_A_CHUNK_BYTES + (uint32_t)W * 128u;
-    const uint32_t s_w = smem_base + SL.w_img, s_a = smem_base + SL.a_ring, s_act = smem_base + SL.act;
-    float* ray_buf = reinterpret_cast<float*>(smem_gen + SL.ray_buf);          // [2][128][8]
+    const TcSmemLayout SL = tc_smem_layout(W, p.hidden_layers, p.w1_slots);
+    const uint32_t s_whid = smem_base + SL.w_hid, s_w1 = smem_base + SL.w1;
+    float* ray_buf = reinterpret_cast<float*>(smem_gen + SL.ray_buf);          // [TC_RAY_BUFS][TC_RAY_FIELDS][128]
     const uint32_t s_bar = smem_base + SL.bars;
-    uint32_t* s_tmem_ptr = reinterpret_cast<uint32_t*>(smem_gen + SL.bars + 240);
-    TcLevel* s_lvl = reinterpret_cast<TcLevel*>(smem_gen + SL.bars + 256);      // 16 levels x 16 B, 16-byte aligned
-    static_assert(8 * BAR_COUNT <= 224, "barrier block overlaps the tile-id / TMEM pointer slots");
+    static_assert(8 * BAR_COUNT <= 480, "barrier block overlaps the tile-id / TMEM pointer slots");
+    volatile int* s_tile = reinterpret_cast<volatile int*>(smem_gen + SL.bars + 480);    // [TC_RAY_BUFS]
+    uint32_t* s_tmem_ptr = reinterpret_cast<uint32_t*>(smem_gen + SL.bars + 496);
     auto bar = [&](int i) { return s_bar + 8u * (uint32_t)i; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int L = p.enc.levels, S = 1 + 2 * p.enc.bands;
     const int epc = p.es_per_chunk, n_chunks = p.n_chunks;
-    constexpr uint32_t TMEM_COLS = (3 * W + 32) <= 256 ? 256 : 512;
-    constexpr int KC = (W + 63) / 64;
+    const uint32_t W1_SLOTS = (uint32_t)p.w1_slots;
 
     // ---- one-time setup ------------------------------------------------------------------------
     if (tid == 0) {
-        for (int i = 0; i < TC_MAX_STAGES; ++i) { mbar_init(bar(BAR_FULL + i), 4u * (uint32_t)epc + 1u); mbar_init(bar(BAR_EMPTY + i), 1); }
+        for (int i = 0; i < TC_MAX_A_SLOTS; ++i) { mbar_init(bar(BAR_A_FULL + i), 4u * (uint32_t)epc); mbar_init(bar(BAR_A_EMPTY + i), 1); }
+        for (int i = 0; i < TC_MAX_W1_SLOTS; ++i) { mbar_init(bar(BAR_W1_FULL + i), 1); mbar_init(bar(BAR_W1_EMPTY + i), 1); }
         for (int i = 0; i < TC_HSLOTS; ++i) { mbar_init(bar(BAR_HFULL + i), 1); mbar_init(bar(BAR_HEMPTY + i), 1); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar(BAR_ACC_FULL + i), 1); mbar_init(bar(BAR_ACC_EMPTY + i), TC_TILE);
-            mbar_init(bar(BAR_RAY_FULL + i), TC_TILE); mbar_init(bar(BAR_RAY_EMPTY + i), TC_GATHER_WARPS);
+            mbar_init(bar(BAR_HID + i), 1);
         }
-        mbar_init(bar(BAR_HID), 1);
+        for (int i = 0; i < TC_RAY_BUFS; ++i) {
+            mbar_init(bar(BAR_RAY_FULL + i), TC_PREP_THREADS); mbar_init(bar(BAR_RAY_EMPTY + i), TC_GATHER_WARPS + TC_TILE);
+        }
+        mbar_init(bar(BAR_WRES), 1);
         fence_barrier_init();
     }
+    TcLevel* s_lvl = reinterpret_cast<TcLevel*>(smem_gen + SL.bars + 512);      // 16 levels x 16 B
     if (tid < NIF_MAX_LEVELS) {
         const int N = tid < L ? p.enc.res[tid] : 1;
         TcLevel lv;
@@ -431,221 +475,285 @@ k_fused_encode_mlp(const TcParams p)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *s_tmem_ptr;
-    const uint32_t tm_acc1 = tmem_base, tm_hid = tmem_base + 2u * W, tm_out = tmem_base + 3u * W;
+    const uint32_t tm_acc1 = tmem_base, tm_ring = tmem_base + C_RING;
 
     const long long n_hit = (long long)p.scratch->n_hit;
     const long long n_tiles = (n_hit + TC_TILE - 1) / TC_TILE;
-    // dynamic tile scheduler: row thread 0 draws tile ids from a global counter in prepare() and
-    // publishes them in s_tile[j & 1] (-1 = no more tiles); every role reads them after ray_full[j & 1]
-    volatile int* s_tile = reinterpret_cast<volatile int*>(smem_gen + SL.bars + 224);
 
-    if (warp < TC_ROW_WARPS) {
-        // ======================= row warps: (a2) for the next tile, MLP tail + (a5) ==============
-        const int r = tid;
-        long long cur_ray = -1, nxt_ray = -1;
-        float cur_ti = 0.f, cur_to = 0.f, nxt_ti = 0.f, nxt_to = 0.f;
-        uint32_t hid_phase = 0, hq = 0;                   // hq: hidden/output weight chunks consumed so far
-        auto run_layer = [&](uint32_t d_tmem, int N) {   // thread 0: one layer, chunks arrive through the H ring
-            tc_fence_after();
-            for (int kc = 0; kc < KC; ++kc, ++hq) {
-                const uint32_t slot = hq % TC_HSLOTS;
-                mbar_wait_sleep(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u, 20000);
+    if (warp < TC_TAIL_WARPS) {
+        // ======================= tail groups: MLP layers 2.. and (a5), alternating tiles ===========
+        const int g = warp >> 2;
+        if (g < NG) {
+            const int tg = tid - g * TC_TILE;                              // row of the tile / TMEM lane
+            const uint32_t t_row = (uint32_t)((warp & 3) * 32) << 16;
+            const uint32_t tm_act = tmem_base + C_ACT + (uint32_t)g * ACT_COLS;
+            uint32_t hid_phase = 0, hq = 0;
+            if (W <= 64 && tg == 0) mbar_wait_sleep(bar(BAR_WRES), 0);    // resident hidden/output weights landed
+            // one layer of this group's tile: A = the group's activations (TMEM), B = weight chunks, D = d_tmem
+            auto run_layer = [&](uint32_t d_tmem, int N, int li) {
                 tc_fence_after();
-                issue_layer_chunk<W>(d_tmem, s_act, s_w + slot * HCHUNK, N, kc);
-                umma_commit(bar(BAR_HEMPTY + slot));
-            }
-            umma_commit(bar(BAR_HID));
-        };
-        int nxt_tile = -1;
-        auto prepare = [&](int j) {                       // rest-space endpoints of the j-th tile -> ray_buf[j&1]
-            const int b = j & 1;
-            mbar_wait_sleep(bar(BAR_RAY_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 20000);
-            if (tid == 0) {
-                const unsigned t = atomicAdd(p.tile_counter, 1u);
-                s_tile[b] = (long long)t < n_tiles ? (int)t : -1;
-            }
-            row_bar_sync();
-            nxt_tile = s_tile[b];
-            const long long h = nxt_tile < 0 ? n_hit : (long long)nxt_tile * TC_TILE + r;
-            float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f;
-            nxt_ray = -1; nxt_ti = 0.f; nxt_to = 0.f;
-            if (h < n_hit) {
-                nxt_ray = p.hit_list[h];
-                nxt_ti = p.out.t_in[nxt_ray]; nxt_to = p.out.t_out[nxt_ray];
-                const float ox = p.origin[3 * nxt_ray], oy = p.origin[3 * nxt_ray + 1], oz = p.origin[3 * nxt_ray + 2];
-                const float dx = p.dir[3 * nxt_ray], dy = p.dir[3 * nxt_ray + 1], dz = p.dir[3 * nxt_ray + 2];
-                if constexpr (LOCAL) {           // deformation given as a lattice: voxel-local inverse (R27)
-                    const float oo[3] = {ox, oy, oz}, dd[3] = {dx, dy, dz};
-                    float ri[3], ro[3];
-                    nif_map_back_pair<true>(nif_ray_map(p.map, p.batch, nxt_ray), p.out.voxel_id[nxt_ray], oo, dd, nxt_ti, nxt_to, ri, ro);
-                    xi = ri[0]; yi = ri[1]; zi = ri[2]; xo = ro[0]; yo = ro[1]; zo = ro[2];
-                } else {
-                float th = p.theta_max, bk = p.bend_k;
-                if (p.batch.pose_id) {           // nif_query_poses: this ray's pose
-                    const NifPoseDesc* pd = p.batch.poses + p.batch.pose_id[nxt_ray];
-                    th = pd->theta_max; bk = pd->bend_k;
-                }
-                nif_inverse_deform(th, bk, fmaf(nxt_ti, dx, ox), fmaf(nxt_ti, dy, oy), fmaf(nxt_ti, dz, oz), xi, yi, zi);
-                nif_inverse_deform(th, bk, fmaf(nxt_to, dx, ox), fmaf(nxt_to, dy, oy), fmaf(nxt_to, dz, oz), xo, yo, zo);
-                }
-            }
-            float* rb = ray_buf + ((size_t)b * TC_TILE + r) * 8;
-            rb[0] = nif_normalise(xi); rb[1] = nif_normalise(yi); rb[2] = nif_normalise(zi);
-            rb[3] = nif_normalise(xo); rb[4] = nif_normalise(yo); rb[5] = nif_normalise(zo);
-            mbar_arrive(bar(BAR_RAY_FULL + b));
-        };
-        prepare(0);
-        const uint32_t t_row = (uint32_t)(warp * 32) << 16;          // this warp's TMEM lane quarter
-        for (int j = 0;; ++j) {
-            if (nxt_tile < 0) break;
-            cur_ray = nxt_ray; cur_ti = nxt_ti; cur_to = nxt_to;
-            prepare(j + 1);
-            const int b = j & 1;
-            // layer 1 accumulator of tile j
-            mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1), 20000);
-            tc_fence_after();
-            drain_relu_to_act<W>(tm_acc1 + (uint32_t)(b * W) + t_row, s_act, (uint32_t)r);
-            tc_fence_before();
-            mbar_arrive(bar(BAR_ACC_EMPTY + b));
-            fence_proxy_async();
-            row_bar_sync();
-            // hidden layers 2..H
-            for (int hl = 1; hl < p.hidden_layers; ++hl) {
-                if (tid == 0) run_layer(tm_hid, W);
-                mbar_wait_sleep(bar(BAR_HID), hid_phase, 20000); hid_phase ^= 1u;
-                tc_fence_after();
-                drain_relu_to_act<W>(tm_hid + t_row, s_act, (uint32_t)r);
-                tc_fence_before();
-                fence_proxy_async();
-                row_bar_sync();
-            }
-            // output layer (12 heads padded to N = 16) and (a5) decode
-            if (tid == 0) run_layer(tm_out, TC_NOUT_PAD);
-            mbar_wait_sleep(bar(BAR_HID), hid_phase, 20000); hid_phase ^= 1u;
-            tc_fence_after();
-            uint32_t zr[16];
-            __syncwarp();
-            tmem_ld_32x16(tm_out + t_row, zr);
-            tmem_ld_wait();
-            tc_fence_before();
-            if (cur_ray >= 0) {
-                float z[NIF_N_OUT];
+                const uint32_t idesc = idesc_f16(TC_TILE, N);
 #pragma unroll
-                for (int a = 0; a < NIF_N_OUT; ++a) z[a] = __uint_as_float(zr[a]);
-                nif_decode_store<LOCAL>(z, cur_ti, cur_to, cur_ray, p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map, p.batch});
-            }
-        }
-    } else if (warp == TC_MMA_WARP) {
-        // ======================= layer-1 MMA issuer =============================================
-        if (lane == 0) {
-            const uint32_t idesc = idesc_f16(TC_TILE, W);
-            uint32_t q = 0;
-            for (int j = 0;; ++j) {
-                const int b = j & 1;
-                mbar_wait_sleep(bar(BAR_RAY_FULL + b), (uint32_t)((j >> 1) & 1), 20000);
-                if (s_tile[b] < 0) break;
-                mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1), 20000);
-                tc_fence_after();
-                for (int c = 0; c < n_chunks; ++c, ++q) {
-                    const uint32_t stage = q % TC_STAGES;
-                    mbar_wait_sleep(bar(BAR_FULL + stage), (q / TC_STAGES) & 1u, 20000);
-                    tc_fence_after();
-                    const uint32_t a0 = s_a + stage * STAGE_BYTES, b0 = a0 + TC_A_CHUNK_BYTES;
-#pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        umma_f16(tm_acc1 + (uint32_t)(b * W), smem_desc_sw128(a0 + (uint32_t)k * 32u),
-                                 smem_desc_sw128(b0 + (uint32_t)k * 32u), idesc, (uint32_t)((c | k) != 0));
-                    umma_commit(bar(BAR_EMPTY + stage));
-                }
-                umma_commit(bar(BAR_ACC_FULL + b));
-            }
-        }
-    } else if (warp == TC_TMA_WARP) {
-        // ======================= layer-1 weight chunks: L2 -> ring stage (cp.async.bulk) ========
-        // W1 (D_in x W fp16) does not stay in shared memory: a small footprint leaves the L1 data
-        // cache large enough to keep the gathers' misses in flight.
-        if (lane == 0) {
-            constexpr uint32_t W1_CHUNK = (uint32_t)W * 128u;
-            uint32_t q = 0;
-            for (int j = 0;; ++j) {
-                mbar_wait_sleep(bar(BAR_RAY_FULL + (j & 1)), (uint32_t)((j >> 1) & 1), 20000);
-                if (s_tile[j & 1] < 0) break;
-                for (int c = 0; c < n_chunks; ++c, ++q) {
-                    const uint32_t stage = q % TC_STAGES;
-                    mbar_wait_sleep(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u, 20000);
-                    mbar_expect_tx(bar(BAR_FULL + stage), W1_CHUNK);
-                    bulk_g2s(s_a + stage * STAGE_BYTES + TC_A_CHUNK_BYTES, p.w_img + (size_t)c * W1_CHUNK, W1_CHUNK,
-                             bar(BAR_FULL + stage));
-                }
-            }
-        } else if (lane == 1) {
-            // hidden layers 2..H and the output layer: KC chunks each, per tile, in the order the row
-            // warps consume them (they are small, so they share one 2-slot ring instead of living in smem)
-            const uint8_t* wh = p.w_img + p.w1_bytes;
-            const uint32_t out_chunk = TC_NOUT_PAD * 128u;
-            uint32_t hq = 0;
-            for (int j = 0;; ++j) {
-                mbar_wait_sleep(bar(BAR_RAY_FULL + (j & 1)), (uint32_t)((j >> 1) & 1), 20000);
-                if (s_tile[j & 1] < 0) break;
-                for (int l = 1; l <= p.hidden_layers; ++l) {
-                    const bool is_out = l == p.hidden_layers;
-                    const uint32_t bytes = is_out ? out_chunk : HCHUNK;
-                    const uint8_t* src = wh + (size_t)(l - 1) * (size_t)(KC * HCHUNK);
-                    for (int kc = 0; kc < KC; ++kc, ++hq) {
+                for (int kc = 0; kc < KC; ++kc) {
+                    uint32_t wchunk;
+                    if constexpr (W <= 64) {
+                        wchunk = s_whid + (uint32_t)(li * KC) * HCHUNK + (uint32_t)kc * (N == TC_NOUT_PAD ? OUTCHUNK : HCHUNK);
+                    } else {
                         const uint32_t slot = hq % TC_HSLOTS;
-                        mbar_wait_sleep(bar(BAR_HEMPTY + slot), ((hq / TC_HSLOTS) & 1u) ^ 1u, 20000);
-                        mbar_expect_tx(bar(BAR_HFULL + slot), bytes);
-                        bulk_g2s(s_w + slot * HCHUNK, src + (size_t)kc * bytes, bytes, bar(BAR_HFULL + slot));
+                        mbar_wait_sleep(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u);
+                        tc_fence_after();
+                        wchunk = s_whid + slot * HCHUNK;
+                    }
+#pragma unroll
+                    for (int k = 0; k < K16; ++k)
+                        umma_f16_ts(d_tmem, tm_act + (uint32_t)(kc * 32 + k * 8), smem_desc_sw128(wchunk + (uint32_t)k * 32u),
+                                    idesc, (uint32_t)((kc | k) != 0));
+                    if constexpr (W > 64) { umma_commit(bar(BAR_HEMPTY + (hq % TC_HSLOTS))); ++hq; }
+                }
+                umma_commit(bar(BAR_HID + g));
+            };
+            for (int j = g;; j += NG) {
+                const int nb = j % TC_RAY_BUFS, b = j & 1;
+                mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
+                if (s_tile[nb] < 0) break;
+                const float* rb = ray_buf + (size_t)nb * TC_RAY_FIELDS * TC_TILE + tg;
+                const float cur_ti = rb[6 * TC_TILE], cur_to = rb[7 * TC_TILE];
+                const long long cur_ray = (long long)__float_as_int(rb[8 * TC_TILE]);
+                mbar_arrive(bar(BAR_RAY_EMPTY + nb));
+                const uint32_t tm_l1 = tm_acc1 + (uint32_t)(b * W);
+                const uint32_t tm_hid = ALIAS ? tm_l1 : tmem_base + C_HID + (uint32_t)(g * W);
+                if (tg == 0) TC_TRACE(j, 1);
+                // layer 1 accumulator of tile j -> ReLU -> fp16 activations
+                mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1));
+                if (tg == 0) TC_TRACE(j, 2);
+                tc_fence_after();
+                drain_relu_to_act<W>(tm_l1 + t_row, tm_act + t_row);
+                tc_fence_before();
+                if constexpr (!ALIAS) mbar_arrive(bar(BAR_ACC_EMPTY + b));
+                named_bar_sync(1 + g, TC_TILE);
+                if (tg == 0) TC_TRACE(j, 3);
+                // hidden layers 2..H
+                for (int hl = 1; hl < p.hidden_layers; ++hl) {
+                    if (tg == 0) run_layer(tm_hid, W, hl - 1);
+                    mbar_wait_sleep(bar(BAR_HID + g), hid_phase); hid_phase ^= 1u;
+                    tc_fence_after();
+                    drain_relu_to_act<W>(tm_hid + t_row, tm_act + t_row);
+                    tc_fence_before();
+                    named_bar_sync(1 + g, TC_TILE);
+                    if (tg == 0) TC_TRACE(j, 3 + hl);
+                }
+                // output layer (12 heads padded to N = 16) and (a5) decode
+                if (tg == 0) run_layer(tm_hid, TC_NOUT_PAD, p.hidden_layers - 1);
+                mbar_wait_sleep(bar(BAR_HID + g), hid_phase); hid_phase ^= 1u;
+                if (tg == 0) TC_TRACE(j, 20);
+                tc_fence_after();
+                uint32_t zr[16];
+                __syncwarp();
+                tmem_ld_32x16(tm_hid + t_row, zr);
+                tmem_ld_wait();
+                tc_fence_before();
+                if constexpr (ALIAS) mbar_arrive(bar(BAR_ACC_EMPTY + b));
+                if (cur_ray >= 0) {
+                    float z[NIF_N_OUT];
+#pragma unroll
+                    for (int a = 0; a < NIF_N_OUT; ++a) z[a] = __uint_as_float(zr[a]);
+                    nif_decode_store<LOCAL>(z, cur_ti, cur_to, cur_ray, p.out, p.flags, NifDecodeCtx{p.origin, p.dir, p.map, p.batch});
+                }
+                if (tg == 0) TC_TRACE(j, 22);
+            }
+        }
+    } else if (warp < TC_GATHER_WARP0) {
+        reg_dec<TC_REGS_MISC>();
+        if (warp == TC_MMA_WARP) {
+            // ======================= layer-1 MMA issuer =============================================
+            if (lane == 0) {
+                const uint32_t idesc = idesc_f16(TC_TILE, W);
+                if (p.w1_resident) mbar_wait_sleep(bar(BAR_WRES), 0);
+                uint32_t q = 0;
+                for (int j = 0;; ++j) {
+                    const int nb = j % TC_RAY_BUFS, b = j & 1;
+                    mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
+                    if (s_tile[nb] < 0) break;
+                    mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
+                    TC_TRACE(j, 25);
+                    tc_fence_after();
+                    for (int c = 0; c < n_chunks; ++c, ++q) {
+                        const uint32_t slot = q % (uint32_t)A_SLOTS;
+                        mbar_wait_sleep(bar(BAR_A_FULL + slot), (q / (uint32_t)A_SLOTS) & 1u);
+                        uint32_t b0;
+                        if (p.w1_resident) b0 = s_w1 + (uint32_t)c * HCHUNK;
+                        else {
+                            const uint32_t ws = q % W1_SLOTS;
+                            mbar_wait_sleep(bar(BAR_W1_FULL + ws), (q / W1_SLOTS) & 1u);
+                            b0 = s_w1 + ws * HCHUNK;
+                        }
+                        if (c == 0) TC_TRACE(j, 26);
+                        tc_fence_after();
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            umma_f16_ts(tm_acc1 + (uint32_t)(b * W), tm_ring + slot * 32u + (uint32_t)k * 8u,
+                                        smem_desc_sw128(b0 + (uint32_t)k * 32u), idesc, (uint32_t)((c | k) != 0));
+                        umma_commit(bar(BAR_A_EMPTY + slot));
+                        if (!p.w1_resident) umma_commit(bar(BAR_W1_EMPTY + (q % W1_SLOTS)));
+                    }
+                    umma_commit(bar(BAR_ACC_FULL + b));
+                    TC_TRACE(j, 27);
+                }
+            }
+        } else if (warp == TC_LOAD_WARP) {
+            // ======================= weights: global (L2) -> shared memory, cp.async.bulk ============
+            if (lane == 0) {
+                const uint32_t hid_total = (W <= 64) ? (p.w_bytes - p.w1_bytes) : 0u;
+                const uint32_t res_bytes = hid_total + (p.w1_resident ? p.w1_bytes : 0u);
+                if (res_bytes) {
+                    mbar_expect_tx(bar(BAR_WRES), res_bytes);
+                    for (uint32_t off = 0; off + 1u <= hid_total; off += 8192u) {
+                        const uint32_t nbytes = hid_total - off < 8192u ? hid_total - off : 8192u;
+                        bulk_g2s(s_whid + off, p.w_img + p.w1_bytes + off, nbytes, bar(BAR_WRES));
+                    }
+                    if (p.w1_resident)
+                        for (int c = 0; c < n_chunks; ++c)
+                            bulk_g2s(s_w1 + (uint32_t)c * HCHUNK, p.w_img + (size_t)c * HCHUNK, HCHUNK, bar(BAR_WRES));
+                } else {
+                    mbar_arrive(bar(BAR_WRES));
+                }
+                if (!p.w1_resident) {
+                    // layer-1 weight chunks stream through the ring in the order the MMA warp consumes them
+                    uint32_t q = 0;
+                    for (int j = 0;; ++j) {
+                        const int nb = j % TC_RAY_BUFS;
+                        mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
+                        if (s_tile[nb] < 0) break;
+                        for (int c = 0; c < n_chunks; ++c, ++q) {
+                            const uint32_t ws = q % W1_SLOTS;
+                            mbar_wait_sleep(bar(BAR_W1_EMPTY + ws), ((q / W1_SLOTS) & 1u) ^ 1u);
+                            mbar_expect_tx(bar(BAR_W1_FULL + ws), HCHUNK);
+                            bulk_g2s(s_w1 + ws * HCHUNK, p.w_img + (size_t)c * HCHUNK, HCHUNK, bar(BAR_W1_FULL + ws));
+                        }
+                    }
+                }
+            } else if (lane == 1 && W > 64) {
+                // W = 128: hidden layers 2..H and the output layer, KC chunks each, per tile, in the order the
+                // (single) tail group consumes them
+                const uint8_t* wh = p.w_img + p.w1_bytes;
+                uint32_t hq = 0;
+                for (int j = 0;; ++j) {
+                    const int nb = j % TC_RAY_BUFS;
+                    mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
+                    if (s_tile[nb] < 0) break;
+                    for (int l = 1; l <= p.hidden_layers; ++l) {
+                        const bool is_out = l == p.hidden_layers;
+                        const uint32_t bytes = is_out ? OUTCHUNK : HCHUNK;
+                        const uint8_t* src = wh + (size_t)(l - 1) * (size_t)(KC * HCHUNK);
+                        for (int kc = 0; kc < KC; ++kc, ++hq) {
+                            const uint32_t slot = hq % TC_HSLOTS;
+                            mbar_wait_sleep(bar(BAR_HEMPTY + slot), ((hq / TC_HSLOTS) & 1u) ^ 1u);
+                            mbar_expect_tx(bar(BAR_HFULL + slot), bytes);
+                            bulk_g2s(s_whid + slot * HCHUNK, src + (size_t)kc * bytes, bytes, bar(BAR_HFULL + slot));
+                        }
                     }
                 }
             }
+        } else {
+            // ======================= prep warps: tile ids, ray fetch, (a2) map back =====================
+            const int pt = tid - TC_PREP_WARP0 * 32;                       // 0..63, two rays each
+            unsigned next_t = 0;
+            if (pt == 0) next_t = atomicAdd(p.tile_counter, 1u);
+            int n_term = 0;
+            for (int j = 0;; ++j) {
+                const int nb = j % TC_RAY_BUFS;
+                mbar_wait_sleep(bar(BAR_RAY_EMPTY + nb), (uint32_t)(((j / TC_RAY_BUFS) & 1) ^ 1));
+                if (pt == 0) {
+                    const int t = (long long)next_t < n_tiles ? (int)next_t : -1;
+                    s_tile[nb] = t;
+                    if (t >= 0) next_t = atomicAdd(p.tile_counter, 1u);    // next tile's id: latency hidden behind this tile's loads
+                    TC_TRACE(j, 0);
+                }
+                named_bar_sync(3, TC_PREP_THREADS);
+                const int tile = s_tile[nb];
+                float* rbuf = ray_buf + (size_t)nb * TC_RAY_FIELDS * TC_TILE;
+#pragma unroll 1
+                for (int half = 0; half < 2; ++half) {
+                    const int r = pt + TC_PREP_THREADS * half;
+                    const long long h = tile < 0 ? n_hit : (long long)tile * TC_TILE + r;
+                    float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f, ti = 0.f, to = 0.f;
+                    long long ray = -1;
+                    if (h < n_hit) {
+                        ray = p.hit_list[h];
+                        ti = p.out.t_in[ray]; to = p.out.t_out[ray];
+                        const float ox = p.origin[3 * ray], oy = p.origin[3 * ray + 1], oz = p.origin[3 * ray + 2];
+                        const float dx = p.dir[3 * ray], dy = p.dir[3 * ray + 1], dz = p.dir[3 * ray + 2];
+                        if constexpr (LOCAL) {           // deformation given as a lattice: voxel-local inverse (R27)
+                            const float oo[3] = {ox, oy, oz}, dd[3] = {dx, dy, dz};
+                            float ri[3], ro[3];
+                            nif_map_back_pair<true>(nif_ray_map(p.map, p.batch, ray), p.out.voxel_id[ray], oo, dd, ti, to, ri, ro);
+                            xi = ri[0]; yi = ri[1]; zi = ri[2]; xo = ro[0]; yo = ro[1]; zo = ro[2];
+                        } else {
+                            float th = p.theta_max, bk = p.bend_k;
+                            if (p.batch.pose_id) {           // nif_query_poses: this ray's pose
+                                const NifPoseDesc* pd = p.batch.poses + p.batch.pose_id[ray];
+                                th = pd->theta_max; bk = pd->bend_k;
+                            }
+                            nif_inverse_deform(th, bk, fmaf(ti, dx, ox), fmaf(ti, dy, oy), fmaf(ti, dz, oz), xi, yi, zi);
+                            nif_inverse_deform(th, bk, fmaf(to, dx, ox), fmaf(to, dy, oy), fmaf(to, dz, oz), xo, yo, zo);
+                        }
+                    }
+                    rbuf[0 * TC_TILE + r] = nif_normalise(xi); rbuf[1 * TC_TILE + r] = nif_normalise(yi); rbuf[2 * TC_TILE + r] = nif_normalise(zi);
+                    rbuf[3 * TC_TILE + r] = nif_normalise(xo); rbuf[4 * TC_TILE + r] = nif_normalise(yo); rbuf[5 * TC_TILE + r] = nif_normalise(zo);
+                    rbuf[6 * TC_TILE + r] = ti; rbuf[7 * TC_TILE + r] = to; rbuf[8 * TC_TILE + r] = __int_as_float((int)ray);
+                }
+                mbar_arrive(bar(BAR_RAY_FULL + nb));
+                if (tile < 0 && ++n_term == NG) break;                     // every tail group sees its own end marker
+            }
         }
     } else {
-        // ======================= gather warps: (a3) encode into the A ring ======================
-        const int gw = warp - (TC_TMA_WARP + 1);
-        const int items_per_chunk = 4 * epc;
-        const int items_per_tile = items_per_chunk * n_chunks;
-        const int units_per_es = (L * F) / 8;                          // 16-byte units one sample fills
+        // ======================= gather warps: (a3) encode into the TMEM A ring =====================
+        reg_inc<TC_REGS_GATHER>();
+        const int gw = warp - TC_GATHER_WARP0;
+        const int g = gw & 3, qr = gw >> 2;                                // row group (= TMEM lane quarter), rank in the group
+        const uint32_t row = (uint32_t)(g * 32 + lane);
+        const uint32_t t_row = (uint32_t)(g * 32) << 16;
+        const int n_pairs = n_chunks * epc;                                // (endpoint, sample) slots per tile, padding included
+        const int units_per_es = (L * F) / 8;                              // 16-byte units (4 TMEM columns) one sample fills
         for (int j = 0;; ++j) {
-            const int b = j & 1;
-            mbar_wait(bar(BAR_RAY_FULL + b), (uint32_t)((j >> 1) & 1));
-            if (s_tile[b] < 0) break;
-            const long long gi0 = (long long)j * items_per_tile;
-            const int first = (int)(((long long)gw - gi0 % TC_GATHER_WARPS + TC_GATHER_WARPS) % TC_GATHER_WARPS);
-            for (int i = first; i < items_per_tile; i += TC_GATHER_WARPS) {
-                const int c = i / items_per_chunk, rem = i - c * items_per_chunk;
-                const int esl = rem >> 2, g = rem & 3;
-                const int es = c * epc + esl;
+            const int nb = j % TC_RAY_BUFS;
+            mbar_wait(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
+            if (s_tile[nb] < 0) break;
+            const float* rb = ray_buf + (size_t)nb * TC_RAY_FIELDS * TC_TILE + row;
+            const long long p0 = (long long)j * n_pairs;
+            const int first = (int)(((long long)qr - p0 % 4 + 4) % 4);
+            for (int e = first; e < n_pairs; e += 4) {
+                const int c = e / epc, esl = e - c * epc;
+                const int es = e;
                 const uint32_t q = (uint32_t)j * (uint32_t)n_chunks + (uint32_t)c;
-                const uint32_t stage = q % TC_STAGES;
-                mbar_wait(bar(BAR_EMPTY + stage), ((q / TC_STAGES) & 1u) ^ 1u);
-                const uint32_t row = (uint32_t)(g * 32 + lane);
-                const uint32_t a_stage = s_a + stage * STAGE_BYTES;
-                const uint32_t unit0 = (uint32_t)(esl * units_per_es);
-                if (p.flags & NIF_PROBE_SKIP_GATHER) {
-                    // diagnostic: synthetic features, no table access -- times the MLP pipeline alone
+                const uint32_t slot = q % (uint32_t)A_SLOTS;
+                mbar_wait(bar(BAR_A_EMPTY + slot), ((q / (uint32_t)A_SLOTS) & 1u) ^ 1u);
+                __syncwarp();                                              // tcgen05.st is .sync.aligned
+                tc_fence_after();
+                const uint32_t a_dst = tm_ring + slot * 32u + (uint32_t)(esl * units_per_es) * 4u + t_row;
+                if constexpr (PROBE) {
+                    // MLP-only probe: synthetic features, no table access
                     for (int u = 0; u < units_per_es; ++u)
-                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), 0x2c002c00u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u);
+                        tmem_st_32x4(a_dst + (uint32_t)u * 4u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u);
                 } else if (CONCAT && es >= 2 && es < p.n_es) {
                     // NIF_ENC_CONCAT: items 0, 1 are phi(entry), phi(exit); the rest carry the gamma scalars as
                     // they are: L*F = 32 -> two 32-column items per endpoint, L*F = 64 -> one 64-column item
                     const int pe_item = es - 2;
-                    const int e = (L * F == 32) ? pe_item >> 1 : pe_item;
+                    const int en = (L * F == 32) ? pe_item >> 1 : pe_item;
                     const int jbase = (L * F == 32) ? (pe_item & 1) * 32 : 0;
-                    const float* rb = ray_buf + ((size_t)b * TC_TILE + row) * 8 + 3 * e;
-                    const float xr[3] = {rb[0], rb[1], rb[2]};
+                    const float xr[3] = {rb[(3 * en) * TC_TILE], rb[(3 * en + 1) * TC_TILE], rb[(3 * en + 2) * TC_TILE]};
                     for (int u = 0; u < units_per_es; ++u) {
                         float v[8];
 #pragma unroll
                         for (int i = 0; i < 8; ++i) v[i] = nif_pe_scalar(xr, jbase + 8 * u + i, p.enc.bands);
-                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), pack_half2(v[0], v[1]), pack_half2(v[2], v[3]),
+                        tmem_st_32x4(a_dst + (uint32_t)u * 4u, pack_half2(v[0], v[1]), pack_half2(v[2], v[3]),
                                      pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
                     }
                 } else if (es < p.n_es) {
-                    const int e = CONCAT ? es : (es >= S ? 1 : 0);
-                    const int s = CONCAT ? 0 : es - e * S;
-                    const float* rb = ray_buf + ((size_t)b * TC_TILE + row) * 8 + 3 * e;
-                    const float px = nif_pe_sample(rb[0], s), py = nif_pe_sample(rb[1], s), pz = nif_pe_sample(rb[2], s);
+                    const int en = CONCAT ? es : (es >= S ? 1 : 0);
+                    const int s = CONCAT ? 0 : es - en * S;
+                    const float px = nif_pe_sample(rb[(3 * en) * TC_TILE], s), py = nif_pe_sample(rb[(3 * en + 1) * TC_TILE], s),
+                                pz = nif_pe_sample(rb[(3 * en + 2) * TC_TILE], s);
                     GatherBatch<F> ba, bb;                                     // two batches in flight
                     constexpr int NL = GatherBatch<F>::NL;
                     ba.issue(p.table, s_lvl, p.enc.log2_T, 0, px, py, pz);
@@ -655,25 +763,26 @@ k_fused_encode_mlp(const TcParams p)
                         ba.consume(pk[0], pk[1]);
                         if (u + 1 < units_per_es) ba.issue(p.table, s_lvl, p.enc.log2_T, (2 * u + 2) * NL, px, py, pz);
                         bb.consume(pk[2], pk[3]);
-                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), pk[0], pk[1], pk[2], pk[3]);
+                        __syncwarp();
+                        tmem_st_32x4(a_dst + (uint32_t)u * 4u, pk[0], pk[1], pk[2], pk[3]);
                     }
                 } else {
-                    for (int u = 0; u < units_per_es; ++u)
-                        st_shared_v4(a_stage + sw128_off(row, unit0 + (uint32_t)u), 0u, 0u, 0u, 0u);
+                    for (int u = 0; u < units_per_es; ++u) tmem_st_32x4(a_dst + (uint32_t)u * 4u, 0u, 0u, 0u, 0u);
                 }
-                fence_proxy_async();
+                tmem_st_wait();
+                tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(BAR_FULL + stage));
+                if (lane == 0) mbar_arrive(bar(BAR_A_FULL + slot));
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar(BAR_RAY_EMPTY + b));
+            if (lane == 0) mbar_arrive(bar(BAR_RAY_EMPTY + nb));
         }
     }
 
     // ---- teardown --------------------------------------------------------------------------------
     tc_fence_before();
     __syncthreads();
-    if (warp == TC_MMA_WARP) { tc_fence_after(); tmem_dealloc(tmem_base, TMEM_COLS); }
+    if (warp == TC_MMA_WARP) { tc_fence_after(); __syncwarp(); tmem_dealloc(tmem_base, TMEM_COLS); }
 }
 
 // ---- weight repacking: row-major (fan_out, fan_in) fp16 -> K-major SWIZZLE_128B B-operand images ----
@@ -716,28 +825,46 @@ TcShape tc_shape(const nif_net_desc* d)
     return s;
 }
 
-constexpr uint32_t TC_MAX_SMEM = 227u * 1024u;
-
-// ring depth: always the full 4-stage ring (W = 32 / 64: 118 / 139 KB, inside the L1-friendly 164 KB carve-out of
-// DESIGN.md 7.3; W = 128: 200 KB).  Shallower rings were measured slower (7.7) and a forced 3-stage ring at
-// W = 128 failed at launch on full-size config 4 in an experiment that was not investigated further, so no other
-// depth is ever selected; a device without enough shared memory gets the FFMA engine instead.
-int tc_pick_stages(int W)
+// Shared-memory budget: 163 KB keeps the kernel inside the 164 KB carve-out, which leaves the L1 data cache
+// large enough to keep the gathers' misses in flight.  Layer-1 weights are resident when
+// everything fits that budget (config 1-3: 104 KB + 18 KB + 14 KB), otherwise they stream through as many
+// chunk slots as fit (4..8).
+#ifndef NIF_TC_SMEM_BUDGET
+#define NIF_TC_SMEM_BUDGET (163u * 1024u)
+#endif
+struct TcW1Plan { int slots, resident; };
+TcW1Plan tc_plan_w1(int W, int hidden_layers, int n_chunks)
 {
-    return tc_smem_layout(TC_MAX_STAGES, W).total <= TC_MAX_SMEM ? TC_MAX_STAGES : 0;
+    const uint32_t fixed = tc_smem_layout(W, hidden_layers, 0).total;
+    const uint32_t chunk = (uint32_t)W * 128u;
+#ifndef NIF_TC_FORCE_STREAM
+    if (fixed + (uint32_t)n_chunks * chunk <= NIF_TC_SMEM_BUDGET) return TcW1Plan{n_chunks, 1};
+#endif
+    int slots = fixed < NIF_TC_SMEM_BUDGET ? (int)((NIF_TC_SMEM_BUDGET - fixed) / chunk) : 0;
+    if (slots > TC_MAX_W1_SLOTS) slots = TC_MAX_W1_SLOTS;
+    if (slots > n_chunks) slots = n_chunks;
+    if (slots < 2 && slots < n_chunks) return TcW1Plan{0, 0};
+    return TcW1Plan{slots, 0};
 }
 
-template <int W, int F, bool CONCAT, bool LOCAL>
+template <int W, int F, bool CONCAT, bool LOCAL, bool PROBE>
 int launch_tc(const TcParams& p, uint32_t smem, int blocks, cudaStream_t stream)
 {
-    NIF_CUDA_TRY(cudaFuncSetAttribute(k_fused_encode_mlp<W, F, CONCAT, LOCAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_fused_encode_mlp<W, F, CONCAT, LOCAL><<<blocks, TC_THREADS, smem, stream>>>(p);
+    NIF_CUDA_TRY(cudaFuncSetAttribute(k_fused_encode_mlp<W, F, CONCAT, LOCAL, PROBE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_fused_encode_mlp<W, F, CONCAT, LOCAL, PROBE><<<blocks, TC_THREADS, smem, stream>>>(p);
     nif_count_launch(1);
     NIF_CUDA_TRY(cudaGetLastError());
     return NIF_OK;
 }
 
 }  // namespace
+
+#ifdef NIF_TC_TRACE
+extern "C" int nif_debug_set_tc_trace(void* buf)
+{
+    return cudaMemcpyToSymbol(g_tc_trace, &buf, sizeof(buf)) == cudaSuccess ? 0 : -5;
+}
+#endif
 
 int nif_tc_supported(const nif_net_desc* d)
 {
@@ -749,8 +876,9 @@ int nif_tc_supported(const nif_net_desc* d)
     if (d->enc_mode == NIF_ENC_CONCAT && ((lf != 32 && lf != 64) || 3 + 6 * d->pe_bands > 64)) return 0;
     if (d->hidden_layers < 1) return 0;
     const TcShape s = tc_shape(d);
-    (void)s;
-    return tc_pick_stages(d->width) >= 2 ? 1 : 0;
+    if (d->width <= 64 && tc_smem_layout(d->width, d->hidden_layers, 2).total > NIF_TC_SMEM_BUDGET) return 0;   // resident hidden weights
+    const TcW1Plan plan = tc_plan_w1(d->width, d->hidden_layers, s.n_chunks);
+    return (plan.resident && plan.slots >= 1) || plan.slots >= 2 ? 1 : 0;
 }
 
 int nif_tc_pack_weights(nif_net* net, cudaStream_t stream)
@@ -797,21 +925,22 @@ int nif_launch_fused_tc(const nif_bvh* bvh, const nif_net* net, const nif_ray_ba
     p.origin = rays->origin; p.dir = rays->dir;
     p.out = *out; p.scratch = scratch; p.tile_counter = &scratch->pad[4]; p.hit_list = hit_list; p.flags = flags;
     p.enc_mode = d->enc_mode;
-    p.stages = tc_pick_stages(d->width);
-    const uint32_t smem = tc_smem_layout(p.stages, d->width).total;
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        NIF_CUDA_TRY(cudaGetDevice(&dev));
-        NIF_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    }
+    const TcW1Plan plan = tc_plan_w1(d->width, d->hidden_layers, s.n_chunks);
+    p.w1_slots = plan.slots; p.w1_resident = plan.resident;
+    const uint32_t smem = tc_smem_layout(d->width, d->hidden_layers, plan.slots).total;
+    const int n_sm = nif_sm_count();
+    if (n_sm <= 0) return NIF_ERR_CUDA;
     const long long max_tiles = (rays->n + TC_TILE - 1) / TC_TILE;
     const int blocks = (int)(max_tiles < n_sm ? max_tiles : n_sm);
     // the concatenation variant is its own instantiation so that the composition kernel's code is untouched
-#define NIF_TC_CASE(WW, FF) if (d->width == WW && d->feat == FF) \
+    // the MLP-only probe (NIF_PROBE_SKIP_GATHER) is its own instantiation of the composition kernel
+#define NIF_TC_CASE(WW, FF) if (d->width == WW && d->feat == FF) { \
+        if (flags & NIF_PROBE_SKIP_GATHER) \
+            return d->enc_mode == NIF_ENC_CONCAT ? launch_tc<WW, FF, true, false, true>(p, smem, blocks, stream) \
+                                                 : launch_tc<WW, FF, false, false, true>(p, smem, blocks, stream); \
         return d->enc_mode == NIF_ENC_CONCAT \
-            ? (bvh->local_inverse ? launch_tc<WW, FF, true, true>(p, smem, blocks, stream) : launch_tc<WW, FF, true, false>(p, smem, blocks, stream)) \
-            : (bvh->local_inverse ? launch_tc<WW, FF, false, true>(p, smem, blocks, stream) : launch_tc<WW, FF, false, false>(p, smem, blocks, stream))
+            ? (bvh->local_inverse ? launch_tc<WW, FF, true, true, false>(p, smem, blocks, stream) : launch_tc<WW, FF, true, false, false>(p, smem, blocks, stream)) \
+            : (bvh->local_inverse ? launch_tc<WW, FF, false, true, false>(p, smem, blocks, stream) : launch_tc<WW, FF, false, false, false>(p, smem, blocks, stream)); }
     NIF_TC_CASE(32, 2); NIF_TC_CASE(64, 2); NIF_TC_CASE(128, 2);
     NIF_TC_CASE(32, 4); NIF_TC_CASE(64, 4); NIF_TC_CASE(128, 4);
 #undef NIF_TC_CASE

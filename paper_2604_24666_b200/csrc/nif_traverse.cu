@@ -584,12 +584,8 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
                         const NifPoseBatch* batch)
 {
     if (rays->n == 0) return NIF_OK;
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        NIF_CUDA_TRY(cudaGetDevice(&dev));
-        NIF_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    }
+    const int n_sm = nif_sm_count();
+    if (n_sm <= 0) return NIF_ERR_CUDA;
     TravParams p;
     p.nodes = bvh->nodes; p.lat = bvh->lattice; p.nv = bvh->nv; p.root = bvh->root;
     p.rlx = bvh->lo[0]; p.rly = bvh->lo[1]; p.rlz = bvh->lo[2];

@@ -104,12 +104,8 @@ extern "C" int nif_query_multi(const nif_bvh* bvh, const nif_net* net, const nif
     NIF_CUDA_TRY(cudaMemsetAsync(walk->steps, 0, n * 4, stream));
     NIF_CUDA_TRY(cudaMemsetAsync(walk->dist_accum, 0, n * 4, stream));
 
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        NIF_CUDA_TRY(cudaGetDevice(&dev));
-        NIF_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    }
+    const int n_sm = nif_sm_count();
+    if (n_sm <= 0) return NIF_ERR_CUDA;
     const bool use_tc = net->desc.dtype == NIF_F16 && net->tc_supported && !(flags & NIF_ENGINE_FFMA);
     for (int round = 0; round < max_steps; ++round) {
         NifWalkRound wr;
