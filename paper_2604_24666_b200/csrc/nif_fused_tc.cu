@@ -51,6 +51,7 @@ constexpr int TC_THREADS = 32 * (TC_GATHER_WARP0 + TC_GATHER_WARPS);      // 896
 constexpr int TC_RAY_BUFS = 3;               // ray_buf depth: prep runs up to two tiles ahead of the tails
 constexpr int TC_RAY_FIELDS = 9;             // xi yi zi xo yo zo t_in t_out ray
 constexpr int TC_MAX_A_SLOTS = 8;            // layer-1 A chunk slots in TMEM (32 columns each)
+constexpr int TC_A_GROUP = 1;                // chunks per full/empty barrier pair of the A ring
 constexpr int TC_MAX_W1_SLOTS = 8;           // layer-1 weight chunk slots when W1 streams
 constexpr int TC_HSLOTS = 2;                 // hidden/output weight chunk ring (W = 128)
 constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded to the UMMA minimum)
@@ -130,6 +131,60 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, ui
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
         "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// One K chunk in ONE asm block: NK UMMAs over consecutive K = 16 slices (A: +8 TMEM columns, B: +32 bytes =
+// +2 in the descriptor's address field) and the commit that releases the chunk.  A single thread issues
+// every MMA of the kernel, so its instruction count per MMA is what bounds the tensor pipe on small
+// layers: one block keeps the descriptor arithmetic to one add per operand and the compiler's
+// elect-one-thread wrapper small.  commit_bar == 0 (NK = 4 only): no commit.
+template <int NK>
+__device__ __forceinline__ void umma_chunk_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
+                                              uint32_t accumulate_first, uint32_t commit_bar)
+{
+    static_assert(NK == 1 || NK == 2 || NK == 4, "K = 16, 32 or 64 per chunk");
+    if constexpr (NK == 4) {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 a1, a2, a3;\n\t"
+            ".reg .b64 b1, b2, b3;\n\t"
+            ".reg .pred cq;\n\t"
+            "setp.ne.b32 p, %4, 0;\n\t"
+            "setp.ne.b32 cq, %5, 0;\n\t"
+            "add.u32 a1, %1, 8;\n\t"
+            "add.u32 a2, %1, 16;\n\t"
+            "add.u32 a3, %1, 24;\n\t"
+            "add.u64 b1, %2, 2;\n\t"
+            "add.u64 b2, %2, 4;\n\t"
+            "add.u64 b3, %2, 6;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a1], b1, %3, 1;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a2], b2, %3, 1;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a3], b3, %3, 1;\n\t"
+            "@cq tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
+            "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate_first), "r"(commit_bar) : "memory");
+    } else if constexpr (NK == 2) {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 a1;\n\t"
+            ".reg .b64 b1;\n\t"
+            "setp.ne.b32 p, %4, 0;\n\t"
+            "add.u32 a1, %1, 8;\n\t"
+            "add.u64 b1, %2, 2;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a1], b1, %3, 1;\n\t"
+            "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
+            "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate_first), "r"(commit_bar) : "memory");
+    } else {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "setp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+            "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
+            "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate_first), "r"(commit_bar) : "memory");
+    }
 }
 // all previously issued MMAs of this thread arrive on `bar` when they complete (implies fence::before_thread_sync)
 __device__ __forceinline__ void umma_commit(uint32_t bar)
@@ -428,7 +483,8 @@ k_fused_encode_mlp(const TcParams p)
     constexpr uint32_t C_RING = C_ACT + NG * ACT_COLS;
     constexpr int A_SLOTS = (512 - (int)C_RING) / 32 < TC_MAX_A_SLOTS ? (512 - (int)C_RING) / 32 : TC_MAX_A_SLOTS;
     constexpr uint32_t TMEM_COLS = 512;
-    static_assert(A_SLOTS >= 4, "layer-1 A ring too short");
+    constexpr int A_GROUPS = A_SLOTS / TC_A_GROUP;                         // ring = A_GROUPS groups of TC_A_GROUP chunk slots
+    static_assert(A_GROUPS >= 2, "layer-1 A ring too short");
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -449,7 +505,7 @@ k_fused_encode_mlp(const TcParams p)
 
     // ---- one-time setup ------------------------------------------------------------------------
     if (tid == 0) {
-        for (int i = 0; i < TC_MAX_A_SLOTS; ++i) { mbar_init(bar(BAR_A_FULL + i), 4u * (uint32_t)epc); mbar_init(bar(BAR_A_EMPTY + i), 1); }
+        for (int i = 0; i < TC_MAX_A_SLOTS; ++i) { mbar_init(bar(BAR_A_FULL + i), 4u * (uint32_t)epc * TC_A_GROUP); mbar_init(bar(BAR_A_EMPTY + i), 1); }
         for (int i = 0; i < TC_MAX_W1_SLOTS; ++i) { mbar_init(bar(BAR_W1_FULL + i), 1); mbar_init(bar(BAR_W1_EMPTY + i), 1); }
         for (int i = 0; i < TC_HSLOTS; ++i) { mbar_init(bar(BAR_HFULL + i), 1); mbar_init(bar(BAR_HEMPTY + i), 1); }
         for (int i = 0; i < 2; ++i) {
@@ -504,13 +560,11 @@ k_fused_encode_mlp(const TcParams p)
                         tc_fence_after();
                         wchunk = s_whid + slot * HCHUNK;
                     }
-#pragma unroll
-                    for (int k = 0; k < K16; ++k)
-                        umma_f16_ts(d_tmem, tm_act + (uint32_t)(kc * 32 + k * 8), smem_desc_sw128(wchunk + (uint32_t)k * 32u),
-                                    idesc, (uint32_t)((kc | k) != 0));
-                    if constexpr (W > 64) { umma_commit(bar(BAR_HEMPTY + (hq % TC_HSLOTS))); ++hq; }
+                    // the chunk's commit releases the weight slot (W = 128) or, on the last chunk, signals the layer
+                    const uint32_t cbar = (W > 64 && kc + 1 < KC) ? bar(BAR_HEMPTY + (hq % TC_HSLOTS)) : bar(BAR_HID + g);
+                    umma_chunk_ts<K16>(d_tmem, tm_act + (uint32_t)(kc * 32), smem_desc_sw128(wchunk), idesc, (uint32_t)(kc != 0), cbar);
+                    if constexpr (W > 64) { if (kc + 1 == KC) umma_commit(bar(BAR_HEMPTY + (hq % TC_HSLOTS))); ++hq; }
                 }
-                umma_commit(bar(BAR_HID + g));
             };
             for (int j = g;; j += NG) {
                 const int nb = j % TC_RAY_BUFS, b = j & 1;
@@ -569,7 +623,11 @@ k_fused_encode_mlp(const TcParams p)
             if (lane == 0) {
                 const uint32_t idesc = idesc_f16(TC_TILE, W);
                 if (p.w1_resident) mbar_wait_sleep(bar(BAR_WRES), 0);
-                uint32_t q = 0;
+                // A chunks are handed over in GROUPS of TC_A_GROUP chunks (one full/empty barrier pair per
+                // group): a try_wait costs ~90 cycles even when the phase is complete, and this one thread's
+                // instruction stream is what bounds the tensor pipe on 64-wide layers
+                const uint64_t w1_desc0 = smem_desc_sw128(s_w1);
+                uint32_t gs = 0, gph = 0, wq = 0;                         // group slot + phase; streamed-W1 chunk counter
                 for (int j = 0;; ++j) {
                     const int nb = j % TC_RAY_BUFS, b = j & 1;
                     mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
@@ -577,24 +635,33 @@ k_fused_encode_mlp(const TcParams p)
                     mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
                     TC_TRACE(j, 25);
                     tc_fence_after();
-                    for (int c = 0; c < n_chunks; ++c, ++q) {
-                        const uint32_t slot = q % (uint32_t)A_SLOTS;
-                        mbar_wait_sleep(bar(BAR_A_FULL + slot), (q / (uint32_t)A_SLOTS) & 1u);
-                        uint32_t b0;
-                        if (p.w1_resident) b0 = s_w1 + (uint32_t)c * HCHUNK;
-                        else {
-                            const uint32_t ws = q % W1_SLOTS;
-                            mbar_wait_sleep(bar(BAR_W1_FULL + ws), (q / W1_SLOTS) & 1u);
-                            b0 = s_w1 + ws * HCHUNK;
-                        }
-                        if (c == 0) TC_TRACE(j, 26);
+                    const uint32_t d_tmem = tm_acc1 + (uint32_t)(b * W);
+                    for (int c0 = 0; c0 < n_chunks; c0 += TC_A_GROUP) {
+#ifdef NIF_TC_EXP_NOWAIT
+                        if (!PROBE)
+#endif
+                        mbar_wait_sleep(bar(BAR_A_FULL + gs), gph);
+                        if (c0 == 0) TC_TRACE(j, 26);
                         tc_fence_after();
 #pragma unroll
-                        for (int k = 0; k < 4; ++k)
-                            umma_f16_ts(tm_acc1 + (uint32_t)(b * W), tm_ring + slot * 32u + (uint32_t)k * 8u,
-                                        smem_desc_sw128(b0 + (uint32_t)k * 32u), idesc, (uint32_t)((c | k) != 0));
-                        umma_commit(bar(BAR_A_EMPTY + slot));
-                        if (!p.w1_resident) umma_commit(bar(BAR_W1_EMPTY + (q % W1_SLOTS)));
+                        for (int ci = 0; ci < TC_A_GROUP; ++ci) {
+                            const int c = c0 + ci;
+                            if (c < n_chunks) {
+                                const bool last = (ci + 1 == TC_A_GROUP) || (c + 1 == n_chunks);
+                                uint64_t bdesc;
+                                if (p.w1_resident) bdesc = w1_desc0 + (uint64_t)((uint32_t)c * (HCHUNK >> 4));
+                                else {
+                                    const uint32_t ws = wq % W1_SLOTS;
+                                    mbar_wait_sleep(bar(BAR_W1_FULL + ws), (wq / W1_SLOTS) & 1u);
+                                    tc_fence_after();
+                                    bdesc = w1_desc0 + (uint64_t)(ws * (HCHUNK >> 4));
+                                }
+                                umma_chunk_ts<4>(d_tmem, tm_ring + (gs * TC_A_GROUP + (uint32_t)ci) * 32u, bdesc, idesc,
+                                                 (uint32_t)(c != 0), last ? bar(BAR_A_EMPTY + gs) : 0u);
+                                if (!p.w1_resident) { umma_commit(bar(BAR_W1_EMPTY + (wq % W1_SLOTS))); ++wq; }
+                            }
+                        }
+                        if (++gs == (uint32_t)A_GROUPS) { gs = 0; gph ^= 1u; }
                     }
                     umma_commit(bar(BAR_ACC_FULL + b));
                     TC_TRACE(j, 27);
@@ -678,6 +745,9 @@ k_fused_encode_mlp(const TcParams p)
                     const long long h = tile < 0 ? n_hit : (long long)tile * TC_TILE + r;
                     float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f, ti = 0.f, to = 0.f;
                     long long ray = -1;
+#ifdef NIF_TC_EXP_NOPREP
+                    if (PROBE && h < n_hit) { ray = h; } else
+#endif
                     if (h < n_hit) {
                         ray = p.hit_list[h];
                         ti = p.out.t_in[ray]; to = p.out.t_out[ray];
@@ -713,7 +783,8 @@ k_fused_encode_mlp(const TcParams p)
         const int g = gw & 3, qr = gw >> 2;                                // row group (= TMEM lane quarter), rank in the group
         const uint32_t row = (uint32_t)(g * 32 + lane);
         const uint32_t t_row = (uint32_t)(g * 32) << 16;
-        const int n_pairs = n_chunks * epc;                                // (endpoint, sample) slots per tile, padding included
+        const int n_groups = (n_chunks + TC_A_GROUP - 1) / TC_A_GROUP;    // chunk groups per tile (the last may be short)
+        const int n_pairs = n_groups * TC_A_GROUP * epc;                   // (endpoint, sample) slots per tile, padding included
         const int units_per_es = (L * F) / 8;                              // 16-byte units (4 TMEM columns) one sample fills
         for (int j = 0;; ++j) {
             const int nb = j % TC_RAY_BUFS;
@@ -722,13 +793,21 @@ k_fused_encode_mlp(const TcParams p)
             const float* rb = ray_buf + (size_t)nb * TC_RAY_FIELDS * TC_TILE + row;
             const long long p0 = (long long)j * n_pairs;
             const int first = (int)(((long long)qr - p0 % 4 + 4) % 4);
+#ifdef NIF_TC_EXP_NOWAIT
+            if (PROBE) { __syncwarp(); if (lane == 0) mbar_arrive(bar(BAR_RAY_EMPTY + nb)); continue; }
+#endif
             for (int e = first; e < n_pairs; e += 4) {
                 const int c = e / epc, esl = e - c * epc;
                 const int es = e;
-                const uint32_t q = (uint32_t)j * (uint32_t)n_chunks + (uint32_t)c;
-                const uint32_t slot = q % (uint32_t)A_SLOTS;
-                mbar_wait(bar(BAR_A_EMPTY + slot), ((q / (uint32_t)A_SLOTS) & 1u) ^ 1u);
+                const uint32_t gq = (uint32_t)j * (uint32_t)n_groups + (uint32_t)(c / TC_A_GROUP);   // group counter
+                const uint32_t gs = gq % (uint32_t)A_GROUPS;
+                const uint32_t slot = gs * TC_A_GROUP + (uint32_t)(c % TC_A_GROUP);
+                mbar_wait(bar(BAR_A_EMPTY + gs), ((gq / (uint32_t)A_GROUPS) & 1u) ^ 1u);
                 __syncwarp();                                              // tcgen05.st is .sync.aligned
+                if (c >= n_chunks) {                                       // padding chunk of a short last group: arrival only
+                    if (lane == 0) mbar_arrive(bar(BAR_A_FULL + gs));
+                    continue;
+                }
                 tc_fence_after();
                 const uint32_t a_dst = tm_ring + slot * 32u + (uint32_t)(esl * units_per_es) * 4u + t_row;
                 if constexpr (PROBE) {
@@ -772,7 +851,7 @@ k_fused_encode_mlp(const TcParams p)
                 tmem_st_wait();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(BAR_A_FULL + slot));
+                if (lane == 0) mbar_arrive(bar(BAR_A_FULL + gs));
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(BAR_RAY_EMPTY + nb));
