@@ -38,12 +38,58 @@ import nif_inputs as I  # noqa: E402
 METRIC = "Mrays/s neural intersection query on 1 B200; tensor-pipe % of peak (MLP)"
 UNIT = "Mrays/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# `ncu --set full` capture named beside it (profiles/); None until a capture exists.
-NCU_TRAFFIC = {
-    # config id: (bytes per launch, profile file)
-    1: (33_850_000, "profiles/fused_encode_mlp_r1.md"),
+
+
+def whole_job_value(world: int, units_per_rank: int, ms_per_step_max_over_ranks: float) -> float:
+    """metric of the whole job: units all ranks processed / the slowest rank's time (Mrays/s)"""
+    return world * units_per_rank / (ms_per_step_max_over_ranks * 1e-3) / 1e6
+
+
+def max_over_ranks(value: float, dist=None, device=None) -> float:
+    """max of a per-rank scalar over all ranks (identity for a single process); works with nccl and gloo"""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+NCU_METRICS = {  # name in the roofline object -> ncu metric (raw page)
+    "l1_wavefronts": "l1tex__data_pipe_lsu_wavefronts.sum",
+    "l1_sectors_global_ld": "l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum",
+    "l2_sectors": "lts__t_sectors_srcunit_tex.sum",          # sectors the L1s requested from L2
+    "dram_bytes_read": "dram__bytes_read.sum",
+    "dram_bytes_write": "dram__bytes_write.sum",
+    "tensor_pipe_pct": "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active",
+    "duration_us_under_ncu": "gpu__time_duration.sum",
 }
+_UNIT_SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "sector": 1.0, "": 1.0, "%": 1.0, "us": 1.0,
+               "ns": 1e-3, "ms": 1e3, "inst": 1.0, "cycle": 1.0}
+
+
+def ncu_counts(cfg_id: int, enc: str) -> dict | None:
+    """Per-launch counters of the dominant kernel from the committed `ncu --set full` export
+    profiles/fused_cfg<id>_r2_raw.csv (made with `bench.py --config <id> --profile-only`, see the .md beside it)."""
+    import csv
+    f = ROOT / "profiles" / (f"fused_cfg{cfg_id}_r2_raw.csv" if enc == "compose" else f"fused_cfg{cfg_id}_{enc}_r2_raw.csv")
+    if not f.exists():
+        return None
+    rows = list(csv.reader(f.open()))
+    hdr, units, vals = rows[0], rows[1], rows[2]
+    out = {"file": str(f.relative_to(ROOT))}
+    run = f.with_name(f.name.replace("_raw.csv", "_run.txt"))        # the --profile-only line of the captured run
+    if run.exists():
+        out["hit_rays_per_launch"] = json.loads(run.read_text())["hit_rays_per_launch"]
+    for key, metric in NCU_METRICS.items():
+        if metric in hdr:
+            i = hdr.index(metric)
+            out[key] = float(vals[i].replace(",", "")) * _UNIT_SCALE.get(units[i], 1.0)
+    # the LSU data-pipe wavefront count is exported per L1 (one per SM) as an average
+    per_sm, n_sm = "SM_A.TriageCompute.l1tex__data_pipe_lsu_wavefronts.avg", "device__attribute_multiprocessor_count"
+    if "l1_wavefronts" not in out and per_sm in hdr and n_sm in hdr:
+        out["l1_wavefronts"] = float(vals[hdr.index(per_sm)].replace(",", "")) * float(vals[hdr.index(n_sm)])
+    return out
 
 
 def measured_peaks() -> dict:
@@ -173,17 +219,31 @@ class OracleRun:
         return time.perf_counter() - t0
 
 
-def cpu_baseline(cfg: I.Config, variant: str, budget_s: float = 15.0) -> dict:
+def cpu_baseline(cfg: I.Config, variant: str, budget_s: float = 12.0) -> dict:
+    """The oracle as it stands on this box's host cores: one core on a bounded, evenly spread
+    sample of the frame, then the same single-threaded function over disjoint ray ranges on every core this
+    process may use (oracle/pool.py)."""
+    from oracle.pool import OraclePool, cpu_model, n_cores
     run = OracleRun(cfg, variant)
     o, d, stride = run.sample(4096)
     t = run.time_query(o, d)                         # calibration pass
     n_sample = int(min(len(run.origin), max(4096, 4096 * budget_s / max(t, 1e-3))))
     n_sample = 1 << int(np.floor(np.log2(n_sample)))
     o, d, stride = run.sample(n_sample)
-    t = run.time_query(o, d)
-    return {"value": len(o) / t / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"every {stride:.1f}th ray of the frame ({len(o)} rays, hits and misses), "
-                      f"single thread, {t:.1f} s; oracle/nif_oracle.c as it stands (gcc -O2, fp32)"}
+    t1 = run.time_query(o, d)
+    one = len(o) / t1 / 1e6
+    cores = n_cores()
+    with OraclePool(cfg.nv, run.occ, run.pose, run.lat, run.params) as pool:
+        oa, da, stride_a = run.sample(min(len(run.origin), n_sample * min(cores, 16)))
+        pool.query(oa[:4096], da[:4096], occlusion_only=cfg.occlusion_only)      # workers up, libraries loaded
+        t0 = time.perf_counter()
+        pool.query(oa, da, occlusion_only=cfg.occlusion_only)
+        ta = time.perf_counter() - t0
+    return {"value": len(oa) / ta / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": cpu_model(),
+            "one_core": {"value": one, "unit": UNIT, "cores": 1,
+                         "sample": f"every {stride:.1f}th ray of the frame ({len(o)} rays, hits and misses), {t1:.1f} s"},
+            "sample": f"every {stride_a:.1f}th ray of the frame ({len(oa)} rays, hits and misses) split over {cores} worker "
+                      f"processes, each running the single-threaded oracle/nif_oracle.c as it stands (gcc -O2, fp32), {ta:.1f} s"}
 
 
 def run_reference(args) -> None:
@@ -242,7 +302,7 @@ def run_ours(args) -> None:
     occ_d = torch.from_numpy(occ).to(dev)
 
     # one BVH + one ray batch per pose ("for each deformation pose, we build a simple BVH");
-    # every rank traces the whole workload with its own ray seed offset = weak scaling
+    # every rank traces the whole workload (the same seeded frame: independent replicas) = weak scaling
     poses, build_ms = [], []
     for pi in range(cfg.n_poses):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -305,29 +365,41 @@ def run_ours(args) -> None:
         n_hit += nif.nif_query_last_hit_count(w_)
 
     # ---- timed region: K steps, device-timed, inputs resident in HBM -------------------------
+    # (no per-kernel events in here: those are collected in a separate pass below)
     sampler = ClockSampler(physical_gpu_index(local_rank))
-    nif.nif_profile_enable(True)
     launches0 = nif.nif_kernel_launch_count()
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     sync_all()
     sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
+    marks[0].record()
+    for i in range(args.steps):
         step()
-    e1.record()
+        marks[i + 1].record()
     sync_all()
     clocks = sampler.stop()
-    elapsed_ms = e0.elapsed_time(e1)
+    elapsed_ms = marks[0].elapsed_time(marks[-1])
+    step_ms = [marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps)]
     launches = nif.nif_kernel_launch_count() - launches0
+    elapsed_ms = max_over_ranks(elapsed_ms, dist if world > 1 else None, dev)
+    ms_per_step = elapsed_ms / args.steps
+    value = whole_job_value(world, n_total, ms_per_step)
+    launches_per_query = 1 if batched else cfg.n_poses     # per-kernel times below are per query launch
+
+    # ---- per-kernel times: the same steps again with the library's event hooks switched on -------
+    nif.nif_profile_enable(True)
+    for _ in range(max(3, min(args.steps, 10))):
+        step()
     prof = nif.nif_profile_read()
     nif.nif_profile_enable(False)
-    if world > 1:
-        t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(t.item())
-    ms_per_step = elapsed_ms / args.steps
-    value = world * n_total / (ms_per_step * 1e-3) / 1e6
-    launches_per_query = 1 if batched else cfg.n_poses     # per-kernel times below are per query launch
+    if args.profile_only:
+        if rank == 0:
+            print(json.dumps({"profile_only": True, "config": workload_name(cfg), "ms_per_step": ms_per_step,
+                              "hit_rays_per_step": n_hit, "hit_rays_per_launch": n_hit / launches_per_query,
+                              "encode_mlp_ms": prof["network_ms"] / max(prof["n_queries"], 1),
+                              "traverse_ms": prof["traverse_ms"] / max(prof["n_queries"], 1)}), flush=True)
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     walk_stats = None
     if args.walk:
@@ -346,7 +418,7 @@ def run_ours(args) -> None:
                 ws = nif.nif_query(p["bvh"], net, p["o"], p["d"], out, workspace=ws, flags=flags | nif.NIF_PROBE_SKIP_GATHER)
         pr = nif.nif_profile_read()
         nif.nif_profile_enable(False)
-        mlp_probe = pr["network_ms"] / max(pr["n_queries"], 1)
+        mlp_probe = pr["network_ms"] / max(pr["n_queries"], 1)          # per nif_query launch = per pose
         for p in poses:                                # leave real results in `out`
             ws = nif.nif_query(p["bvh"], net, p["o"], p["d"], out, workspace=ws, flags=flags)
         torch.cuda.synchronize()
@@ -364,11 +436,8 @@ def run_ours(args) -> None:
         for p in poses:
             nif.nif_query_host(p["bvh"], net, stage, p["o_h"], p["d_h"], out_h, flags=flags)   # synchronises
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_value = world * n_total * e2e_steps / e2e_s / 1e6
+    e2e_s = max_over_ranks(e2e_s, dist if world > 1 else None, dev)
+    e2e_value = whole_job_value(world, n_total, e2e_s / e2e_steps * 1e3)
     work = algorithmic_work(cfg)
     h2d = n_total * work["hbm_bytes_per_ray_in"]
     d2h = n_total * work["hbm_bytes_per_ray_out"]
@@ -379,6 +448,10 @@ def run_ours(args) -> None:
         return
 
     # ---- roofline of the dominant kernel (fused encode+MLP), measured live -------------------
+    # The kernel is a gather machine: its binding units are the L1/LSU data pipe (wavefronts: a gather by 32
+    # lanes into 32 different lines costs 32 of them) and the L2 (HBM for config 4) sector path behind it.
+    # Ceilings are measured live with the library's two probes; the kernel's own wavefront / sector / DRAM
+    # counts per launch come from the committed ncu export under profiles/ (scaled by hit rays per launch).
     peaks = measured_peaks()
     nq = max(prof["n_queries"], 1)
     net_ms = prof["network_ms"] / nq                    # average launch duration, CUDA events
@@ -386,44 +459,74 @@ def run_ours(args) -> None:
     hits_per_launch = n_hit / launches_per_query
     table_bytes = params.table_storage().nbytes
     l2_resident = table_bytes <= (64 << 20)              # 126 MB L2: a 32 MiB table stays resident, 512 MiB does not
-    probe_bytes = (32 << 20) if l2_resident else (256 << 20)
-    probe = nif.nif_probe_gather(torch.from_numpy(params.table_storage()).to(dev).view(torch.uint8).reshape(-1)
-                                 if args.probe_table else torch.empty(probe_bytes, dtype=torch.uint8, device=dev))
+    smem_kernel = 140 * 1024                             # one block per SM with the fused kernel's carve-out
+    pbuf = torch.empty((32 << 20) if l2_resident else (512 << 20), dtype=torch.uint8, device=dev)
+    probe_l1 = nif.nif_probe_gather(pbuf[:32 << 20], smem_bytes=smem_kernel, mode=0)    # L1 wavefront ceiling
+    probe_l2 = nif.nif_probe_gather(pbuf[:32 << 20], smem_bytes=0, mode=1)              # L2 -> SM sector rate
+    probe_hbm = None if l2_resident else nif.nif_probe_gather(pbuf, smem_bytes=0, mode=1)   # HBM random-sector rate
+    del pbuf
     useful_gbs = hits_per_launch * work["useful_gather_bytes"] / (net_ms * 1e-3) / 1e9
-    gather_gbs = hits_per_launch * work["sector_gather_bytes"] / (net_ms * 1e-3) / 1e9
     tensor_tfs = hits_per_launch * work["mlp_flops_per_hit_ray"] / (net_ms * 1e-3) / 1e12
-    traffic = NCU_TRAFFIC.get(cfg.cfg_id, (None, None))
-    roofline = {"kernel": "k_fused_encode_mlp (tcgen05)" if not (flags & nif.NIF_ENGINE_FFMA) and cfg.net.dtype == "f16"
-                and nif.nif_net_uses_tensor_cores(net) else "k_encode_mlp_ffma",
-                "bound": "l2-gather" if l2_resident else "hbm-gather",
-                "achieved": useful_gbs, "peak": probe["gbps"], "unit": "GB/s",
-                "frac": useful_gbs / probe["gbps"], "traffic": traffic[0],
-                "peak_source": f"measured live: nif_probe_gather, independent random 32 B sectors over a "
-                               f"{probe_bytes >> 20} MiB buffer ({'L2' if l2_resident else 'HBM'}-resident like the table), all SMs; "
-                               "MEASURED_PEAKS.json has no gather figure (its HBM and tensor peaks are in .hbm / .tensor)",
-                "algorithmic": f"useful gather bytes (SURVEY 8(d).2): {work['gathers_per_hit_ray']} gathers x "
-                               f"{work['useful_gather_bytes'] // work['gathers_per_hit_ray']} B per hit ray x "
-                               f"{hits_per_launch:.0f} hit rays per launch",
-                "frac_note": "useful bytes delivered per second over the best rate at which the memory system delivers "
-                             "32 B sectors; the sectors ncu counted at L2 (profiles/) are within 8 % of the useful bytes "
-                             "on config 1 because binned rays share sectors",
-                "sector_worst_case": {"achieved": gather_gbs, "frac": gather_gbs / probe["gbps"],
-                                      "what": "every lane's gather counted as its own 32 B sector (SURVEY 8(d).2 worst case); "
-                                              "exceeds 1 when the 32 rays of a warp share sectors"},
+    counts = ncu_counts(cfg.cfg_id, args.enc)
+    is_tc = (not (flags & nif.NIF_ENGINE_FFMA)) and cfg.net.dtype == "f16" and nif.nif_net_uses_tensor_cores(net)
+    roofline = {"kernel": "k_fused_encode_mlp (tcgen05)" if is_tc else "k_encode_mlp_ffma",
                 "avg_launch_ms": net_ms, "share_of_step": net_ms * launches_per_query / ms_per_step,
-                "tensor": {"bound": "tensor", "achieved": tensor_tfs, "peak": peaks["tf_sustained"],
-                           "unit": "TFLOP/s", "frac": tensor_tfs / peaks["tf_sustained"],
-                           "peak_source": f"{peaks['source']} bf16 sustained (fp16 same pipe)"},
-                "hbm": {"bound": "hbm", "achieved": ((n_total / launches_per_query) * (work["hbm_bytes_per_ray_in"] + work["hbm_bytes_per_ray_out"]))
-                        / ((net_ms + trav_ms) * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                        "peak_source": f"{peaks['source']} copy bandwidth"}}
-    roofline["hbm"]["frac"] = roofline["hbm"]["achieved"] / peaks["hbm_gbs"]
+                "algorithmic": f"{work['gathers_per_hit_ray']} gathers x {work['useful_gather_bytes'] // work['gathers_per_hit_ray']} B "
+                               f"per hit ray x {hits_per_launch:.0f} hit rays per launch (SURVEY 8(d).2)",
+                "useful_gather_gbs": useful_gbs,
+                "ceilings": {
+                    "l1_wavefronts_per_s": probe_l1["sectors_per_s"],
+                    "l1_wavefronts_source": "measured live: nif_probe_gather mode 0 (every lane its own 128 B line of a 32 MiB "
+                                            "L2-resident buffer, one block per SM with 140 KB of shared memory like the kernel)",
+                    "l2_sectors_per_s": probe_l2["sectors_per_s"],
+                    "l2_sectors_source": "measured live: nif_probe_gather mode 1 (warp-coalesced random 128 B lines of a 32 MiB "
+                                         "L2-resident buffer, 64 warps per SM)",
+                    "hbm_random_sectors_per_s": probe_hbm["sectors_per_s"] if probe_hbm else None,
+                    "hbm_random_sectors_source": "measured live: nif_probe_gather mode 1 over a 512 MiB buffer (HBM-resident like "
+                                                 "the table)" if probe_hbm else None,
+                    "hbm_copy_gbs": peaks["hbm_gbs"], "hbm_copy_source": f"{peaks['source']} (MEASURED_PEAKS.json)"}}
+    if counts and "l1_wavefronts" in counts:
+        # per-launch counts of THIS launch = ncu's counts scaled by hit rays (the capture was made on the same workload)
+        k = hits_per_launch / counts.get("hit_rays_per_launch", hits_per_launch)
+        wf, l2s = counts["l1_wavefronts"] * k, counts.get("l2_sectors", 0.0) * k
+        dram = (counts.get("dram_bytes_read", 0.0) + counts.get("dram_bytes_write", 0.0)) * k
+        units = {"l1-wavefronts": (wf, probe_l1["sectors_per_s"]), "l2-sectors": (l2s, probe_l2["sectors_per_s"]),
+                 "hbm-copy-bytes": (dram / 32.0, peaks["hbm_gbs"] * 1e9 / 32.0)}
+        if probe_hbm:
+            units["hbm-random-sectors"] = (dram / 32.0, probe_hbm["sectors_per_s"])
+        t_unit = {name: c / r for name, (c, r) in units.items()}
+        bound = max(t_unit, key=t_unit.get)
+        roofline.update({
+            "bound": bound, "achieved": units[bound][0] * 32 / (net_ms * 1e-3) / 1e9, "peak": units[bound][1] * 32 / 1e9,
+            "unit": "GB/s", "frac": t_unit[bound] / (net_ms * 1e-3), "traffic": dram,
+            "frac_by_unit": {name: t / (net_ms * 1e-3) for name, t in t_unit.items()},
+            "counts_per_launch": {"l1_wavefronts": wf, "l1_sectors_global_ld": counts.get("l1_sectors_global_ld", 0.0) * k,
+                                  "l2_sectors_requested_by_l1": l2s, "dram_bytes": dram, "per_hit_ray": {
+                                      "l1_wavefronts": wf / max(hits_per_launch, 1), "l1_sectors": counts.get("l1_sectors_global_ld", 0.0) * k / max(hits_per_launch, 1),
+                                      "l2_sectors": l2s / max(hits_per_launch, 1), "dram_bytes": dram / max(hits_per_launch, 1)}},
+            "counts_source": counts["file"],
+            "what": "for each unit on the gather path: the time it needs for this launch's own count at its measured ceiling, over "
+                    "the event-timed launch duration; `bound` is the unit with the largest such fraction and achieved / peak are "
+                    "its traffic in GB/s (32 B per wavefront or sector)"})
+    else:
+        roofline.update({"bound": "l1-wavefronts", "achieved": useful_gbs, "peak": probe_l1["gbps"], "unit": "GB/s",
+                         "frac": useful_gbs / probe_l1["gbps"], "traffic": None,
+                         "what": "no ncu export for this configuration under profiles/: useful gather bytes over the divergent-"
+                                 "gather ceiling (a lower bound of the true fraction: binned rays share sectors)"})
+    roofline["tensor"] = {"bound": "tensor", "achieved": tensor_tfs, "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
+                          "frac": tensor_tfs / peaks["tf_sustained"], "peak_source": f"{peaks['source']} bf16 sustained (fp16 same pipe)"}
+    roofline["hbm_io"] = {"bound": "hbm", "achieved": ((n_total / launches_per_query) * (work["hbm_bytes_per_ray_in"] + work["hbm_bytes_per_ray_out"]))
+                          / ((net_ms + trav_ms) * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                          "what": "compulsory ray input / output bytes of the whole query over its duration",
+                          "peak_source": f"{peaks['source']} copy bandwidth"}
+    roofline["hbm_io"]["frac"] = roofline["hbm_io"]["achieved"] / peaks["hbm_gbs"]
     if mlp_probe:
-        tf = hits_per_launch * work["mlp_flops_per_hit_ray"] / (mlp_probe * 1e-3) / 1e12
+        hits_probe = n_hit / cfg.n_poses                 # the probe runs one nif_query per pose
+        tf = hits_probe * work["mlp_flops_per_hit_ray"] / (mlp_probe * 1e-3) / 1e12
         roofline["tensor_mlp_only_probe"] = {
-            "what": "same kernel with NIF_PROBE_SKIP_GATHER: constant A operand, no table gathers; MLP flops of "
-                    "the real network / event-timed kernel duration", "avg_launch_ms": mlp_probe,
-            "achieved": tf, "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": tf / peaks["tf_burst"],
+            "what": "the PROBE instantiation of the same kernel (NIF_PROBE_SKIP_GATHER): constant A operand, no table "
+                    "gathers; MLP flops of the real network / event-timed kernel duration, launch and pipeline fill included",
+            "avg_launch_ms": mlp_probe, "achieved": tf, "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": tf / peaks["tf_burst"],
             "peak_source": f"{peaks['source']} bf16 burst (fp16 same pipe)"}
     kernels = {"traverse_ms": trav_ms, "encode_mlp_ms": net_ms, "traverse_share": trav_ms * launches_per_query / ms_per_step,
                "queries_per_step": launches_per_query,
@@ -432,7 +535,9 @@ def run_ours(args) -> None:
 
     base = cpu_baseline(cfg, args.params) if (world == 1 and not args.no_cpu_baseline) else None
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
+            "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_best": float(np.min(step_ms)),
+            "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f16" if cfg.net.dtype == "f16" else "f32",
             "data": "synthetic",
             "config": {"workload": workload_name(cfg), "params": args.params, "rays_per_step_per_gpu": n_total,
@@ -475,7 +580,17 @@ def main() -> None:
                     help="multi-pose configs: one nif_query_poses per step (default) or one nif_query per pose")
     ap.add_argument("--walk", type=int, default=0, help="time nif_query_multi with this max_steps instead of nif_query "
                                                         "(SURVEY 8(f) f1; not the headline; use --params varpres)")
+    ap.add_argument("--profile-only", action="store_true",
+                    help="warm-up + a few steps of the query only (no probes, e2e or CPU baseline): the command the "
+                         "ncu captures under profiles/ were made with")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` run plainly: become N ranks (one per GPU) under torch.distributed.run
+        import subprocess
+        port = 29500 + (os.getpid() % 2000)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve()), *sys.argv[1:]]
+        raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -19,8 +19,9 @@
  *     buffers of a nif_stage.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  nif_query only
  *     enqueues work and returns; calls documented as "synchronises" wait for the stream.
- *     The enqueue-only calls (nif_query, nif_query_multi, nif_query_poses) allocate nothing and
- *     can be captured in a CUDA graph and replayed (rays and outputs are read/written at replay).
+ *     The enqueue-only calls (nif_query, nif_query_multi, nif_query_poses) allocate nothing, copy nothing
+ *     from host memory and can be captured in a CUDA graph and replayed (rays and outputs are read /
+ *     written at replay; the BVHs' device data and pose parameters are the ones seen at capture time).
  *   - Return value: NIF_OK (0) or a negative nif_status.  On error no output is written.
  *     No exceptions, no abort(), nothing printed.
  *   - There is no CPU fallback: on a device that is not compute capability 10.x every entry
@@ -42,7 +43,8 @@ typedef enum {
     NIF_ERR_UNSUPPORTED = -2,      /* shape/dtype the kernels do not cover, or not an sm_100 GPU */
     NIF_ERR_DEFORM_SINGULAR = -3,  /* bend folds over: some occupied corner has k*y >= 1 - 1e-3 (R7) */
     NIF_ERR_WORKSPACE = -4,        /* workspace too small or misaligned                        */
-    NIF_ERR_CUDA = -5              /* a CUDA runtime call failed                               */
+    NIF_ERR_CUDA = -5,             /* a CUDA runtime call failed                               */
+    NIF_ERR_INTERNAL = -6          /* an internal limit was exceeded (reported by nif_query_last_hit_count) */
 } nif_status;
 
 enum { NIF_F32 = 0, NIF_F16 = 1 };            /* nif_net_desc.dtype */
@@ -291,8 +293,10 @@ int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
 
 /* -------- diagnostics --------------------------------------------------------------------- */
 
-/* Counters of the last nif_query on this thread's workspace: hit rays found by the traversal.
- * Reads 8 bytes back from the workspace; SYNCHRONISES `stream`. */
+/* Counters of the last nif_query on this workspace: hit rays found by the traversal.  Reads the 64-byte
+ * scratch header back; SYNCHRONISES `stream`.  Returns NIF_ERR_INTERNAL if a per-ray traversal stack
+ * overflowed during that query (the hierarchy is at most 9 levels deep for nv <= 512 and the stack holds
+ * 7 entries per level, so this cannot happen; it is a status instead of a silent truncation). */
 int nif_query_last_hit_count(const void* workspace, void* stream, int64_t* n_hit);
 
 /* Per-kernel timing of nif_query (bench.py's roofline figure is taken from it).  After
@@ -303,14 +307,19 @@ int nif_query_last_hit_count(const void* workspace, void* stream, int64_t* n_hit
 int nif_profile_enable(int on);
 int nif_profile_read(double* traverse_ms, double* network_ms, int64_t* n_queries);
 
-/* Random-sector gather probe: the denominator of the gather roofline.
- * All SMs issue independent 4-byte loads at pseudo-random 32-byte sectors of the DEVICE buffer
- * `buf` (`bytes` rounded down to a power-of-two number of sectors); `iters` batches of 8 loads
- * per thread, 512-thread blocks.  `smem_bytes` of (untouched) dynamic shared memory per block
- * shrink the L1 data cache to what a kernel with that footprint is left with (4 blocks per SM, 2
- * above 56 KiB, 1 above 113 KiB).  Returns the best of 3 timed launches as 32-byte sectors
- * per second (and its milliseconds in *ms, optional).  SYNCHRONISES. */
-int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t smem_bytes, void* stream,
+/* Gather probes: the denominators of the gather roofline.  All SMs issue independent
+ * 4-byte loads into the DEVICE buffer `buf` (`bytes` rounded down to a power-of-two number of 32-byte sectors),
+ * `iters` batches of 8 loads per thread, 512-thread blocks.
+ *   mode 0, "divergent": every lane reads its own pseudo-random sector (its own 128-byte line), as the hashed
+ *           levels of the encoding do; a warp load is 32 L1 wavefronts, so this is the L1/LSU divergent-access
+ *           ceiling.  Returned rate: lane loads = wavefronts = sectors per second.
+ *   mode 1, "coalesced sectors": a warp reads one pseudo-random 128-byte line (4 sectors, 8 lanes each); one
+ *           wavefront moves 4 sectors, so the rate is what L2 (a buffer that fits it) or HBM (a larger one)
+ *           delivers to the SMs.  Returned rate: 32-byte sectors per second.
+ * `smem_bytes` of (untouched) dynamic shared memory per block shrink the L1 data cache to what a kernel with
+ * that footprint is left with (4 blocks per SM, 2 above 56 KiB, 1 above 113 KiB).  Best of 3 timed launches
+ * (its milliseconds in *ms, optional).  SYNCHRONISES. */
+int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t smem_bytes, int mode, void* stream,
                      double* sectors_per_s, double* ms);
 
 /* Kernels launched by the library since load (every nif_* call adds its launches). */

@@ -113,8 +113,8 @@ def lib() -> C.CDLL:
         L.nif_query_last_hit_count.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
         L.nif_profile_enable.argtypes = [C.c_int]
         L.nif_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
-        L.nif_probe_gather.argtypes = [C.c_void_p, C.c_size_t, C.c_int, C.c_size_t, C.c_void_p, C.POINTER(C.c_double),
-                                       C.POINTER(C.c_double)]
+        L.nif_probe_gather.argtypes = [C.c_void_p, C.c_size_t, C.c_int, C.c_size_t, C.c_int, C.c_void_p,
+                                       C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -376,11 +376,12 @@ def nif_profile_read() -> dict:
     return {"traverse_ms": t.value, "network_ms": m.value, "n_queries": n.value}
 
 
-def nif_probe_gather(buf: torch.Tensor, iters: int = 64, smem_bytes: int = 0, stream=None) -> dict:
-    """Random 32-byte-sector gather rate over `buf` (CUDA tensor); see include/nif.h."""
+def nif_probe_gather(buf: torch.Tensor, iters: int = 64, smem_bytes: int = 0, mode: int = 0, stream=None) -> dict:
+    """Gather probe over `buf` (CUDA tensor): mode 0 = divergent lanes (L1 wavefront ceiling), mode 1 =
+    warp-coalesced random lines (L2 / HBM sector rate); see include/nif.h."""
     assert buf.is_cuda and buf.is_contiguous()
     r, ms = C.c_double(), C.c_double()
-    _check(lib().nif_probe_gather(buf.data_ptr(), buf.numel() * buf.element_size(), iters, smem_bytes,
+    _check(lib().nif_probe_gather(buf.data_ptr(), buf.numel() * buf.element_size(), iters, smem_bytes, mode,
                                   _stream_ptr(stream), C.byref(r), C.byref(ms)), "nif_probe_gather")
     return {"sectors_per_s": r.value, "gbps": r.value * 32 / 1e9, "ms": ms.value}
 

@@ -41,6 +41,7 @@ extern "C" const char* nif_error_string(int status)
         case NIF_ERR_DEFORM_SINGULAR: return "deformation folds over (bend k*y >= 1)";
         case NIF_ERR_WORKSPACE: return "workspace too small or misaligned";
         case NIF_ERR_CUDA: return "CUDA runtime error";
+        case NIF_ERR_INTERNAL: return "internal limit exceeded (traversal stack overflow): results invalid";
         default: return "unknown status";
     }
 }
@@ -238,7 +239,7 @@ extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_b
     if (rays->n == 0) return NIF_OK;
     size_t need = 0;
     nif_query_workspace_bytes(rays->n, &need);
-    if (!workspace || ((uintptr_t)workspace & 255u) != 0 || workspace_bytes < need - 256) return NIF_ERR_WORKSPACE;
+    if (!workspace || ((uintptr_t)workspace & 255u) != 0 || workspace_bytes < need) return NIF_ERR_WORKSPACE;
     cudaStream_t stream = (cudaStream_t)stream_;
     NifQueryWs ws;
     nif_query_ws_layout(bvh, rays->n, workspace, &ws);
@@ -257,6 +258,18 @@ extern "C" int nif_query(const nif_bvh* bvh, const nif_net* net, const nif_ray_b
     nif_prof_mark(prof, 2, stream);
     return rc;
 }
+
+namespace {
+// pose descriptors travel as a KERNEL PARAMETER (16 x 64 B per launch), not through a host-to-device copy:
+// nif_query_poses stays enqueue-only and capturable in a CUDA graph (a captured memcpy would keep a pointer
+// to the caller's stack); a replay uses the descriptors as they were at capture time
+struct PoseDescPack { NifPoseDesc d[16]; };
+__global__ void k_write_pose_desc(const PoseDescPack pack, NifPoseDesc* __restrict__ dst, int n)
+{
+    const int i = threadIdx.x >> 4, w = threadIdx.x & 15;            // 16 words of 4 bytes per descriptor
+    if (i < n) reinterpret_cast<uint32_t*>(dst + i)[w] = reinterpret_cast<const uint32_t*>(&pack.d[i])[w];
+}
+}  // namespace
 
 // Several poses of one object in ONE query: every ray names its pose (SURVEY 8(f) f2, B:9 "one BVH per pose ...
 // network shared across all poses").  Hit rays are binned by rest-space voxel across poses, so the encode tiles
@@ -291,16 +304,21 @@ extern "C" int nif_query_poses(const nif_bvh* const* bvhs, int32_t n_poses, cons
     NifQueryWs ws;
     nif_query_ws_layout(bvhs[0], rays->n, workspace, &ws);
     NifPoseDesc* d_desc = (NifPoseDesc*)((char*)workspace + align_up(qbytes, 256));
-    NifPoseDesc h_desc[NIF_MAX_POSES];
-    memset(h_desc, 0, sizeof(h_desc));
-    for (int i = 0; i < n_poses; ++i) {
-        const nif_bvh* b = bvhs[i];
-        h_desc[i].nodes = b->nodes; h_desc[i].lat = b->lattice; h_desc[i].root = b->root;
-        for (int a = 0; a < 3; ++a) { h_desc[i].lo[a] = b->lo[a]; h_desc[i].hi[a] = b->hi[a]; }
-        h_desc[i].theta_max = b->theta_max; h_desc[i].bend_k = b->bend_k; h_desc[i].local_inverse = b->local_inverse;
+    for (int base = 0; base < n_poses; base += 16) {
+        PoseDescPack pack;
+        memset(&pack, 0, sizeof(pack));
+        const int m = n_poses - base < 16 ? n_poses - base : 16;
+        for (int i = 0; i < m; ++i) {
+            const nif_bvh* b = bvhs[base + i];
+            NifPoseDesc& d = pack.d[i];
+            d.nodes = b->nodes; d.lat = b->lattice; d.root = b->root;
+            for (int a = 0; a < 3; ++a) { d.lo[a] = b->lo[a]; d.hi[a] = b->hi[a]; }
+            d.theta_max = b->theta_max; d.bend_k = b->bend_k; d.local_inverse = b->local_inverse;
+        }
+        k_write_pose_desc<<<1, 256, 0, stream>>>(pack, d_desc + base, m);
+        nif_count_launch(1);
     }
-    // pageable source: the copy is staged before the call returns, so the stack array may go out of scope
-    NIF_CUDA_TRY(cudaMemcpyAsync(d_desc, h_desc, sizeof(NifPoseDesc) * (size_t)n_poses, cudaMemcpyHostToDevice, stream));
+    NIF_CUDA_TRY(cudaGetLastError());
     NifPoseBatch batch{d_desc, pose_id, n_poses};
     const bool traverse_only = (flags & NIF_TRAVERSE_ONLY) != 0;
     NIF_CUDA_TRY(cudaMemsetAsync(workspace, 0, sizeof(NifQueryScratch) + (traverse_only ? 0 : (size_t)ws.n_bins * 4), stream));
@@ -320,12 +338,14 @@ extern "C" int nif_query_poses(const nif_bvh* const* bvhs, int32_t n_poses, cons
 extern "C" int nif_query_last_hit_count(const void* workspace, void* stream_, int64_t* n_hit)
 {
     if (!workspace || !n_hit) return NIF_ERR_INVALID_ARG;
-    unsigned long long v = 0;
+    NifQueryScratch h;
     cudaStream_t stream = (cudaStream_t)stream_;
-    NIF_CUDA_TRY(cudaMemcpyAsync(&v, workspace, sizeof(v), cudaMemcpyDeviceToHost, stream));
+    NIF_CUDA_TRY(cudaMemcpyAsync(&h, workspace, sizeof(h), cudaMemcpyDeviceToHost, stream));
     NIF_CUDA_TRY(cudaStreamSynchronize(stream));
-    *n_hit = (int64_t)v;
-    return NIF_OK;
+    *n_hit = (int64_t)h.n_hit;
+    // pad[3]: set by the traversal kernels if a per-ray stack ever overflowed (cannot happen for nv <= 512,
+    // see STACK_MAX in nif_traverse.cu): the results of that query are not trustworthy
+    return h.pad[3] ? NIF_ERR_INTERNAL : NIF_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -384,12 +404,26 @@ extern "C" void nif_stage_destroy(nif_stage* s)
     delete s;
 }
 
+static int query_host_enqueue(const nif_bvh* bvh, const nif_net* net, nif_stage* st,
+                              const nif_ray_batch* rays, const nif_query_out* out, unsigned flags);
+
 extern "C" int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* st,
                               const nif_ray_batch* rays, const nif_query_out* out, unsigned flags)
 {
     if (!st) return NIF_ERR_INVALID_ARG;
     int rc = validate_query(bvh, net, rays, out, flags);
     if (rc != NIF_OK) return rc;
+    rc = query_host_enqueue(bvh, net, st, rays, out, flags);
+    // success or not, nothing may still be copying into the caller's buffers when this returns
+    for (int i = 0; i < NSLOT; ++i)
+        if (cudaStreamSynchronize(st->stream[i]) != cudaSuccess) { (void)cudaGetLastError(); if (rc == NIF_OK) rc = NIF_ERR_CUDA; }
+    return rc;
+}
+
+static int query_host_enqueue(const nif_bvh* bvh, const nif_net* net, nif_stage* st,
+                              const nif_ray_batch* rays, const nif_query_out* out, unsigned flags)
+{
+    int rc = NIF_OK;
     const bool heads = !(flags & NIF_TRAVERSE_ONLY);
     const bool full = heads && !(flags & NIF_OCCLUSION_ONLY);
     int chunk_idx = 0;
@@ -436,6 +470,5 @@ extern "C" int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage*
         if (qo.hit_position) NIF_CUDA_TRY(back(out->hit_position, b * 12, st->o_hit, mm * 12));
         if (qo.hit_position_rest) NIF_CUDA_TRY(back(out->hit_position_rest, b * 12, st->o_hitr, mm * 12));
     }
-    for (int i = 0; i < NSLOT; ++i) NIF_CUDA_TRY(cudaStreamSynchronize(st->stream[i]));
     return NIF_OK;
 }

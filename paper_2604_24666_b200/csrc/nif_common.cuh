@@ -130,6 +130,7 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
                         const NifPoseBatch* batch = nullptr);
 int nif_launch_bin_hits(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
                         const NifQueryWs* ws, const NifWalkRound* walk, cudaStream_t stream);
+int nif_launch_clear_bins(const NifQueryWs* ws, const unsigned int* n_list, cudaStream_t stream);
 void nif_query_ws_layout(const nif_bvh* bvh, int64_t n, void* workspace, NifQueryWs* ws);
 int nif_launch_ffma(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
                     const nif_query_out* out, const NifQueryScratch* scratch,

@@ -81,30 +81,37 @@ extern "C" int nif_profile_read(double* traverse_ms, double* network_ms, int64_t
     return NIF_OK;
 }
 
-// ---- random-sector gather probe --------------------------------------------------------------
+// ---- gather probes: the denominators of the gather roofline ------------------------------------
 namespace {
 
-// Every thread issues `iters` batches of 8 independent 4-byte loads at pseudo-random 32-byte
-// sectors of buf[0, n_sectors*32): the access pattern of the hashed levels of the encoding
-// (one 4-byte entry per gather, no two lanes in one sector).  Counter-based hash, no state.
+// Counter-based hash, no state.
 __device__ __forceinline__ uint32_t mix32(uint32_t x)
 {
     x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
     return x;
 }
 
+// MODE 0 "divergent": every lane loads 4 bytes from its own pseudo-random 32-byte sector (its own 128-byte
+//   line), 8 independent loads per batch: the access pattern of a hashed level, where no two lanes share a
+//   sector.  A warp load is then 32 L1 wavefronts: this measures the L1/LSU divergent-access ceiling
+//   (wavefronts per second), with the lines coming from L2 (or HBM for a large buffer).
+// MODE 1 "coalesced sectors": the 32 lanes of a warp read one pseudo-random 128-byte line (4 bytes each: 4
+//   sectors, 8 lanes per sector), 8 independent lines per batch: one L1 wavefront moves 4 sectors, so the
+//   LSU is far from its limit and the rate is what L2 (or HBM) delivers to the SMs in 32-byte sectors.
+template <int MODE>
 __global__ void __launch_bounds__(512)
-k_probe_gather(const uint32_t* __restrict__ buf, uint32_t sector_mask, int iters, uint32_t* __restrict__ sink)
+k_probe_gather(const uint32_t* __restrict__ buf, uint32_t mask, int iters, uint32_t* __restrict__ sink)
 {
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t acc = 0;
-    uint32_t ctr = tid * 0x9e3779b9u;
+    const uint32_t ctr = (MODE == 0 ? tid : (tid >> 5)) * 0x9e3779b9u;
     for (int it = 0; it < iters; ++it) {
         uint32_t v[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            const uint32_t s = mix32(ctr + (uint32_t)(it * 8 + j)) & sector_mask;
-            v[j] = __ldg(buf + (size_t)s * 8u + (tid & 7u));
+            const uint32_t s = mix32(ctr + (uint32_t)(it * 8 + j)) & mask;
+            if (MODE == 0) v[j] = __ldg(buf + (size_t)s * 8u + (tid & 7u));                 // s = sector index
+            else v[j] = __ldg(buf + (size_t)s * 32u + (tid & 31u));                          // s = line index
         }
 #pragma unroll
         for (int j = 0; j < 8; ++j) acc ^= v[j];
@@ -114,10 +121,10 @@ k_probe_gather(const uint32_t* __restrict__ buf, uint32_t sector_mask, int iters
 
 }  // namespace
 
-extern "C" int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t smem_bytes, void* stream_,
+extern "C" int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t smem_bytes, int mode, void* stream_,
                                 double* sectors_per_s, double* ms)
 {
-    if (smem_bytes > 227u * 1024u) return NIF_ERR_INVALID_ARG;
+    if (smem_bytes > 227u * 1024u || (mode != 0 && mode != 1)) return NIF_ERR_INVALID_ARG;
     if (!buf || !sectors_per_s || iters < 1 || bytes < 4096) return NIF_ERR_INVALID_ARG;
     if (!nif_device_supported()) return NIF_ERR_UNSUPPORTED;
     cudaStream_t stream = (cudaStream_t)stream_;
@@ -128,17 +135,20 @@ extern "C" int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t
     cudaEvent_t e0, e1;
     NIF_CUDA_TRY(cudaEventCreate(&e0));
     NIF_CUDA_TRY(cudaEventCreate(&e1));
-    int sms = 148;
-    (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
+    const int sms = nif_sm_count();
+    if (sms <= 0) return NIF_ERR_CUDA;
     // dynamic shared memory the probe does not touch: it only shrinks the L1 data cache to what a
     // kernel with that much shared memory is left with (one block per SM above ~113 KB)
-    NIF_CUDA_TRY(cudaFuncSetAttribute(k_probe_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+    if (mode == 0) NIF_CUDA_TRY(cudaFuncSetAttribute(k_probe_gather<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+    else NIF_CUDA_TRY(cudaFuncSetAttribute(k_probe_gather<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
     const int per_sm = smem_bytes > 113u * 1024u ? 1 : (smem_bytes > 56u * 1024u ? 2 : 4);
     const int blocks = sms * per_sm, threads = 512;
+    const uint32_t mask = (uint32_t)((mode == 0 ? n_sectors : n_sectors / 4) - 1);
     double best = 1e30;
     for (int rep = 0; rep < 4; ++rep) {                            // rep 0 warms L2 with the buffer
         NIF_CUDA_TRY(cudaEventRecord(e0, stream));
-        k_probe_gather<<<blocks, threads, smem_bytes, stream>>>((const uint32_t*)buf, (uint32_t)(n_sectors - 1), iters, sink);
+        if (mode == 0) k_probe_gather<0><<<blocks, threads, smem_bytes, stream>>>((const uint32_t*)buf, mask, iters, sink);
+        else k_probe_gather<1><<<blocks, threads, smem_bytes, stream>>>((const uint32_t*)buf, mask, iters, sink);
         NIF_CUDA_TRY(cudaEventRecord(e1, stream));
         NIF_CUDA_TRY(cudaEventSynchronize(e1));
         nif_count_launch(1);
@@ -148,8 +158,8 @@ extern "C" int nif_probe_gather(const void* buf, size_t bytes, int iters, size_t
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
     NIF_CUDA_TRY(cudaGetLastError());
-    const double loads = (double)blocks * threads * (double)iters * 8.0;
-    *sectors_per_s = loads / (best * 1e-3);
+    const double lane_loads = (double)blocks * threads * (double)iters * 8.0;
+    *sectors_per_s = (mode == 0 ? lane_loads : lane_loads / 8.0) / (best * 1e-3);     // 8 lanes share a sector in mode 1
     if (ms) *ms = best;
     return NIF_OK;
 }

@@ -156,7 +156,9 @@ __device__ __forceinline__ bool voxel_hit(const float4* __restrict__ lat, int nv
 
 constexpr int TRAV_BLOCK = 128;
 constexpr int TRAV_BLOCKS_PER_SM = 6;
-constexpr int STACK_MAX = 96;                 // 7 pushes per level net, <= 10 levels
+constexpr int STACK_MAX = 96;                 // a node pops 1 entry and pushes <= 8: 7 net per level
+constexpr int TRAV_MAX_LEVELS = 9;            // nv <= 512 (checked in nif_build.cu) -> padded 512^3 -> 9 octree levels
+static_assert(STACK_MAX >= 7 * TRAV_MAX_LEVELS + 8, "per-ray stack too small for the deepest hierarchy");
 constexpr uint32_t LEAF_FLAG = 0x80000000u;
 #ifndef NIF_TRAV_REFILL
 #define NIF_TRAV_REFILL 12
@@ -173,6 +175,7 @@ struct TravParams {
     const float* dir;
     nif_query_out out;
     unsigned int* ray_counter;                // dynamic ray fetch (scratch header)
+    unsigned int* overflow_flag;              // scratch header: set if a stack ever overflowed (reported as NIF_ERR_INTERNAL)
     const unsigned int* coherent_flag;        // written by k_ray_coherence: 1 -> simple kernel, 0 -> persistent
     uint32_t* bin_count;
     uint32_t* rank;
@@ -378,7 +381,10 @@ k_traverse_persistent(const TravParams p)
                 NIF_CE(2, 4) NIF_CE(3, 5)
                 NIF_CE(1, 2) NIF_CE(3, 4) NIF_CE(5, 6)
 #undef NIF_CE
-                if (count > STACK_MAX - sp) count = STACK_MAX - sp;         // cannot happen for nv <= 512
+                if (count > STACK_MAX - sp) {                               // excluded by the static_assert above for nv <= 512;
+                    count = STACK_MAX - sp;                                 // never silently: the query reports NIF_ERR_INTERNAL
+                    *p.overflow_flag = 1u;
+                }
                 const uint32_t unv = (uint32_t)p.nv;
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
@@ -478,8 +484,8 @@ k_traverse_simple(const TravParams p)
         for (int c = 0; c < 8; ++c) {
             if (!((meta.x >> c) & 1u)) continue;
             float cn;
-            if (slab_node(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn) &&
-                !(cn > best_in) && sp < STACK_MAX) {
+            if (slab_node(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn) && !(cn > best_in)) {
+                if (sp >= STACK_MAX) { *p.overflow_flag = 1u; continue; }   // see k_traverse_persistent
                 int q = sp++;
                 while (q > sp0 && __uint_as_float(stack[q - 1].y) < cn) { stack[q] = stack[q - 1]; --q; }
                 stack[q] = make_uint2(child[c] | leaf, __float_as_uint(cn));
@@ -531,8 +537,10 @@ k_ray_coherence(long long n, const float* __restrict__ origin, const float* __re
 // contiguous range from the global cursor (scratch->n_hit): bins of a block stay in order, blocks
 // land in arrival order -- enough locality for the encode kernel's tiles, no multi-pass scan.
 __global__ void __launch_bounds__(1024)
-k_bin_offsets(uint32_t* __restrict__ bin_count, uint32_t n_bins, NifQueryScratch* __restrict__ scratch)
+k_bin_offsets(uint32_t* __restrict__ bin_count, uint32_t n_bins, NifQueryScratch* __restrict__ scratch,
+              const unsigned int* __restrict__ n_list)
 {
+    if (n_list && *n_list == 0u) return;                  // walk round with no ray left: nothing was binned
     __shared__ uint32_t warp_sum[32];
     __shared__ unsigned long long block_base;
     const uint32_t b = blockIdx.x * 1024u + threadIdx.x;
@@ -577,7 +585,24 @@ k_scatter_hits(long long n, int nv, int bin_shift, int nvb, const int32_t* __res
     hit_list[bin_start[bin] + rank[ray]] = (int32_t)ray;
 }
 
+// walk rounds >= 1: zero the bin counters only if some ray still walks (an empty round must stay cheap)
+__global__ void __launch_bounds__(256)
+k_clear_bins(uint32_t* __restrict__ bin_count, uint32_t n_bins, const unsigned int* __restrict__ n_list)
+{
+    if (*n_list == 0u) return;
+    for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n_bins; i += gridDim.x * 256u) bin_count[i] = 0u;
+}
+
 }  // namespace
+
+int nif_launch_clear_bins(const NifQueryWs* ws, const unsigned int* n_list, cudaStream_t stream)
+{
+    const unsigned blocks = (ws->n_bins + 255u) / 256u;
+    k_clear_bins<<<blocks < 1184u ? blocks : 1184u, 256, 0, stream>>>(ws->bin_count, ws->n_bins, n_list);
+    nif_count_launch(1);
+    NIF_CUDA_TRY(cudaGetLastError());
+    return NIF_OK;
+}
 
 int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif_query_out* out,
                         const NifQueryWs* ws, unsigned flags, const NifWalkRound* walk, cudaStream_t stream,
@@ -592,6 +617,7 @@ int nif_launch_traverse(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
     p.rhx = bvh->hi[0]; p.rhy = bvh->hi[1]; p.rhz = bvh->hi[2];
     p.n = (long long)rays->n; p.origin = rays->origin; p.dir = rays->dir; p.out = *out;
     p.ray_counter = &ws->scratch->tile_counter;
+    p.overflow_flag = &ws->scratch->pad[3];
     p.bin_count = ws->bin_count; p.rank = ws->rank; p.bin_shift = ws->bin_shift; p.nvb = ws->nvb;
     p.flags = flags;
     p.ray_list = walk && walk->round > 0 ? walk->ray_list : nullptr;
@@ -631,7 +657,8 @@ int nif_launch_bin_hits(const nif_bvh* bvh, const nif_ray_batch* rays, const nif
                         const NifQueryWs* ws, const NifWalkRound* walk, cudaStream_t stream)
 {
     if (rays->n == 0) return NIF_OK;
-    k_bin_offsets<<<(ws->n_bins + 1023u) / 1024u, 1024, 0, stream>>>(ws->bin_count, ws->n_bins, ws->scratch);
+    k_bin_offsets<<<(ws->n_bins + 1023u) / 1024u, 1024, 0, stream>>>(ws->bin_count, ws->n_bins, ws->scratch,
+                                                                      walk && walk->round > 0 ? walk->n_list : nullptr);
     k_scatter_hits<<<(unsigned)((rays->n + 255) / 256), 256, 0, stream>>>(
         (long long)rays->n, bvh->nv, ws->bin_shift, ws->nvb, out->voxel_id, ws->bin_count, ws->rank, ws->hit_list,
         walk && walk->round > 0 ? walk->ray_list : nullptr, walk ? walk->n_list : nullptr);

@@ -110,7 +110,14 @@ extern "C" int nif_query_multi(const nif_bvh* bvh, const nif_net* net, const nif
     for (int round = 0; round < max_steps; ++round) {
         NifWalkRound wr;
         wr.round = round; wr.ray_list = live_list; wr.n_list = &live_count[round]; wr.dist_accum = walk->dist_accum;
-        NIF_CUDA_TRY(cudaMemsetAsync(workspace, 0, sizeof(NifQueryScratch) + (size_t)ws.n_bins * 4, stream));
+        // round 0 clears header + bins with one memset; later rounds clear the header and let a kernel clear the
+        // bins only if some ray still walks, so that the rounds after the last live ray cost a few empty launches
+        if (round == 0) NIF_CUDA_TRY(cudaMemsetAsync(workspace, 0, sizeof(NifQueryScratch) + (size_t)ws.n_bins * 4, stream));
+        else {
+            NIF_CUDA_TRY(cudaMemsetAsync(workspace, 0, sizeof(NifQueryScratch), stream));
+            rc = nif_launch_clear_bins(&ws, &live_count[round], stream);
+            if (rc != NIF_OK) return rc;
+        }
         const int prof = nif_prof_begin(stream);
         rc = nif_launch_traverse(bvh, rays, out, &ws, flags, &wr, stream);
         if (rc == NIF_OK) rc = nif_launch_bin_hits(bvh, rays, out, &ws, &wr, stream);

@@ -75,3 +75,49 @@ def test_two_ranks_shard_rays_without_exchange(tmp_path, oracle):
     t_max, hits = np.load(tmp_path / "meta.npy")
     assert np.array_equal(got, vid)                      # sharded == single rank, ray for ray
     assert t_max == world and hits == int((vid >= 0).sum())
+
+
+# ---- what bench.py actually does at N > 1: every rank runs the whole frame (replicas, weak scaling), the
+# slowest rank's device time is taken (max over ranks) and the whole-job value is world x rays / that time ----
+def _bench_worker(rank: int, world: int, port: int, out_dir: str):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import bench
+        n_rays = 2_073_600
+        my_ms = 0.9 + 0.3 * rank                        # stand-in for this rank's device-timed elapsed time
+        dist.barrier()
+        ms = bench.max_over_ranks(my_ms, dist)
+        value = bench.whole_job_value(world, n_rays, ms)
+        if rank == 0:
+            np.save(os.path.join(out_dir, "bench.npy"), np.array([ms, value]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+def test_bench_aggregate_is_world_times_rays_over_slowest_rank(tmp_path):
+    import bench
+    world = 2
+    mp.spawn(_bench_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    ms, value = np.load(tmp_path / "bench.npy")
+    assert ms == pytest.approx(1.2)                      # the slowest of 0.9 and 1.2
+    assert value == pytest.approx(2 * 2_073_600 / 1.2e-3 / 1e6)
+    # single process: identity
+    assert bench.max_over_ranks(3.5) == 3.5 and bench.whole_job_value(1, 1000, 1.0) == pytest.approx(1.0)
+
+
+def test_bench_gpus_flag_reexecs_under_torchrun(monkeypatch):
+    """`python bench.py --gpus 2` run plainly must become two ranks (torch.distributed.run), not time one GPU."""
+    import subprocess, sys
+    import bench
+    calls = []
+    monkeypatch.setattr(subprocess, "call", lambda cmd: calls.append(cmd) or 0)
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "2", "--steps", "3"])
+    with pytest.raises(SystemExit) as e:
+        bench.main()
+    assert e.value.code == 0 and len(calls) == 1
+    cmd = calls[0]
+    assert "torch.distributed.run" in cmd and "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
+    assert cmd[-4:] == ["--gpus", "2", "--steps", "3"]
