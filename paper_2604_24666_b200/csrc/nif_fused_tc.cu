@@ -132,11 +132,12 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, ui
         "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
         "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
-// One K chunk in ONE asm block: NK UMMAs over consecutive K = 16 slices (A: +8 TMEM columns, B: +32 bytes =
-// +2 in the descriptor's address field) and the commit that releases the chunk.  A single thread issues
-// every MMA of the kernel, so its instruction count per MMA is what bounds the tensor pipe on small
-// layers: one block keeps the descriptor arithmetic to one add per operand and the compiler's
-// elect-one-thread wrapper small.  commit_bar == 0 (NK = 4 only): no commit.
+// One K chunk in ONE asm block, called by a CONVERGED warp: elect.sync picks the issuing lane, which issues NK
+// UMMAs over consecutive K = 16 slices (A: +8 TMEM columns, B: +32 bytes = +2 in the descriptor's address
+// field) and, if commit_bar != 0, the commit that releases the chunk.  Measured on B200: code
+// that runs the MMA loop on one lane of a diverged warp makes ptxas wrap every tcgen05.mma in an elect-one loop
+// and issues an M128 N64 K16 UMMA every 56 cycles (the tensor pipe needs 32); the warp-converged form below
+// issues one every 32 cycles, i.e. the 64-wide layers run at the tensor pipe's rate.
 template <int NK>
 __device__ __forceinline__ void umma_chunk_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
                                               uint32_t accumulate_first, uint32_t commit_bar)
@@ -145,46 +146,62 @@ __device__ __forceinline__ void umma_chunk_ts(uint32_t d_tmem, uint32_t a_tmem, 
     if constexpr (NK == 4) {
         asm volatile(
             "{\n\t"
-            ".reg .pred p;\n\t"
+            ".reg .pred p, pe, cq;\n\t"
             ".reg .b32 a1, a2, a3;\n\t"
             ".reg .b64 b1, b2, b3;\n\t"
-            ".reg .pred cq;\n\t"
+            "elect.sync _|pe, 0xffffffff;\n\t"
             "setp.ne.b32 p, %4, 0;\n\t"
-            "setp.ne.b32 cq, %5, 0;\n\t"
+            "setp.ne.and.b32 cq, %5, 0, pe;\n\t"
             "add.u32 a1, %1, 8;\n\t"
             "add.u32 a2, %1, 16;\n\t"
             "add.u32 a3, %1, 24;\n\t"
             "add.u64 b1, %2, 2;\n\t"
             "add.u64 b2, %2, 4;\n\t"
             "add.u64 b3, %2, 6;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a1], b1, %3, 1;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a2], b2, %3, 1;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a3], b3, %3, 1;\n\t"
+            "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+            "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [a1], b1, %3, 1;\n\t"
+            "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [a2], b2, %3, 1;\n\t"
+            "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [a3], b3, %3, 1;\n\t"
             "@cq tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
             "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate_first), "r"(commit_bar) : "memory");
     } else if constexpr (NK == 2) {
         asm volatile(
             "{\n\t"
-            ".reg .pred p;\n\t"
+            ".reg .pred p, pe, cq;\n\t"
             ".reg .b32 a1;\n\t"
             ".reg .b64 b1;\n\t"
+            "elect.sync _|pe, 0xffffffff;\n\t"
             "setp.ne.b32 p, %4, 0;\n\t"
+            "setp.ne.and.b32 cq, %5, 0, pe;\n\t"
             "add.u32 a1, %1, 8;\n\t"
             "add.u64 b1, %2, 2;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], [a1], b1, %3, 1;\n\t"
-            "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
+            "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+            "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [a1], b1, %3, 1;\n\t"
+            "@cq tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
             "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate_first), "r"(commit_bar) : "memory");
     } else {
         asm volatile(
             "{\n\t"
-            ".reg .pred p;\n\t"
+            ".reg .pred p, pe, cq;\n\t"
+            "elect.sync _|pe, 0xffffffff;\n\t"
             "setp.ne.b32 p, %4, 0;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
-            "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
+            "setp.ne.and.b32 cq, %5, 0, pe;\n\t"
+            "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+            "@cq tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
             "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate_first), "r"(commit_bar) : "memory");
     }
+}
+// the same for a lone commit (converged warp, one elected lane): all previously issued MMAs of the ELECTED lane
+// arrive on `bar` when they complete.  elect.sync with a full mask always elects the same lane, so commits and
+// MMAs come from one thread.
+__device__ __forceinline__ void umma_commit_elect(uint32_t bar)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred pe;\n\t"
+        "elect.sync _|pe, 0xffffffff;\n\t"
+        "@pe tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t"
+        "}" ::"r"(bar) : "memory");
 }
 // all previously issued MMAs of this thread arrive on `bar` when they complete (implies fence::before_thread_sync)
 __device__ __forceinline__ void umma_commit(uint32_t bar)
@@ -544,7 +561,8 @@ k_fused_encode_mlp(const TcParams p)
             const uint32_t t_row = (uint32_t)((warp & 3) * 32) << 16;
             const uint32_t tm_act = tmem_base + C_ACT + (uint32_t)g * ACT_COLS;
             uint32_t hid_phase = 0, hq = 0;
-            if (W <= 64 && tg == 0) mbar_wait_sleep(bar(BAR_WRES), 0);    // resident hidden/output weights landed
+            const bool issuer = (warp & 3) == 0;                           // the group's first warp issues its MMAs (converged)
+            if (W <= 64 && issuer) mbar_wait_sleep(bar(BAR_WRES), 0);     // resident hidden/output weights landed
             // one layer of this group's tile: A = the group's activations (TMEM), B = weight chunks, D = d_tmem
             auto run_layer = [&](uint32_t d_tmem, int N, int li) {
                 tc_fence_after();
@@ -558,12 +576,13 @@ k_fused_encode_mlp(const TcParams p)
                         const uint32_t slot = hq % TC_HSLOTS;
                         mbar_wait_sleep(bar(BAR_HFULL + slot), (hq / TC_HSLOTS) & 1u);
                         tc_fence_after();
+                        __syncwarp();
                         wchunk = s_whid + slot * HCHUNK;
                     }
                     // the chunk's commit releases the weight slot (W = 128) or, on the last chunk, signals the layer
                     const uint32_t cbar = (W > 64 && kc + 1 < KC) ? bar(BAR_HEMPTY + (hq % TC_HSLOTS)) : bar(BAR_HID + g);
                     umma_chunk_ts<K16>(d_tmem, tm_act + (uint32_t)(kc * 32), smem_desc_sw128(wchunk), idesc, (uint32_t)(kc != 0), cbar);
-                    if constexpr (W > 64) { if (kc + 1 == KC) umma_commit(bar(BAR_HEMPTY + (hq % TC_HSLOTS))); ++hq; }
+                    if constexpr (W > 64) { if (kc + 1 == KC) umma_commit_elect(bar(BAR_HEMPTY + (hq % TC_HSLOTS))); ++hq; }
                 }
             };
             for (int j = g;; j += NG) {
@@ -588,7 +607,7 @@ k_fused_encode_mlp(const TcParams p)
                 if (tg == 0) TC_TRACE(j, 3);
                 // hidden layers 2..H
                 for (int hl = 1; hl < p.hidden_layers; ++hl) {
-                    if (tg == 0) run_layer(tm_hid, W, hl - 1);
+                    if (issuer) run_layer(tm_hid, W, hl - 1);
                     mbar_wait_sleep(bar(BAR_HID + g), hid_phase); hid_phase ^= 1u;
                     tc_fence_after();
                     drain_relu_to_act<W>(tm_hid + t_row, tm_act + t_row);
@@ -597,7 +616,7 @@ k_fused_encode_mlp(const TcParams p)
                     if (tg == 0) TC_TRACE(j, 3 + hl);
                 }
                 // output layer (12 heads padded to N = 16) and (a5) decode
-                if (tg == 0) run_layer(tm_hid, TC_NOUT_PAD, p.hidden_layers - 1);
+                if (issuer) run_layer(tm_hid, TC_NOUT_PAD, p.hidden_layers - 1);
                 mbar_wait_sleep(bar(BAR_HID + g), hid_phase); hid_phase ^= 1u;
                 if (tg == 0) TC_TRACE(j, 20);
                 tc_fence_after();
@@ -619,8 +638,8 @@ k_fused_encode_mlp(const TcParams p)
     } else if (warp < TC_GATHER_WARP0) {
         reg_dec<TC_REGS_MISC>();
         if (warp == TC_MMA_WARP) {
-            // ======================= layer-1 MMA issuer =============================================
-            if (lane == 0) {
+            // ======================= layer-1 MMA issuer (whole warp converged, one elected lane issues) ====
+            {
                 const uint32_t idesc = idesc_f16(TC_TILE, W);
                 if (p.w1_resident) mbar_wait_sleep(bar(BAR_WRES), 0);
                 // A chunks are handed over in GROUPS of TC_A_GROUP chunks (one full/empty barrier pair per
@@ -633,16 +652,15 @@ k_fused_encode_mlp(const TcParams p)
                     mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
                     if (s_tile[nb] < 0) break;
                     mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
-                    TC_TRACE(j, 25);
+                    if (lane == 0) TC_TRACE(j, 25);
                     tc_fence_after();
+                    __syncwarp();
                     const uint32_t d_tmem = tm_acc1 + (uint32_t)(b * W);
                     for (int c0 = 0; c0 < n_chunks; c0 += TC_A_GROUP) {
-#ifdef NIF_TC_EXP_NOWAIT
-                        if (!PROBE)
-#endif
                         mbar_wait_sleep(bar(BAR_A_FULL + gs), gph);
-                        if (c0 == 0) TC_TRACE(j, 26);
+                        if (c0 == 0 && lane == 0) TC_TRACE(j, 26);
                         tc_fence_after();
+                        __syncwarp();
 #pragma unroll
                         for (int ci = 0; ci < TC_A_GROUP; ++ci) {
                             const int c = c0 + ci;
@@ -654,17 +672,18 @@ k_fused_encode_mlp(const TcParams p)
                                     const uint32_t ws = wq % W1_SLOTS;
                                     mbar_wait_sleep(bar(BAR_W1_FULL + ws), (wq / W1_SLOTS) & 1u);
                                     tc_fence_after();
+                                    __syncwarp();
                                     bdesc = w1_desc0 + (uint64_t)(ws * (HCHUNK >> 4));
                                 }
                                 umma_chunk_ts<4>(d_tmem, tm_ring + (gs * TC_A_GROUP + (uint32_t)ci) * 32u, bdesc, idesc,
                                                  (uint32_t)(c != 0), last ? bar(BAR_A_EMPTY + gs) : 0u);
-                                if (!p.w1_resident) { umma_commit(bar(BAR_W1_EMPTY + (wq % W1_SLOTS))); ++wq; }
+                                if (!p.w1_resident) { umma_commit_elect(bar(BAR_W1_EMPTY + (wq % W1_SLOTS))); ++wq; }
                             }
                         }
                         if (++gs == (uint32_t)A_GROUPS) { gs = 0; gph ^= 1u; }
                     }
-                    umma_commit(bar(BAR_ACC_FULL + b));
-                    TC_TRACE(j, 27);
+                    umma_commit_elect(bar(BAR_ACC_FULL + b));
+                    if (lane == 0) TC_TRACE(j, 27);
                 }
             }
         } else if (warp == TC_LOAD_WARP) {
@@ -745,10 +764,10 @@ k_fused_encode_mlp(const TcParams p)
                     const long long h = tile < 0 ? n_hit : (long long)tile * TC_TILE + r;
                     float xi = 0.f, yi = 0.f, zi = 0.f, xo = 0.f, yo = 0.f, zo = 0.f, ti = 0.f, to = 0.f;
                     long long ray = -1;
-#ifdef NIF_TC_EXP_NOPREP
-                    if (PROBE && h < n_hit) { ray = h; } else
-#endif
-                    if (h < n_hit) {
+                    if (PROBE && h < n_hit) {                // MLP-only probe: ray fetch only, no map back (a2)
+                        ray = p.hit_list[h];
+                        ti = p.out.t_in[ray]; to = p.out.t_out[ray];
+                    } else if (h < n_hit) {
                         ray = p.hit_list[h];
                         ti = p.out.t_in[ray]; to = p.out.t_out[ray];
                         const float ox = p.origin[3 * ray], oy = p.origin[3 * ray + 1], oz = p.origin[3 * ray + 2];
@@ -793,9 +812,6 @@ k_fused_encode_mlp(const TcParams p)
             const float* rb = ray_buf + (size_t)nb * TC_RAY_FIELDS * TC_TILE + row;
             const long long p0 = (long long)j * n_pairs;
             const int first = (int)(((long long)qr - p0 % 4 + 4) % 4);
-#ifdef NIF_TC_EXP_NOWAIT
-            if (PROBE) { __syncwarp(); if (lane == 0) mbar_arrive(bar(BAR_RAY_EMPTY + nb)); continue; }
-#endif
             for (int e = first; e < n_pairs; e += 4) {
                 const int c = e / epc, esl = e - c * epc;
                 const int es = e;
