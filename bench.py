@@ -438,6 +438,18 @@ def run_ours(args) -> None:
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, dist if world > 1 else None, dev)
     e2e_value = whole_job_value(world, n_total, e2e_s / e2e_steps * 1e3)
+    # the same with the compact return (ids/t for every ray, head rows for hit rays only)
+    hit_ray_h = torch.empty(n_per_pose, dtype=torch.int32).pin_memory()
+    stage = nif.Stage(max(1, args.chunk // 2))          # less to copy back per chunk: shorter chunks pipeline better
+    for p in poses:
+        nif.nif_query_host_compact(p["bvh"], net, stage, p["o_h"], p["d_h"], out_h, hit_ray_h, flags=flags)
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        for p in poses:
+            nif.nif_query_host_compact(p["bvh"], net, stage, p["o_h"], p["d_h"], out_h, hit_ray_h, flags=flags)
+    e2ec_s = max_over_ranks(time.perf_counter() - t0, dist if world > 1 else None, dev)
+    e2ec_value = whole_job_value(world, n_total, e2ec_s / e2e_steps * 1e3)
     work = algorithmic_work(cfg)
     h2d = n_total * work["hbm_bytes_per_ray_in"]
     d2h = n_total * work["hbm_bytes_per_ray_out"]
@@ -548,7 +560,10 @@ def run_ours(args) -> None:
                        "poses": ("one nif_query_poses over all poses" if batched else "one nif_query per pose"),
                        "parallelism": f"dp{world} (independent frames per rank, no collective)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "nif_query_host (pinned host buffers, chunked, 3 streams)", "steps": e2e_steps},
+                    "api": "nif_query_host (pinned host buffers, chunked, 3 streams)", "steps": e2e_steps,
+                    "compact": {"value": e2ec_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                                "d2h_bytes_per_step": n_total * 12 + n_hit * (4 + work["hbm_bytes_per_ray_out"] - 12),
+                                "api": "nif_query_host_compact: ids and t for every ray, head outputs for hit rays only"}},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "kernels": kernels,
             "mhit_rays_per_s": world * n_hit / (ms_per_step * 1e-3) / 1e6}
     if walk_stats is not None:

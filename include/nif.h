@@ -291,6 +291,17 @@ void nif_stage_destroy(nif_stage* stage);
 int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
                    const nif_ray_batch* rays_host, const nif_query_out* out_host, unsigned flags);
 
+/* The same with a COMPACT return: voxel_id, t_in, t_out for every ray (HOST, n entries each, as above), but head
+ * outputs only for the rays that hit a voxel -- a miss ray's heads are zeros by definition (R18), and on a
+ * primary-ray frame most of the bytes the dense entry point copies back are those zeros.  *n_hit receives the
+ * number of hit rays; row i (0 <= i < *n_hit) of every head array in `out_host` (HOST, capacity n rows) holds the
+ * outputs of ray hit_ray_host[i] (HOST, capacity n).  Rows are grouped by staging chunk and, inside a chunk,
+ * by the voxel the ray hit; no other order is promised.  raw_logits and the hit-position outputs are not
+ * available in this form (must be NULL); NIF_OCCLUSION_ONLY writes only `occlusion`.  SYNCHRONISES. */
+int nif_query_host_compact(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
+                           const nif_ray_batch* rays_host, const nif_query_out* out_host,
+                           int32_t* hit_ray_host, int64_t* n_hit, unsigned flags);
+
 /* -------- diagnostics --------------------------------------------------------------------- */
 
 /* Counters of the last nif_query on this workspace: hit rays found by the traversal.  Reads the 64-byte

@@ -113,6 +113,8 @@ def lib() -> C.CDLL:
         L.nif_query_last_hit_count.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
         L.nif_profile_enable.argtypes = [C.c_int]
         L.nif_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.nif_query_host_compact.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut),
+                                             C.c_void_p, C.POINTER(C.c_int64), C.c_uint]
         L.nif_probe_gather.argtypes = [C.c_void_p, C.c_size_t, C.c_int, C.c_size_t, C.c_int, C.c_void_p,
                                        C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
@@ -384,6 +386,21 @@ def nif_probe_gather(buf: torch.Tensor, iters: int = 64, smem_bytes: int = 0, mo
     _check(lib().nif_probe_gather(buf.data_ptr(), buf.numel() * buf.element_size(), iters, smem_bytes, mode,
                                   _stream_ptr(stream), C.byref(r), C.byref(ms)), "nif_probe_gather")
     return {"sectors_per_s": r.value, "gbps": r.value * 32 / 1e9, "ms": ms.value}
+
+
+def nif_query_host_compact(bvh: Bvh, net: Net | None, stage: "Stage", origin: torch.Tensor, direction: torch.Tensor,
+                           out: dict, hit_ray: torch.Tensor, flags: int = 0) -> int:
+    """nif_query_host with a compact return: dense voxel_id / t_in / t_out, head rows only for hit rays
+    (row i belongs to ray hit_ray[i]).  All tensors HOST (ideally pinned).  Returns the number of hit rays."""
+    n = origin.shape[0]
+    assert not origin.is_cuda and not direction.is_cuda and origin.is_contiguous() and hit_ray.dtype == torch.int32
+    rb = _RayBatch(n, origin.data_ptr(), direction.data_ptr())
+    q = _out_struct(out)
+    n_hit = C.c_int64()
+    _check(lib().nif_query_host_compact(bvh.handle, net.handle if net is not None else None, stage.handle,
+                                        C.byref(rb), C.byref(q), hit_ray.data_ptr(), C.byref(n_hit), flags),
+           "nif_query_host_compact")
+    return n_hit.value
 
 
 class Stage:

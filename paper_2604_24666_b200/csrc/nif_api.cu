@@ -361,6 +361,10 @@ struct nif_stage {
     size_t slot_bytes, ws_bytes;
     // offsets inside a slot
     size_t o_origin, o_dir, o_vid, o_tin, o_tout, o_occ, o_dist, o_dtot, o_nrm, o_alb, o_mat, o_raw, o_hit, o_hitr, o_ws;
+    // nif_query_host_compact: compacted head rows of the chunk's hit rays + their ray indices
+    size_t c_ray, c_occ, c_dist, c_dtot, c_nrm, c_alb, c_mat;
+    unsigned long long* h_count;     // pinned host, NSLOT hit counts
+    cudaEvent_t ev[NSLOT];
 };
 
 extern "C" int nif_stage_create(int64_t chunk_rays, nif_stage** out)
@@ -381,9 +385,15 @@ extern "C" int nif_stage_create(int64_t chunk_rays, nif_stage** out)
     s->o_hit = take(n * 12); s->o_hitr = take(n * 12);
     nif_query_workspace_bytes(chunk_rays, &s->ws_bytes);
     s->o_ws = take(s->ws_bytes);
+    s->c_ray = take(n * 4); s->c_occ = take(n * 4); s->c_dist = take(n * 4); s->c_dtot = take(n * 4);
+    s->c_nrm = take(n * 12); s->c_alb = take(n * 12); s->c_mat = take(n * 16);
     s->slot_bytes = off;
+    if (cudaHostAlloc((void**)&s->h_count, NSLOT * sizeof(unsigned long long), cudaHostAllocDefault) != cudaSuccess) {
+        (void)cudaGetLastError(); delete s; return NIF_ERR_CUDA;
+    }
     for (int i = 0; i < NSLOT; ++i) {
         if (cudaStreamCreateWithFlags(&s->stream[i], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&s->ev[i], cudaEventDisableTiming) != cudaSuccess ||
             cudaMalloc((void**)&s->dev[i], s->slot_bytes) != cudaSuccess) {
             (void)cudaGetLastError();
             nif_stage_destroy(s);
@@ -399,8 +409,10 @@ extern "C" void nif_stage_destroy(nif_stage* s)
     if (!s) return;
     for (int i = 0; i < NSLOT; ++i) {
         if (s->dev[i]) cudaFree(s->dev[i]);
+        if (s->ev[i]) cudaEventDestroy(s->ev[i]);
         if (s->stream[i]) cudaStreamDestroy(s->stream[i]);
     }
+    if (s->h_count) cudaFreeHost(s->h_count);
     delete s;
 }
 
@@ -471,4 +483,118 @@ static int query_host_enqueue(const nif_bvh* bvh, const nif_net* net, nif_stage*
         if (qo.hit_position_rest) NIF_CUDA_TRY(back(out->hit_position_rest, b * 12, st->o_hitr, mm * 12));
     }
     return NIF_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// nif_query_host with a COMPACT return: ids and t for every ray, head outputs only for the rays that hit.
+// A miss ray's heads are zeros by definition (R18); on a primary-ray frame 88 % of the 48 head bytes per ray
+// that the dense entry point copies back over PCIe are those zeros.
+// ---------------------------------------------------------------------------------------------
+namespace {
+struct CompactDst { int32_t* ray; float *occ, *dist, *dtot, *nrm, *alb, *mat; };
+
+__global__ void __launch_bounds__(256)
+k_compact_heads(const NifQueryScratch* __restrict__ scratch, const int32_t* __restrict__ hit_list, const nif_query_out dense,
+                const CompactDst c, int32_t ray_base, unsigned flags)
+{
+    const long long n_hit = (long long)scratch->n_hit;
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n_hit; i += (long long)gridDim.x * 256) {
+        const int32_t r = hit_list[i];
+        c.ray[i] = r + ray_base;
+        c.occ[i] = dense.occlusion[r];
+        if (flags & NIF_OCCLUSION_ONLY) continue;
+        c.dist[i] = dense.distance[r]; c.dtot[i] = dense.dist_total[r];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { c.nrm[3 * i + a] = dense.normal[3 * r + a]; c.alb[3 * i + a] = dense.albedo[3 * r + a]; }
+#pragma unroll
+        for (int a = 0; a < 4; ++a) c.mat[4 * i + a] = dense.material_logits[4 * r + a];
+    }
+}
+}  // namespace
+
+static int query_host_compact_enqueue(const nif_bvh* bvh, const nif_net* net, nif_stage* st, const nif_ray_batch* rays,
+                                      const nif_query_out* out, int32_t* hit_ray, int64_t* n_hit_total, unsigned flags)
+{
+    const bool full = !(flags & NIF_OCCLUSION_ONLY);
+    const int n_sm = nif_sm_count();
+    if (n_sm <= 0) return NIF_ERR_CUDA;
+    int64_t total = 0;
+    int pending_slot = -1;
+    // copies the compacted rows of the chunk in `slot` back once its hit count has arrived on the host
+    auto finish = [&](int slot) -> int {
+        NIF_CUDA_TRY(cudaEventSynchronize(st->ev[slot]));
+        const size_t m = (size_t)st->h_count[slot], b = (size_t)total;
+        cudaStream_t stream = st->stream[slot];
+        char* d = st->dev[slot];
+        if (m) {
+            NIF_CUDA_TRY(cudaMemcpyAsync(hit_ray + b, d + st->c_ray, m * 4, cudaMemcpyDeviceToHost, stream));
+            NIF_CUDA_TRY(cudaMemcpyAsync(out->occlusion + b, d + st->c_occ, m * 4, cudaMemcpyDeviceToHost, stream));
+            if (full) {
+                NIF_CUDA_TRY(cudaMemcpyAsync(out->distance + b, d + st->c_dist, m * 4, cudaMemcpyDeviceToHost, stream));
+                NIF_CUDA_TRY(cudaMemcpyAsync(out->dist_total + b, d + st->c_dtot, m * 4, cudaMemcpyDeviceToHost, stream));
+                NIF_CUDA_TRY(cudaMemcpyAsync(out->normal + 3 * b, d + st->c_nrm, m * 12, cudaMemcpyDeviceToHost, stream));
+                NIF_CUDA_TRY(cudaMemcpyAsync(out->albedo + 3 * b, d + st->c_alb, m * 12, cudaMemcpyDeviceToHost, stream));
+                NIF_CUDA_TRY(cudaMemcpyAsync(out->material_logits + 4 * b, d + st->c_mat, m * 16, cudaMemcpyDeviceToHost, stream));
+            }
+        }
+        total += (int64_t)m;
+        return NIF_OK;
+    };
+    int chunk_idx = 0;
+    int64_t m = 0;
+    for (int64_t begin = 0; begin < rays->n; begin += m, ++chunk_idx) {
+        int64_t want = st->chunk;
+        if (chunk_idx < 3 && rays->n > st->chunk) want = st->chunk >> (3 - chunk_idx);
+        if (want < 1) want = 1;
+        m = (rays->n - begin < want) ? rays->n - begin : want;
+        const int slot = chunk_idx % NSLOT;
+        cudaStream_t stream = st->stream[slot];
+        char* d = st->dev[slot];
+        NIF_CUDA_TRY(cudaMemcpyAsync(d + st->o_origin, rays->origin + 3 * begin, (size_t)m * 12, cudaMemcpyHostToDevice, stream));
+        NIF_CUDA_TRY(cudaMemcpyAsync(d + st->o_dir, rays->dir + 3 * begin, (size_t)m * 12, cudaMemcpyHostToDevice, stream));
+        nif_ray_batch rb; rb.n = m; rb.origin = (const float*)(d + st->o_origin); rb.dir = (const float*)(d + st->o_dir);
+        nif_query_out qo;
+        memset(&qo, 0, sizeof(qo));
+        qo.voxel_id = (int32_t*)(d + st->o_vid); qo.t_in = (float*)(d + st->o_tin); qo.t_out = (float*)(d + st->o_tout);
+        qo.occlusion = (float*)(d + st->o_occ); qo.distance = (float*)(d + st->o_dist);
+        qo.dist_total = (float*)(d + st->o_dtot); qo.normal = (float*)(d + st->o_nrm);
+        qo.albedo = (float*)(d + st->o_alb); qo.material_logits = (float*)(d + st->o_mat);
+        int rc = nif_query(bvh, net, &rb, &qo, d + st->o_ws, st->ws_bytes, flags, stream);
+        if (rc != NIF_OK) return rc;
+        NifQueryWs ws;
+        nif_query_ws_layout(bvh, m, d + st->o_ws, &ws);
+        CompactDst c{(int32_t*)(d + st->c_ray), (float*)(d + st->c_occ), (float*)(d + st->c_dist), (float*)(d + st->c_dtot),
+                     (float*)(d + st->c_nrm), (float*)(d + st->c_alb), (float*)(d + st->c_mat)};
+        const long long blocks_want = (m + 255) / 256;
+        k_compact_heads<<<(unsigned)(blocks_want < 4LL * n_sm ? blocks_want : 4LL * n_sm), 256, 0, stream>>>(ws.scratch, ws.hit_list, qo, c, (int32_t)begin, flags);
+        nif_count_launch(1);
+        NIF_CUDA_TRY(cudaGetLastError());
+        NIF_CUDA_TRY(cudaMemcpyAsync(&st->h_count[slot], &ws.scratch->n_hit, sizeof(unsigned long long), cudaMemcpyDeviceToHost, stream));
+        NIF_CUDA_TRY(cudaEventRecord(st->ev[slot], stream));
+        const size_t b = (size_t)begin, mm = (size_t)m;
+        NIF_CUDA_TRY(cudaMemcpyAsync(out->voxel_id + b, d + st->o_vid, mm * 4, cudaMemcpyDeviceToHost, stream));
+        NIF_CUDA_TRY(cudaMemcpyAsync(out->t_in + b, d + st->o_tin, mm * 4, cudaMemcpyDeviceToHost, stream));
+        NIF_CUDA_TRY(cudaMemcpyAsync(out->t_out + b, d + st->o_tout, mm * 4, cudaMemcpyDeviceToHost, stream));
+        if (pending_slot >= 0) { rc = finish(pending_slot); if (rc != NIF_OK) return rc; }
+        pending_slot = slot;
+    }
+    if (pending_slot >= 0) { int rc = finish(pending_slot); if (rc != NIF_OK) return rc; }
+    *n_hit_total = total;
+    return NIF_OK;
+}
+
+extern "C" int nif_query_host_compact(const nif_bvh* bvh, const nif_net* net, nif_stage* st, const nif_ray_batch* rays,
+                                      const nif_query_out* out, int32_t* hit_ray, int64_t* n_hit, unsigned flags)
+{
+    if (!st || !hit_ray || !n_hit) return NIF_ERR_INVALID_ARG;
+    if (flags & NIF_TRAVERSE_ONLY) return NIF_ERR_INVALID_ARG;
+    int rc = validate_query(bvh, net, rays, out, flags);
+    if (rc != NIF_OK) return rc;
+    if (out->raw_logits || out->hit_position || out->hit_position_rest) return NIF_ERR_INVALID_ARG;
+    *n_hit = 0;
+    rc = query_host_compact_enqueue(bvh, net, st, rays, out, hit_ray, n_hit, flags);
+    for (int i = 0; i < NSLOT; ++i)
+        if (cudaStreamSynchronize(st->stream[i]) != cudaSuccess) { (void)cudaGetLastError(); if (rc == NIF_OK) rc = NIF_ERR_CUDA; }
+    return rc;
 }

@@ -115,6 +115,34 @@ def test_host_buffer_entry_matches_device_entry(H, nif):
         assert np.array_equal(v.numpy(), dev[k], equal_nan=True), k
 
 
+@pytest.mark.parametrize("occlusion_only", [False, True])
+def test_compact_host_return_matches_device_entry(H, nif, occlusion_only):
+    # nif_query_host_compact: dense ids/t, head rows only for the hit rays (row i <-> ray hit_ray[i]); chunked
+    case = H.make_case(1, n_rays=50_000)
+    flags = nif.NIF_OCCLUSION_ONLY if occlusion_only else 0
+    dev = H.run_gpu(case, flags=flags, raw_logits=False)
+    n = len(case.origin)
+    o = torch.from_numpy(case.origin).pin_memory(); d = torch.from_numpy(case.direction).pin_memory()
+    out = nif.alloc_outputs(n, pinned_host=True)
+    for v in out.values():
+        v.fill_(-7)
+    hit_ray = torch.full((n,), -1, dtype=torch.int32).pin_memory()
+    stage = nif.Stage(16_384)
+    n_hit = nif.nif_query_host_compact(case.bvh, case.net, stage, o, d, out, hit_ray, flags=flags)
+    hits = np.nonzero(dev["voxel_id"] >= 0)[0]
+    assert n_hit == len(hits) > 1000
+    for k in ("voxel_id", "t_in", "t_out"):
+        assert np.array_equal(out[k].numpy(), dev[k]), k
+    hr = hit_ray.numpy()[:n_hit]
+    assert np.array_equal(np.sort(hr), hits)                      # every hit ray exactly once
+    keys = ["occlusion"] if occlusion_only else ["occlusion", "distance", "dist_total", "normal", "albedo", "material_logits"]
+    for k in keys:
+        assert np.array_equal(out[k].numpy()[:n_hit], dev[k][hr]), k
+        assert (out[k].numpy()[n_hit:] == -7).all(), k             # nothing written past the hit rows
+    if occlusion_only:
+        assert (out["normal"].numpy() == -7).all()
+
+
 FULL = [  # cfg, pose, parameter variant
     (1, 0, "varpres"),
     (1, 0, "uniform0.1"),
