@@ -96,7 +96,7 @@ __device__ __forceinline__ uint32_t mix32(uint32_t x)
 //   sector.  A warp load is then 32 L1 wavefronts: this measures the L1/LSU divergent-access ceiling
 //   (wavefronts per second), with the lines coming from L2 (or HBM for a large buffer).
 // MODE 1 "coalesced sectors": the 32 lanes of a warp read one pseudo-random 128-byte line (4 bytes each: 4
-//   sectors, 8 lanes per sector), 8 independent lines per batch: one L1 wavefront moves 4 sectors, so the
+//   sectors, 8 lanes per sector), 16 independent lines per batch: one L1 wavefront moves 4 sectors, so the
 //   LSU is far from its limit and the rate is what L2 (or HBM) delivers to the SMs in 32-byte sectors.
 template <int MODE>
 __global__ void __launch_bounds__(512)
@@ -105,16 +105,17 @@ k_probe_gather(const uint32_t* __restrict__ buf, uint32_t mask, int iters, uint3
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t acc = 0;
     const uint32_t ctr = (MODE == 0 ? tid : (tid >> 5)) * 0x9e3779b9u;
-    for (int it = 0; it < iters; ++it) {
-        uint32_t v[8];
+    constexpr int NB = MODE == 0 ? 8 : 16;          // independent loads in flight per thread
+    for (int it = 0; it < iters * 8 / NB; ++it) {
+        uint32_t v[NB];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const uint32_t s = mix32(ctr + (uint32_t)(it * 8 + j)) & mask;
+        for (int j = 0; j < NB; ++j) {
+            const uint32_t s = mix32(ctr + (uint32_t)(it * NB + j)) & mask;
             if (MODE == 0) v[j] = __ldg(buf + (size_t)s * 8u + (tid & 7u));                 // s = sector index
             else v[j] = __ldg(buf + (size_t)s * 32u + (tid & 31u));                          // s = line index
         }
 #pragma unroll
-        for (int j = 0; j < 8; ++j) acc ^= v[j];
+        for (int j = 0; j < NB; ++j) acc ^= v[j];
     }
     if (acc == 0x12345678u) sink[0] = acc;      // defeats dead-code elimination, never true in practice
 }
