@@ -392,6 +392,11 @@ def run_ours(args) -> None:
     prof = nif.nif_profile_read()
     nif.nif_profile_enable(False)
     if args.profile_only:
+        if args.with_probe and nif.nif_net_uses_tensor_cores(net):
+            for _ in range(4):                         # the MLP-only probe instantiation, for an ncu capture of it
+                for p in poses:
+                    ws = nif.nif_query(p["bvh"], net, p["o"], p["d"], out, workspace=ws, flags=flags | nif.NIF_PROBE_SKIP_GATHER)
+            torch.cuda.synchronize()
         if rank == 0:
             print(json.dumps({"profile_only": True, "config": workload_name(cfg), "ms_per_step": ms_per_step,
                               "hit_rays_per_step": n_hit, "hit_rays_per_launch": n_hit / launches_per_query,
@@ -604,6 +609,7 @@ def main() -> None:
     ap.add_argument("--profile-only", action="store_true",
                     help="warm-up + a few steps of the query only (no probes, e2e or CPU baseline): the command the "
                          "ncu captures under profiles/ were made with")
+    ap.add_argument("--with-probe", action="store_true", help="with --profile-only: also launch the MLP-only probe kernel")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # `python bench.py --gpus N` run plainly: become N ranks (one per GPU) under torch.distributed.run
