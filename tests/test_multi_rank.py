@@ -121,3 +121,14 @@ def test_bench_gpus_flag_reexecs_under_torchrun(monkeypatch):
     cmd = calls[0]
     assert "torch.distributed.run" in cmd and "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
     assert cmd[-4:] == ["--gpus", "2", "--steps", "3"]
+
+
+def test_bench_reads_its_counts_from_the_committed_ncu_exports():
+    """roofline counts come from profiles/*.csv (ncu --page raw --csv), not from constants in bench.py"""
+    import bench
+    for cfg_id in (1, 4):
+        c = bench.ncu_counts(cfg_id, "compose")
+        assert c is not None and c["file"].startswith("profiles/")
+        for k in ("l1_wavefronts", "l2_sectors", "dram_bytes_read", "hit_rays_per_launch"):
+            assert c[k] > 0, (cfg_id, k)
+    assert bench.ncu_counts(3, "compose") is None       # no export for this config: bench falls back and says so
