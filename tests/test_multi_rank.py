@@ -131,4 +131,4 @@ def test_bench_reads_its_counts_from_the_committed_ncu_exports():
         assert c is not None and c["file"].startswith("profiles/")
         for k in ("l1_wavefronts", "l2_sectors", "dram_bytes_read", "hit_rays_per_launch"):
             assert c[k] > 0, (cfg_id, k)
-    assert bench.ncu_counts(3, "compose") is None       # no export for this config: bench falls back and says so
+    assert bench.ncu_counts(0, "compose") is None       # no export for this config: bench falls back and says so
