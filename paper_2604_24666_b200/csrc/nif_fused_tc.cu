@@ -15,7 +15,7 @@
 //   * accumulators: layer 1 double-buffered (tile t+1 accumulates while tile t is in its tail), one
 //     hidden/output accumulator per tail group (W = 128: aliased onto the drained layer-1 buffer).
 //
-// Warp roles (one CTA per SM, 28 warps; setmaxnreg moves registers from the small roles to the
+// Warp roles (one CTA per SM, 32 warps; setmaxnreg moves registers from the other roles to the
 // gather warps, whose loop needs 80):
 //   warps 0-3 / 4-7  tail groups 0 / 1, alternating tiles: drain the layer-1 accumulator (tcgen05.ld),
 //                    ReLU -> fp16 -> tcgen05.st as the next A operand, one thread issues the hidden /
@@ -26,7 +26,7 @@
 //                    not resident; lane 1 streams hidden/output chunks (W = 128).
 //   warps 10-11      "prep": draw tile ids from the global counter, fetch the tile's rays through
 //                    hit_list and map entry/exit points back to rest space (a2) -> ray_buf (3 deep).
-//   warps 12-27      gather warps: lane = ray of row group (warp % 4); one work item = (endpoint, PE
+//   warps 12-31      gather warps: lane = ray of row group (warp % 4); one work item = (endpoint, PE
 //                    sample): the L levels of that sample are interpolated (8 table gathers each, fp32,
 //                    two batches of loads in flight) and written as fp16 into the chunk slot (a3).
 // Template parameters: W, F; CONCAT = concatenation reading of the hybrid encoding (R1); LOCAL =
@@ -46,9 +46,9 @@ constexpr int TC_LOAD_WARP = 9;
 constexpr int TC_PREP_WARP0 = 10;            // warps 10, 11
 constexpr int TC_PREP_THREADS = 64;
 constexpr int TC_GATHER_WARP0 = 12;
-constexpr int TC_GATHER_WARPS = 16;          // 4 row groups x TC_GPR warps (20 warps at 72 registers: cfg 1 +5 %, cfg 4 -3 %)
+constexpr int TC_GATHER_WARPS = 20;          // 4 row groups x TC_GPR warps: as many as the register file allows at 80 each
 constexpr int TC_GPR = TC_GATHER_WARPS / 4;
-constexpr int TC_THREADS = 32 * (TC_GATHER_WARP0 + TC_GATHER_WARPS);      // 896
+constexpr int TC_THREADS = 32 * (TC_GATHER_WARP0 + TC_GATHER_WARPS);      // 1024
 constexpr int TC_RAY_BUFS = 3;               // ray_buf depth: prep runs up to two tiles ahead of the tails
 constexpr int TC_RAY_FIELDS = 9;             // xi yi zi xo yo zo t_in t_out ray
 constexpr int TC_MAX_A_SLOTS = 8;            // layer-1 A chunk slots in TMEM (32 columns each)
@@ -56,7 +56,12 @@ constexpr int TC_A_GROUP = 1;                // chunks per full/empty barrier pa
 constexpr int TC_MAX_W1_SLOTS = 8;           // layer-1 weight chunk slots when W1 streams
 constexpr int TC_HSLOTS = 2;                 // hidden/output weight chunk ring (W = 128)
 constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded to the UMMA minimum)
-constexpr int TC_REGS_MISC = 40, TC_REGS_GATHER = 80;   // launch: 72 x 28 warps; setmaxnreg only redistributes what a dec released: 8 x 72 + 4 x 40 + 16 x 80 = 28 x 72
+// Launched with 64 registers per thread (1024 threads); setmaxnreg then moves registers from the roles that are off the
+// critical path of the real (gather-bound) kernel to the gather warps, whose loop needs 80 and which are the kernel's
+// memory-level parallelism: tails 40, small roles 24, gather 80 (8 x 40 + 4 x 24 + 20 x 80 = 2016 <= 32 x 64; a
+// setmaxnreg.inc can only take what a dec released).  Measured: 16 gather warps (tails 72, small roles 40) 0.706 / 5.00 ms on
+// config 1 / 4, 20 gather warps 0.673 / 4.87 ms; the tails and the prep warps spill ~150 B and do not care.
+constexpr int TC_REGS_MISC = 24, TC_REGS_GATHER = 80, TC_REGS_TAIL = 40;   // launch: 72 x 28 warps; setmaxnreg only redistributes what a dec released: 8 x 72 + 4 x 40 + 16 x 80 = 28 x 72
 
 // ---- PTX wrappers -----------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -556,6 +561,7 @@ k_fused_encode_mlp(const TcParams p)
 
     if (warp < TC_TAIL_WARPS) {
         // ======================= tail groups: MLP layers 2.. and (a5), alternating tiles ===========
+        reg_dec<TC_REGS_TAIL>();
         const int g = warp >> 2;
         if (g < NG) {
             const int tg = tid - g * TC_TILE;                              // row of the tile / TMEM lane
