@@ -46,31 +46,38 @@ __device__ __forceinline__ void nif_load_voxel_corners(const float4* __restrict_
 __device__ __forceinline__ void nif_inverse_trilinear(const float (&q)[8][3], const int (&cell)[3], int nv,
                                                       float X, float Y, float Z, float& x, float& y, float& z)
 {
-    const float P[3] = {X, Y, Z};
+    // Shape-function form (written independently of the oracle's nested-lerp form): T = sum_c N_c q_c with
+    // N_c = a_c(u) b_c(v) g_c(w), a = (1-u, u) etc.; the Jacobian columns are sum_c (dN_c/du) q_c, ...; the
+    // Newton step solves J d = P - T with the adjugate (cofactor) inverse.
     float u = 0.5f, v = 0.5f, w = 0.5f;
     for (int it = 0; it < NIF_NEWTON_ITERS; ++it) {
-        float Ju[3], Jv[3], Jw[3], r[3];
+        const float au[2] = {1.0f - u, u}, bv[2] = {1.0f - v, v}, gw[2] = {1.0f - w, w};
+        float T[3] = {0.f, 0.f, 0.f}, J[3][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}};   // J[row = axis][col = u,v,w]
 #pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const float d00 = q[1][a] - q[0][a], d10 = q[3][a] - q[2][a], d01 = q[5][a] - q[4][a], d11 = q[7][a] - q[6][a];
-            const float c00 = q[0][a] + u * d00, c10 = q[2][a] + u * d10, c01 = q[4][a] + u * d01, c11 = q[6][a] + u * d11;
-            const float e0 = c10 - c00, e1 = c11 - c01;
-            const float c0 = c00 + v * e0, c1 = c01 + v * e1;
-            Jw[a] = c1 - c0;
-            Jv[a] = e0 + w * (e1 - e0);
-            const float f0 = d00 + v * (d10 - d00), f1 = d01 + v * (d11 - d01);
-            Ju[a] = f0 + w * (f1 - f0);
-            r[a] = P[a] - (c0 + w * (c1 - c0));
+        for (int c = 0; c < 8; ++c) {
+            const int i = c & 1, j = (c >> 1) & 1, k = c >> 2;
+            const float n = au[i] * bv[j] * gw[k];
+            const float du = (i ? 1.0f : -1.0f) * bv[j] * gw[k];
+            const float dv = au[i] * (j ? 1.0f : -1.0f) * gw[k];
+            const float dw = au[i] * bv[j] * (k ? 1.0f : -1.0f);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                T[a] = fmaf(n, q[c][a], T[a]);
+                J[a][0] = fmaf(du, q[c][a], J[a][0]); J[a][1] = fmaf(dv, q[c][a], J[a][1]); J[a][2] = fmaf(dw, q[c][a], J[a][2]);
+            }
         }
-        const float cx = Jv[1] * Jw[2] - Jv[2] * Jw[1], cy = Jv[2] * Jw[0] - Jv[0] * Jw[2], cz = Jv[0] * Jw[1] - Jv[1] * Jw[0];
-        const float det = Ju[0] * cx + Ju[1] * cy + Ju[2] * cz;
+        const float r0 = X - T[0], r1 = Y - T[1], r2 = Z - T[2];
+        // cofactors of J
+        const float c00 = J[1][1] * J[2][2] - J[1][2] * J[2][1], c01 = J[1][2] * J[2][0] - J[1][0] * J[2][2], c02 = J[1][0] * J[2][1] - J[1][1] * J[2][0];
+        const float det = J[0][0] * c00 + J[0][1] * c01 + J[0][2] * c02;
         if (det == 0.0f) break;
-        const float du = (r[0] * cx + r[1] * cy + r[2] * cz) / det;
-        const float rx = r[1] * Jw[2] - r[2] * Jw[1], ry = r[2] * Jw[0] - r[0] * Jw[2], rz = r[0] * Jw[1] - r[1] * Jw[0];
-        const float dv = (Ju[0] * rx + Ju[1] * ry + Ju[2] * rz) / det;
-        const float sx = Jv[1] * r[2] - Jv[2] * r[1], sy = Jv[2] * r[0] - Jv[0] * r[2], sz = Jv[0] * r[1] - Jv[1] * r[0];
-        const float dw = (Ju[0] * sx + Ju[1] * sy + Ju[2] * sz) / det;
-        u += du; v += dv; w += dw;
+        const float c10 = J[0][2] * J[2][1] - J[0][1] * J[2][2], c11 = J[0][0] * J[2][2] - J[0][2] * J[2][0], c12 = J[0][1] * J[2][0] - J[0][0] * J[2][1];
+        const float c20 = J[0][1] * J[1][2] - J[0][2] * J[1][1], c21 = J[0][2] * J[1][0] - J[0][0] * J[1][2], c22 = J[0][0] * J[1][1] - J[0][1] * J[1][0];
+        const float inv = 1.0f / det;
+        // d = J^-1 r = adj(J) r / det, adj(J)[i][j] = cofactor[j][i]
+        u += (c00 * r0 + c10 * r1 + c20 * r2) * inv;
+        v += (c01 * r0 + c11 * r1 + c21 * r2) * inv;
+        w += (c02 * r0 + c12 * r1 + c22 * r2) * inv;
     }
     const float fnv = (float)nv;
     x = (2.0f * ((float)cell[0] + u) - fnv) / fnv;
