@@ -283,7 +283,7 @@ __host__ __device__ __forceinline__ uint32_t sw128_off(uint32_t row, uint32_t un
     return row * 128u + ((unit ^ (row & 7u)) << 4);
 }
 
-// ---- optional per-tile timestamps (compile with -DNIF_TC_TRACE; _work/ scripts read them) ---------
+// ---- optional per-tile timestamps (compile with -DNIF_TC_TRACE; nif_debug_set_tc_trace hands in the buffer) ----
 #ifdef NIF_TC_TRACE
 __device__ unsigned int* g_tc_trace = nullptr;        // [cta][NIF_TC_TRACE_TILES][32] clock() samples
 #define NIF_TC_TRACE_TILES 24
