@@ -834,9 +834,12 @@ k_fused_encode_mlp(const TcParams p)
                 tc_fence_after();
                 const uint32_t a_dst = tm_ring + slot * 32u + (uint32_t)(esl * units_per_es) * 4u + t_row;
                 if constexpr (PROBE) {
-                    // MLP-only probe: synthetic features, no table access
-                    for (int u = 0; u < units_per_es; ++u)
-                        tmem_st_32x4(a_dst + (uint32_t)u * 4u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u);
+                    // MLP-only probe: synthetic features, no table access.  The constant is written on the first pass
+                    // over the ring only (the MMAs do not modify A): afterwards an item is the slot hand-over alone, so
+                    // that the probe measures the MLP pipeline and not the cost of faking its input
+                    if (gq < (uint32_t)A_GROUPS)
+                        for (int u = 0; u < units_per_es; ++u)
+                            tmem_st_32x4(a_dst + (uint32_t)u * 4u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u);
                 } else if (CONCAT && es >= 2 && es < p.n_es) {
                     // NIF_ENC_CONCAT: items 0, 1 are phi(entry), phi(exit); the rest carry the gamma scalars as
                     // they are: L*F = 32 -> two 32-column items per endpoint, L*F = 64 -> one 64-column item
