@@ -61,7 +61,7 @@ constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded 
 // memory-level parallelism: tails 40, small roles 24, gather 80 (8 x 40 + 4 x 24 + 20 x 80 = 2016 <= 32 x 64; a
 // setmaxnreg.inc can only take what a dec released).  Measured: 16 gather warps (tails 72, small roles 40) 0.706 / 5.00 ms on
 // config 1 / 4, 20 gather warps 0.673 / 4.87 ms; the tails and the prep warps spill ~150 B and do not care.
-constexpr int TC_REGS_MISC = 24, TC_REGS_GATHER = 80, TC_REGS_TAIL = 40;   // launch: 72 x 28 warps; setmaxnreg only redistributes what a dec released: 8 x 72 + 4 x 40 + 16 x 80 = 28 x 72
+constexpr int TC_REGS_MISC = 24, TC_REGS_GATHER = 80, TC_REGS_TAIL = 40;
 
 // ---- PTX wrappers -----------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
