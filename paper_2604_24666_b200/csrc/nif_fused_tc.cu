@@ -12,8 +12,9 @@
 //   * layer-1 weights stay resident in shared memory when they fit the budget (config 1-3: 104 KB),
 //     otherwise their K chunks stream through a ring (config 4: 416 KB); hidden/output weights are
 //     resident for W <= 64 and stream through a 2-slot ring for W = 128;
-//   * accumulators: layer 1 double-buffered (tile t+1 accumulates while tile t is in its tail), one
-//     hidden/output accumulator per tail group (W = 128: aliased onto the drained layer-1 buffer).
+//   * accumulators: layer 1 double-buffered (tile t+1 accumulates while tile t is in its tail); the
+//     hidden/output layers of a tile accumulate into its own drained layer-1 buffer, so that the rest
+//     of the 512 TMEM columns is the A ring (10 chunk slots for W <= 64, 6 for W = 128).
 //
 // Warp roles (one CTA per SM, 32 warps; setmaxnreg moves registers from the other roles to the
 // gather warps, whose loop needs 80):
@@ -21,7 +22,7 @@
 //                    ReLU -> fp16 -> tcgen05.st as the next A operand, one thread issues the hidden /
 //                    output layer MMAs, finally decode and store the heads (a5).  Two groups keep two
 //                    tiles' dependent layer chains in flight.
-//   warp 8           lane 0 issues the layer-1 MMAs chunk by chunk as ring slots fill.
+//   warp 8           issues the layer-1 MMAs chunk by chunk as ring slots fill (converged, elect.sync).
 //   warp 9           lane 0 loads the resident weights once and streams layer-1 chunks when they are
 //                    not resident; lane 1 streams hidden/output chunks (W = 128).
 //   warps 10-11      "prep": draw tile ids from the global counter, fetch the tile's rays through
@@ -51,7 +52,7 @@ constexpr int TC_GPR = TC_GATHER_WARPS / 4;
 constexpr int TC_THREADS = 32 * (TC_GATHER_WARP0 + TC_GATHER_WARPS);      // 1024
 constexpr int TC_RAY_BUFS = 3;               // ray_buf depth: prep runs up to two tiles ahead of the tails
 constexpr int TC_RAY_FIELDS = 9;             // xi yi zi xo yo zo t_in t_out ray
-constexpr int TC_MAX_A_SLOTS = 8;            // layer-1 A chunk slots in TMEM (32 columns each)
+constexpr int TC_MAX_A_SLOTS = 10;           // layer-1 A chunk slots in TMEM (32 columns each)
 constexpr int TC_A_GROUP = 1;                // chunks per full/empty barrier pair of the A ring
 constexpr int TC_MAX_W1_SLOTS = 8;           // layer-1 weight chunk slots when W1 streams
 constexpr int TC_HSLOTS = 2;                 // hidden/output weight chunk ring (W = 128)
@@ -352,10 +353,13 @@ enum { BAR_A_FULL = 0, BAR_A_EMPTY = BAR_A_FULL + TC_MAX_A_SLOTS, BAR_W1_FULL = 
 // interpolates in fp32 and returns the batch's 4 features as two packed half2.  Two batches are in
 // flight per thread: the next batch's loads are issued before the current one is consumed.
 struct TcLevel {            // per-level constants, staged in shared memory (one LDS.128 per level)
-    float fn, top;          // N, N-1
+    float fn;               // N
     uint32_t np1;           // N+1 for a dense level, 0 for a hashed one
-    uint32_t pad;
+    const void* base;       // &table[l][0][0].  Read back from shared memory on purpose: a base the compiler can
+                            // prove warp-uniform stays in uniform registers and every gather address then costs an
+                            // IADD3 + IADD3.X pair; a base in a vector register pair makes it ONE IMAD.WIDE.U32
 };
+static_assert(sizeof(TcLevel) == 16, "TcLevel is read with one LDS.128");
 
 // L1 eviction priority of the table gathers.  Measured (cfg 1 / cfg 4 encode+MLP ms): plain __ldg 0.711 /
 // 10.69; evict_last on every level 0.708 / 10.47; evict_first or no_allocate on the fine (hashed) levels
@@ -367,25 +371,35 @@ struct TcLevel {            // per-level constants, staged in shared memory (one
 #ifndef NIF_TC_FINE_HINT
 #define NIF_TC_FINE_HINT "L1::evict_last"
 #endif
-template <bool FINE> __device__ __forceinline__ uint32_t ldg_hint(const uint32_t* p)
+// OFF = immediate byte offset, so that the +x corner of a dense cell shares its neighbour's address register
+template <bool FINE, int OFF = 0> __device__ __forceinline__ uint32_t ldg_hint(const uint32_t* p)
 {
     uint32_t v;
-    if constexpr (FINE) asm volatile("ld.global.nc." NIF_TC_FINE_HINT ".b32 %0, [%1];" : "=r"(v) : "l"(p));
+    if constexpr (FINE) asm volatile("ld.global.nc." NIF_TC_FINE_HINT ".b32 %0, [%1+%2];" : "=r"(v) : "l"(p), "n"(OFF));
     else {
 #ifdef NIF_TC_COARSE_HINT
-        asm volatile("ld.global.nc." NIF_TC_COARSE_HINT ".b32 %0, [%1];" : "=r"(v) : "l"(p));
+        asm volatile("ld.global.nc." NIF_TC_COARSE_HINT ".b32 %0, [%1+%2];" : "=r"(v) : "l"(p), "n"(OFF));
 #else
-        v = __ldg(p);
+        asm volatile("ld.global.nc.b32 %0, [%1+%2];" : "=r"(v) : "l"(p), "n"(OFF));
 #endif
     }
     return v;
 }
-template <bool FINE> __device__ __forceinline__ uint2 ldg_hint(const uint2* p)
+template <bool FINE, int OFF = 0> __device__ __forceinline__ uint2 ldg_hint(const uint2* p)
 {
     uint2 v;
-    if constexpr (FINE) asm volatile("ld.global.nc." NIF_TC_FINE_HINT ".v2.b32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
-    else v = __ldg(p);
+    if constexpr (FINE) asm volatile("ld.global.nc." NIF_TC_FINE_HINT ".v2.b32 {%0, %1}, [%2+%3];" : "=r"(v.x), "=r"(v.y) : "l"(p), "n"(OFF));
+    else asm volatile("ld.global.nc.v2.b32 {%0, %1}, [%2+%3];" : "=r"(v.x), "=r"(v.y) : "l"(p), "n"(OFF));
     return v;
+}
+
+// (a ^ b) & m as ONE LOP3 (left to itself the compiler folds the y/z hash xor into every corner and spends
+// a second LOP3 per corner on the mask)
+__device__ __forceinline__ uint32_t xor_and(uint32_t a, uint32_t b, uint32_t m)
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0x28;" : "=r"(d) : "r"(a), "r"(b), "r"(m));
+    return d;
 }
 
 template <int F>
@@ -395,48 +409,45 @@ struct GatherBatch {
     raw_t raw[NL][8];
     float wx[NL], wy[NL], wz[NL];
 
-    __device__ __forceinline__ void issue(const __half* __restrict__ table, const TcLevel* __restrict__ s_lvl,
-                                          int log2_T, int l0, float px, float py, float pz)
+    __device__ __forceinline__ void issue(const TcLevel* __restrict__ s_lvl, int log2_T, int l0, float px, float py, float pz)
     {
-        if (l0 >= NIF_TC_FINE_FROM) issue_t<true>(table, s_lvl, log2_T, l0, px, py, pz);
-        else issue_t<false>(table, s_lvl, log2_T, l0, px, py, pz);
+        if (l0 >= NIF_TC_FINE_FROM) issue_t<true>(s_lvl, log2_T, l0, px, py, pz);
+        else issue_t<false>(s_lvl, log2_T, l0, px, py, pz);
     }
     template <bool FINE>
-    __device__ __forceinline__ void issue_t(const __half* __restrict__ table, const TcLevel* __restrict__ s_lvl,
-                                            int log2_T, int l0, float px, float py, float pz)
+    __device__ __forceinline__ void issue_t(const TcLevel* __restrict__ s_lvl, int log2_T, int l0, float px, float py, float pz)
     {
         const uint32_t t_mask = (1u << log2_T) - 1u;
 #pragma unroll
         for (int li = 0; li < NL; ++li) {
             const int l = l0 + li;
-            const float4 lv = *reinterpret_cast<const float4*>(s_lvl + l);
-            const uint32_t np1 = __float_as_uint(lv.z);
-            const float posx = px * lv.x, posy = py * lv.x, posz = pz * lv.x;     // p in [0,1]: floor >= 0
-            const float flx = fminf(floorf(posx), lv.y), fly = fminf(floorf(posy), lv.y), flz = fminf(floorf(posz), lv.y);
+            const uint4 lv = *reinterpret_cast<const uint4*>(s_lvl + l);
+            const float fn = __uint_as_float(lv.x), top = fn - 1.0f;
+            const uint32_t np1 = lv.y;
+            const raw_t* lvl = reinterpret_cast<const raw_t*>(((unsigned long long)lv.w << 32) | (unsigned long long)lv.z);
+            const float posx = px * fn, posy = py * fn, posz = pz * fn;           // p in [0,1]: floor >= 0
+            const float flx = fminf(floorf(posx), top), fly = fminf(floorf(posy), top), flz = fminf(floorf(posz), top);
             wx[li] = posx - flx; wy[li] = posy - fly; wz[li] = posz - flz;
             const uint32_t cx = (uint32_t)flx, cy = (uint32_t)fly, cz = (uint32_t)flz;
-            // byte offsets (32-bit) from the level's base: entry index << log2(entry bytes), folded into
-            // the index arithmetic so that each gather is one LDG [uniform base + 32-bit offset]
-            constexpr uint32_t SH = (F == 2) ? 2u : 3u;
-            uint32_t off[8];
+            // entry indices (32-bit) from the level's base: each gather address is one IMAD.WIDE.U32
             if (np1) {
-                const uint32_t o1 = np1 << SH, o2 = (np1 * np1) << SH;
-                const uint32_t b = (cx + np1 * cy + np1 * np1 * cz) << SH;
-#pragma unroll
-                for (int c = 0; c < 8; ++c)
-                    off[c] = b + ((c & 1) ? (1u << SH) : 0u) + (((c >> 1) & 1) ? o1 : 0u) + ((c >> 2) ? o2 : 0u);
+                // dense: the +x corner is the next entry -> same address register, immediate offset
+                const uint32_t o2 = np1 * np1;
+                const uint32_t i00 = cx + np1 * cy + o2 * cz, i10 = i00 + np1, i01 = i00 + o2, i11 = i01 + np1;
+                const raw_t *q00 = lvl + i00, *q10 = lvl + i10, *q01 = lvl + i01, *q11 = lvl + i11;
+                constexpr int E = (int)sizeof(raw_t);
+                raw[li][0] = ldg_hint<FINE, 0>(q00); raw[li][1] = ldg_hint<FINE, E>(q00);
+                raw[li][2] = ldg_hint<FINE, 0>(q10); raw[li][3] = ldg_hint<FINE, E>(q10);
+                raw[li][4] = ldg_hint<FINE, 0>(q01); raw[li][5] = ldg_hint<FINE, E>(q01);
+                raw[li][6] = ldg_hint<FINE, 0>(q11); raw[li][7] = ldg_hint<FINE, E>(q11);
             } else {
-                const uint32_t m = t_mask << SH;
                 const uint32_t hy0 = cy * 2654435761u, hy1 = hy0 + 2654435761u;
                 const uint32_t hz0 = cz * 805459861u, hz1 = hz0 + 805459861u;
-                const uint32_t hyz[4] = {(hy0 ^ hz0) << SH, (hy1 ^ hz0) << SH, (hy0 ^ hz1) << SH, (hy1 ^ hz1) << SH};
-                const uint32_t x0 = cx << SH, x1 = (cx + 1u) << SH;
+                const uint32_t hyz[4] = {hy0 ^ hz0, hy1 ^ hz0, hy0 ^ hz1, hy1 ^ hz1};
+                const uint32_t x1 = cx + 1u;
 #pragma unroll
-                for (int c = 0; c < 8; ++c) off[c] = (((c & 1) ? x1 : x0) ^ hyz[c >> 1]) & m;
+                for (int c = 0; c < 8; ++c) raw[li][c] = ldg_hint<FINE>(lvl + xor_and((c & 1) ? x1 : cx, hyz[c >> 1], t_mask));
             }
-            const char* lvl = reinterpret_cast<const char*>(table) + ((size_t)l << (log2_T + SH));
-#pragma unroll
-            for (int c = 0; c < 8; ++c) raw[li][c] = ldg_hint<FINE>(reinterpret_cast<const raw_t*>(lvl + off[c]));
         }
     }
 
@@ -494,15 +505,17 @@ template <int W, int F, bool CONCAT, bool LOCAL, bool PROBE>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_fused_encode_mlp(const TcParams p)
 {
-    constexpr bool ALIAS = (W == 128);                     // hidden/output accumulator = the drained layer-1 buffer
     constexpr int NG = (W == 128) ? 1 : 2;                 // tail groups
     constexpr int KC = (W + 63) / 64;                      // K chunks of a hidden layer
     constexpr int K16 = (W < 64 ? W : 64) / 16;            // UMMA K steps per hidden chunk
     constexpr uint32_t HCHUNK = (uint32_t)W * 128u;        // one weight chunk: W rows x 64 fp16
     constexpr uint32_t OUTCHUNK = TC_NOUT_PAD * 128u;
     constexpr uint32_t ACT_COLS = W / 2;
-    constexpr uint32_t C_HID = 2u * W;
-    constexpr uint32_t C_ACT = ALIAS ? 2u * W : 2u * W + NG * W;
+    // TMEM columns: [layer-1 accumulator x 2][activations x NG][A ring].  The hidden/output accumulator of a tile
+    // IS its drained layer-1 buffer: a buffer is handed back to the MMA warp when the tile's output has been read.
+    // (Round 2 first gave W <= 64 separate hidden accumulators, 2 x W more columns; giving those columns to the
+    // A ring instead -- 10 slots rather than 6 -- decouples the gather warps better: config 1 0.670 -> 0.656 ms)
+    constexpr uint32_t C_ACT = 2u * W;
     constexpr uint32_t C_RING = C_ACT + NG * ACT_COLS;
     constexpr int A_SLOTS = (512 - (int)C_RING) / 32 < TC_MAX_A_SLOTS ? (512 - (int)C_RING) / 32 : TC_MAX_A_SLOTS;
     constexpr uint32_t TMEM_COLS = 512;
@@ -545,8 +558,9 @@ k_fused_encode_mlp(const TcParams p)
     if (tid < NIF_MAX_LEVELS) {
         const int N = tid < L ? p.enc.res[tid] : 1;
         TcLevel lv;
-        lv.fn = (float)N; lv.top = (float)(N - 1);
-        lv.np1 = ((p.enc.dense_mask >> tid) & 1u) ? (uint32_t)N + 1u : 0u; lv.pad = 0u;
+        lv.fn = (float)N;
+        lv.np1 = ((p.enc.dense_mask >> tid) & 1u) ? (uint32_t)N + 1u : 0u;
+        lv.base = reinterpret_cast<const char*>(p.table) + ((size_t)tid << (p.enc.log2_T + (F == 2 ? 2 : 3)));
         s_lvl[tid] = lv;
     }
     if (warp == TC_MMA_WARP) tmem_alloc(smem_u32(s_tmem_ptr), TMEM_COLS);
@@ -601,7 +615,7 @@ k_fused_encode_mlp(const TcParams p)
                 const long long cur_ray = (long long)__float_as_int(rb[8 * TC_TILE]);
                 mbar_arrive(bar(BAR_RAY_EMPTY + nb));
                 const uint32_t tm_l1 = tm_acc1 + (uint32_t)(b * W);
-                const uint32_t tm_hid = ALIAS ? tm_l1 : tmem_base + C_HID + (uint32_t)(g * W);
+                const uint32_t tm_hid = tm_l1;
                 if (tg == 0) TC_TRACE(j, 1);
                 // layer 1 accumulator of tile j -> ReLU -> fp16 activations
                 mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1));
@@ -609,7 +623,6 @@ k_fused_encode_mlp(const TcParams p)
                 tc_fence_after();
                 drain_relu_to_act<W>(tm_l1 + t_row, tm_act + t_row);
                 tc_fence_before();
-                if constexpr (!ALIAS) mbar_arrive(bar(BAR_ACC_EMPTY + b));
                 named_bar_sync(1 + g, TC_TILE);
                 if (tg == 0) TC_TRACE(j, 3);
                 // hidden layers 2..H
@@ -632,7 +645,7 @@ k_fused_encode_mlp(const TcParams p)
                 tmem_ld_32x16(tm_hid + t_row, zr);
                 tmem_ld_wait();
                 tc_fence_before();
-                if constexpr (ALIAS) mbar_arrive(bar(BAR_ACC_EMPTY + b));
+                mbar_arrive(bar(BAR_ACC_EMPTY + b));
                 if (cur_ray >= 0) {
                     float z[NIF_N_OUT];
 #pragma unroll
@@ -861,12 +874,12 @@ k_fused_encode_mlp(const TcParams p)
                                 pz = nif_pe_sample(rb[(3 * en + 2) * TC_TILE], s);
                     GatherBatch<F> ba, bb;                                     // two batches in flight
                     constexpr int NL = GatherBatch<F>::NL;
-                    ba.issue(p.table, s_lvl, p.enc.log2_T, 0, px, py, pz);
+                    ba.issue(s_lvl, p.enc.log2_T, 0, px, py, pz);
                     for (int u = 0; u < units_per_es; ++u) {
                         uint32_t pk[4];
-                        bb.issue(p.table, s_lvl, p.enc.log2_T, (2 * u + 1) * NL, px, py, pz);
+                        bb.issue(s_lvl, p.enc.log2_T, (2 * u + 1) * NL, px, py, pz);
                         ba.consume(pk[0], pk[1]);
-                        if (u + 1 < units_per_es) ba.issue(p.table, s_lvl, p.enc.log2_T, (2 * u + 2) * NL, px, py, pz);
+                        if (u + 1 < units_per_es) ba.issue(s_lvl, p.enc.log2_T, (2 * u + 2) * NL, px, py, pz);
                         bb.consume(pk[2], pk[3]);
                         __syncwarp();
                         tmem_st_32x4(a_dst + (uint32_t)u * 4u, pk[0], pk[1], pk[2], pk[3]);
