@@ -12,9 +12,10 @@
 //   * layer-1 weights stay resident in shared memory when they fit the budget (config 1-3: 104 KB),
 //     otherwise their K chunks stream through a ring (config 4: 416 KB); hidden/output weights are
 //     resident for W <= 64 and stream through a 2-slot ring for W = 128;
-//   * accumulators: layer 1 double-buffered (tile t+1 accumulates while tile t is in its tail); the
-//     hidden/output layers of a tile accumulate into its own drained layer-1 buffer, so that the rest
-//     of the 512 TMEM columns is the A ring (10 chunk slots for W <= 64, 6 for W = 128).
+//   * accumulators: a tile owns one TMEM accumulator buffer from its first layer-1 MMA to the read of its
+//     output (the hidden/output layers accumulate into the drained layer-1 buffer); three buffers for
+//     W <= 64 (layer 1 of tile t+1 runs while the two tail groups work on tiles t and t-1), two for
+//     W = 128; the rest of the 512 TMEM columns is the A ring (8 / 6 chunk slots).
 //
 // Warp roles (one CTA per SM, 32 warps; setmaxnreg moves registers from the other roles to the
 // gather warps, whose loop needs 80):
@@ -53,7 +54,7 @@ constexpr int TC_THREADS = 32 * (TC_GATHER_WARP0 + TC_GATHER_WARPS);      // 102
 constexpr int TC_RAY_BUFS = 3;               // ray_buf depth: prep runs up to two tiles ahead of the tails
 constexpr int TC_RAY_FIELDS = 9;             // xi yi zi xo yo zo t_in t_out ray
 constexpr int TC_MAX_A_SLOTS = 10;           // layer-1 A chunk slots in TMEM (32 columns each)
-constexpr int TC_A_GROUP = 1;                // chunks per full/empty barrier pair of the A ring
+constexpr int TC_MAX_ACC = 3;                // layer-1 accumulator buffers (W <= 64: 3, W = 128: 2)
 constexpr int TC_MAX_W1_SLOTS = 8;           // layer-1 weight chunk slots when W1 streams
 constexpr int TC_HSLOTS = 2;                 // hidden/output weight chunk ring (W = 128)
 constexpr int TC_NOUT_PAD = 16;              // output layer N (12 heads padded to the UMMA minimum)
@@ -151,20 +152,26 @@ __device__ __forceinline__ void umma_chunk_ts(uint32_t d_tmem, uint32_t a_tmem, 
 {
     static_assert(NK == 1 || NK == 2 || NK == 4, "K = 16, 32 or 64 per chunk");
     if constexpr (NK == 4) {
+        // the K = 16 slices advance the descriptor's 14-bit address field by 2 (32 bytes): a 32-bit add on the low
+        // word (a chunk never straddles the 256 KB field), the high word is shared
         asm volatile(
             "{\n\t"
             ".reg .pred p, pe, cq;\n\t"
-            ".reg .b32 a1, a2, a3;\n\t"
+            ".reg .b32 a1, a2, a3, lo, hi, l1, l2, l3;\n\t"
             ".reg .b64 b1, b2, b3;\n\t"
             "elect.sync _|pe, 0xffffffff;\n\t"
             "setp.ne.b32 p, %4, 0;\n\t"
             "setp.ne.and.b32 cq, %5, 0, pe;\n\t"
+            "mov.b64 {lo, hi}, %2;\n\t"
             "add.u32 a1, %1, 8;\n\t"
             "add.u32 a2, %1, 16;\n\t"
             "add.u32 a3, %1, 24;\n\t"
-            "add.u64 b1, %2, 2;\n\t"
-            "add.u64 b2, %2, 4;\n\t"
-            "add.u64 b3, %2, 6;\n\t"
+            "add.u32 l1, lo, 2;\n\t"
+            "add.u32 l2, lo, 4;\n\t"
+            "add.u32 l3, lo, 6;\n\t"
+            "mov.b64 b1, {l1, hi};\n\t"
+            "mov.b64 b2, {l2, hi};\n\t"
+            "mov.b64 b3, {l3, hi};\n\t"
             "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
             "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [a1], b1, %3, 1;\n\t"
             "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [a2], b2, %3, 1;\n\t"
@@ -343,7 +350,7 @@ __host__ __device__ inline TcSmemLayout tc_smem_layout(int W, int hidden_layers,
 
 enum { BAR_A_FULL = 0, BAR_A_EMPTY = BAR_A_FULL + TC_MAX_A_SLOTS, BAR_W1_FULL = BAR_A_EMPTY + TC_MAX_A_SLOTS,
        BAR_W1_EMPTY = BAR_W1_FULL + TC_MAX_W1_SLOTS, BAR_ACC_FULL = BAR_W1_EMPTY + TC_MAX_W1_SLOTS,
-       BAR_ACC_EMPTY = BAR_ACC_FULL + 2, BAR_RAY_FULL = BAR_ACC_EMPTY + 2, BAR_RAY_EMPTY = BAR_RAY_FULL + TC_RAY_BUFS,
+       BAR_ACC_EMPTY = BAR_ACC_FULL + TC_MAX_ACC, BAR_RAY_FULL = BAR_ACC_EMPTY + TC_MAX_ACC, BAR_RAY_EMPTY = BAR_RAY_FULL + TC_RAY_BUFS,
        BAR_HID = BAR_RAY_EMPTY + TC_RAY_BUFS, BAR_HFULL = BAR_HID + 2, BAR_HEMPTY = BAR_HFULL + TC_HSLOTS,
        BAR_WRES = BAR_HEMPTY + TC_HSLOTS, BAR_COUNT = BAR_WRES + 1 };
 
@@ -511,16 +518,18 @@ k_fused_encode_mlp(const TcParams p)
     constexpr uint32_t HCHUNK = (uint32_t)W * 128u;        // one weight chunk: W rows x 64 fp16
     constexpr uint32_t OUTCHUNK = TC_NOUT_PAD * 128u;
     constexpr uint32_t ACT_COLS = W / 2;
-    // TMEM columns: [layer-1 accumulator x 2][activations x NG][A ring].  The hidden/output accumulator of a tile
-    // IS its drained layer-1 buffer: a buffer is handed back to the MMA warp when the tile's output has been read.
-    // (Round 2 first gave W <= 64 separate hidden accumulators, 2 x W more columns; giving those columns to the
-    // A ring instead -- 10 slots rather than 6 -- decouples the gather warps better: config 1 0.670 -> 0.656 ms)
-    constexpr uint32_t C_ACT = 2u * W;
+    // TMEM columns: [accumulator x NACC][activations x NG][A ring].  A tile keeps ONE accumulator buffer from its first
+    // layer-1 MMA to the read of its output: the hidden/output layers accumulate into the drained layer-1 buffer.  W <= 64:
+    // three buffers, so that the layer-1 MMAs of tile t+1 never wait for the tails of tiles t and t-1 (one per tail
+    // group), and 8 ring slots; W = 128: two buffers (one tail group), 6 ring slots.  (Round 2 first gave W <= 64 two
+    // layer-1 buffers plus a hidden accumulator per tail group -- 6 ring slots; the deeper ring decouples the gather
+    // warps better: config 1 0.670 -> 0.656 ms.)
+    constexpr int NACC = (W == 128) ? 2 : 3;
+    constexpr uint32_t C_ACT = (uint32_t)NACC * W;
     constexpr uint32_t C_RING = C_ACT + NG * ACT_COLS;
     constexpr int A_SLOTS = (512 - (int)C_RING) / 32 < TC_MAX_A_SLOTS ? (512 - (int)C_RING) / 32 : TC_MAX_A_SLOTS;
     constexpr uint32_t TMEM_COLS = 512;
-    constexpr int A_GROUPS = A_SLOTS / TC_A_GROUP;                         // ring = A_GROUPS groups of TC_A_GROUP chunk slots
-    static_assert(A_GROUPS >= 2, "layer-1 A ring too short");
+    static_assert(A_SLOTS >= 2, "layer-1 A ring too short");
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -541,13 +550,11 @@ k_fused_encode_mlp(const TcParams p)
 
     // ---- one-time setup ------------------------------------------------------------------------
     if (tid == 0) {
-        for (int i = 0; i < TC_MAX_A_SLOTS; ++i) { mbar_init(bar(BAR_A_FULL + i), 4u * (uint32_t)epc * TC_A_GROUP); mbar_init(bar(BAR_A_EMPTY + i), 1); }
+        for (int i = 0; i < TC_MAX_A_SLOTS; ++i) { mbar_init(bar(BAR_A_FULL + i), 4u * (uint32_t)epc); mbar_init(bar(BAR_A_EMPTY + i), 1); }
         for (int i = 0; i < TC_MAX_W1_SLOTS; ++i) { mbar_init(bar(BAR_W1_FULL + i), 1); mbar_init(bar(BAR_W1_EMPTY + i), 1); }
         for (int i = 0; i < TC_HSLOTS; ++i) { mbar_init(bar(BAR_HFULL + i), 1); mbar_init(bar(BAR_HEMPTY + i), 1); }
-        for (int i = 0; i < 2; ++i) {
-            mbar_init(bar(BAR_ACC_FULL + i), 1); mbar_init(bar(BAR_ACC_EMPTY + i), TC_TILE);
-            mbar_init(bar(BAR_HID + i), 1);
-        }
+        for (int i = 0; i < TC_MAX_ACC; ++i) { mbar_init(bar(BAR_ACC_FULL + i), 1); mbar_init(bar(BAR_ACC_EMPTY + i), TC_TILE); }
+        for (int i = 0; i < 2; ++i) mbar_init(bar(BAR_HID + i), 1);
         for (int i = 0; i < TC_RAY_BUFS; ++i) {
             mbar_init(bar(BAR_RAY_FULL + i), TC_PREP_THREADS); mbar_init(bar(BAR_RAY_EMPTY + i), TC_GATHER_WARPS + TC_TILE);
         }
@@ -607,7 +614,7 @@ k_fused_encode_mlp(const TcParams p)
                 }
             };
             for (int j = g;; j += NG) {
-                const int nb = j % TC_RAY_BUFS, b = j & 1;
+                const int nb = j % TC_RAY_BUFS, b = j % NACC;
                 mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
                 if (s_tile[nb] < 0) break;
                 const float* rb = ray_buf + (size_t)nb * TC_RAY_FIELDS * TC_TILE + tg;
@@ -618,7 +625,7 @@ k_fused_encode_mlp(const TcParams p)
                 const uint32_t tm_hid = tm_l1;
                 if (tg == 0) TC_TRACE(j, 1);
                 // layer 1 accumulator of tile j -> ReLU -> fp16 activations
-                mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j >> 1) & 1));
+                mbar_wait_sleep(bar(BAR_ACC_FULL + b), (uint32_t)((j / NACC) & 1));
                 if (tg == 0) TC_TRACE(j, 2);
                 tc_fence_after();
                 drain_relu_to_act<W>(tm_l1 + t_row, tm_act + t_row);
@@ -662,49 +669,46 @@ k_fused_encode_mlp(const TcParams p)
             {
                 const uint32_t idesc = idesc_f16(TC_TILE, W);
                 if (p.w1_resident) mbar_wait_sleep(bar(BAR_WRES), 0);
-                // A chunks are handed over in GROUPS of TC_A_GROUP chunks (one full/empty barrier pair per
-                // group): a try_wait costs ~90 cycles even when the phase is complete, and this one thread's
-                // instruction stream is what bounds the tensor pipe on 64-wide layers
+                // one full/empty barrier pair per chunk slot (pairs per group of two chunks were measured: slower, 7.7)
                 const uint64_t w1_desc0 = smem_desc_sw128(s_w1);
-                uint32_t gs = 0, gph = 0, wq = 0;                         // group slot + phase; streamed-W1 chunk counter
-                for (int j = 0;; ++j) {
-                    const int nb = j % TC_RAY_BUFS, b = j & 1;
-                    mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
-                    if (s_tile[nb] < 0) break;
-                    mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j >> 1) & 1) ^ 1));
-                    if (lane == 0) TC_TRACE(j, 25);
-                    tc_fence_after();
-                    __syncwarp();
-                    const uint32_t d_tmem = tm_acc1 + (uint32_t)(b * W);
-                    for (int c0 = 0; c0 < n_chunks; c0 += TC_A_GROUP) {
-                        mbar_wait_sleep(bar(BAR_A_FULL + gs), gph);
-                        if (c0 == 0 && lane == 0) TC_TRACE(j, 26);
+                // the loop body is instantiated per residency: this warp's instruction stream is what bounds the tensor
+                // pipe on narrow layers, so nothing it can decide once is decided per chunk
+                auto layer1 = [&](auto resident_tag) {
+                    constexpr bool RES = decltype(resident_tag)::value;
+                    uint32_t gs = 0, gph = 0, ws = 0, wph = 0;            // A slot + phase; streamed-W1 slot + phase
+                    for (int j = 0;; ++j) {
+                        const int nb = j % TC_RAY_BUFS, b = j % NACC;
+                        mbar_wait_sleep(bar(BAR_RAY_FULL + nb), (uint32_t)((j / TC_RAY_BUFS) & 1));
+                        if (s_tile[nb] < 0) break;
+                        mbar_wait_sleep(bar(BAR_ACC_EMPTY + b), (uint32_t)(((j / NACC) & 1) ^ 1));
+                        if (lane == 0) TC_TRACE(j, 25);
                         tc_fence_after();
                         __syncwarp();
-#pragma unroll
-                        for (int ci = 0; ci < TC_A_GROUP; ++ci) {
-                            const int c = c0 + ci;
-                            if (c < n_chunks) {
-                                const bool last = (ci + 1 == TC_A_GROUP) || (c + 1 == n_chunks);
-                                uint64_t bdesc;
-                                if (p.w1_resident) bdesc = w1_desc0 + (uint64_t)((uint32_t)c * (HCHUNK >> 4));
-                                else {
-                                    const uint32_t ws = wq % W1_SLOTS;
-                                    mbar_wait_sleep(bar(BAR_W1_FULL + ws), (wq / W1_SLOTS) & 1u);
-                                    tc_fence_after();
-                                    __syncwarp();
-                                    bdesc = w1_desc0 + (uint64_t)(ws * (HCHUNK >> 4));
-                                }
-                                umma_chunk_ts<4>(d_tmem, tm_ring + (gs * TC_A_GROUP + (uint32_t)ci) * 32u, bdesc, idesc,
-                                                 (uint32_t)(c != 0), last ? bar(BAR_A_EMPTY + gs) : 0u);
-                                if (!p.w1_resident) { umma_commit_elect(bar(BAR_W1_EMPTY + (wq % W1_SLOTS))); ++wq; }
+                        const uint32_t d_tmem = tm_acc1 + (uint32_t)(b * W);
+                        uint64_t bdesc = w1_desc0;
+                        for (int c = 0; c < n_chunks; ++c) {
+                            const uint32_t a_tmem = tm_ring + gs * 32u, a_empty = bar(BAR_A_EMPTY + gs);    // before the wait
+                            mbar_wait_sleep(bar(BAR_A_FULL + gs), gph);
+                            if (c == 0 && lane == 0) TC_TRACE(j, 26);
+                            if constexpr (!RES) {
+                                mbar_wait_sleep(bar(BAR_W1_FULL + ws), wph);
+                                bdesc = w1_desc0 + (uint64_t)(ws * (HCHUNK >> 4));
                             }
+                            tc_fence_after();
+                            __syncwarp();
+                            umma_chunk_ts<4>(d_tmem, a_tmem, bdesc, idesc, (uint32_t)(c != 0), a_empty);
+                            if constexpr (RES) bdesc += (uint64_t)(HCHUNK >> 4);
+                            else {
+                                umma_commit_elect(bar(BAR_W1_EMPTY + ws));
+                                if (++ws == W1_SLOTS) { ws = 0; wph ^= 1u; }
+                            }
+                            if (++gs == (uint32_t)A_SLOTS) { gs = 0; gph ^= 1u; }
                         }
-                        if (++gs == (uint32_t)A_GROUPS) { gs = 0; gph ^= 1u; }
+                        umma_commit_elect(bar(BAR_ACC_FULL + b));
+                        if (lane == 0) TC_TRACE(j, 27);
                     }
-                    umma_commit_elect(bar(BAR_ACC_FULL + b));
-                    if (lane == 0) TC_TRACE(j, 27);
-                }
+                };
+                if (p.w1_resident) layer1(std::true_type{}); else layer1(std::false_type{});
             }
         } else if (warp == TC_LOAD_WARP) {
             // ======================= weights: global (L2) -> shared memory, cp.async.bulk ============
@@ -822,8 +826,7 @@ k_fused_encode_mlp(const TcParams p)
         const int g = gw & 3, qr = gw >> 2;                                // row group (= TMEM lane quarter), rank in the group
         const uint32_t row = (uint32_t)(g * 32 + lane);
         const uint32_t t_row = (uint32_t)(g * 32) << 16;
-        const int n_groups = (n_chunks + TC_A_GROUP - 1) / TC_A_GROUP;    // chunk groups per tile (the last may be short)
-        const int n_pairs = n_groups * TC_A_GROUP * epc;                   // (endpoint, sample) slots per tile, padding included
+        const int n_pairs = n_chunks * epc;                                // (endpoint, sample) slots per tile, padding included
         const int units_per_es = (L * F) / 8;                              // 16-byte units (4 TMEM columns) one sample fills
         for (int j = 0;; ++j) {
             const int nb = j % TC_RAY_BUFS;
@@ -835,22 +838,17 @@ k_fused_encode_mlp(const TcParams p)
             for (int e = first; e < n_pairs; e += TC_GPR) {
                 const int c = e / epc, esl = e - c * epc;
                 const int es = e;
-                const uint32_t gq = (uint32_t)j * (uint32_t)n_groups + (uint32_t)(c / TC_A_GROUP);   // group counter
-                const uint32_t gs = gq % (uint32_t)A_GROUPS;
-                const uint32_t slot = gs * TC_A_GROUP + (uint32_t)(c % TC_A_GROUP);
-                mbar_wait(bar(BAR_A_EMPTY + gs), ((gq / (uint32_t)A_GROUPS) & 1u) ^ 1u);
+                const uint32_t gq = (uint32_t)j * (uint32_t)n_chunks + (uint32_t)c;                  // chunk counter
+                const uint32_t slot = gq % (uint32_t)A_SLOTS;
+                mbar_wait(bar(BAR_A_EMPTY + slot), ((gq / (uint32_t)A_SLOTS) & 1u) ^ 1u);
                 __syncwarp();                                              // tcgen05.st is .sync.aligned
-                if (c >= n_chunks) {                                       // padding chunk of a short last group: arrival only
-                    if (lane == 0) mbar_arrive(bar(BAR_A_FULL + gs));
-                    continue;
-                }
                 tc_fence_after();
                 const uint32_t a_dst = tm_ring + slot * 32u + (uint32_t)(esl * units_per_es) * 4u + t_row;
                 if constexpr (PROBE) {
                     // MLP-only probe: synthetic features, no table access.  The constant is written on the first pass
                     // over the ring only (the MMAs do not modify A): afterwards an item is the slot hand-over alone, so
                     // that the probe measures the MLP pipeline and not the cost of faking its input
-                    if (gq < (uint32_t)A_GROUPS)
+                    if (gq < (uint32_t)A_SLOTS)
                         for (int u = 0; u < units_per_es; ++u)
                             tmem_st_32x4(a_dst + (uint32_t)u * 4u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u, 0x2c002c00u);
                 } else if (CONCAT && es >= 2 && es < p.n_es) {
@@ -890,7 +888,7 @@ k_fused_encode_mlp(const TcParams p)
                 tmem_st_wait();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(BAR_A_FULL + gs));
+                if (lane == 0) mbar_arrive(bar(BAR_A_FULL + slot));
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(BAR_RAY_EMPTY + nb));
