@@ -44,7 +44,8 @@ typedef enum {
     NIF_ERR_DEFORM_SINGULAR = -3,  /* bend folds over: some occupied corner has k*y >= 1 - 1e-3 (R7) */
     NIF_ERR_WORKSPACE = -4,        /* workspace too small or misaligned                        */
     NIF_ERR_CUDA = -5,             /* a CUDA runtime call failed                               */
-    NIF_ERR_INTERNAL = -6          /* an internal limit was exceeded (reported by nif_query_last_hit_count) */
+    NIF_ERR_INTERNAL = -6,         /* an internal limit was exceeded (reported by nif_query_last_hit_count) */
+    NIF_ERR_STATIC_LIMIT = -7      /* nif_query_static: batch larger than NIF_STATIC_MAX_RAYS   */
 } nif_status;
 
 enum { NIF_F32 = 0, NIF_F16 = 1 };            /* nif_net_desc.dtype */
@@ -301,6 +302,32 @@ int nif_query_host(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
 int nif_query_host_compact(const nif_bvh* bvh, const nif_net* net, nif_stage* stage,
                            const nif_ray_batch* rays_host, const nif_query_out* out_host,
                            int32_t* hit_ray_host, int64_t* n_hit, unsigned flags);
+
+/* -------- the query without any allocation ------------------------------------------------- */
+
+/* nif_query for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same steps (a1)-(a5), the same kernels, the same outputs and
+ * flags as nif_query -- but the scratch (hit counter, hit-ray bins, hit list) lives in a device array that is
+ * part of the library image instead of a caller workspace.
+ *   - Limit: rays->n <= NIF_STATIC_MAX_RAYS (2,097,152 = one 1920x1080 frame and a bit); a larger batch
+ *     returns NIF_ERR_STATIC_LIMIT and enqueues nothing.  Use nif_query with your own workspace beyond it.
+ *   - Cost: every GPU on which the library is loaded holds NIF_STATIC_SCRATCH_BYTES (24 MiB) of device memory
+ *     until the process exits, whether or not this entry point is ever called.
+ *   - The call makes no cudaMalloc / cudaFree and calls no allocating library routine: it enqueues one
+ *     cudaMemsetAsync and the kernels on `stream` and returns without synchronising.  The first call made with
+ *     a given device current looks the array's device address up (cudaGetSymbolAddress, once per device, with
+ *     that device current): make that first call outside a graph capture.
+ *   - Sharing: ALL calls on a device use the one array, which keeps the previous call's contents; the parts
+ *     that must start at zero (header, bin counters) are cleared on `stream` at the start of each call.  Calls
+ *     are safe back to back on one stream; calls whose GPU work can overlap (different streams without an
+ *     ordering between them, or concurrent host threads on different streams) RACE on the array and give
+ *     wrong results.  nif_query_last_hit_count is not available for it (no workspace pointer to hand in).
+ * All pointers as in nif_query: `rays`, `out` DEVICE arrays owned by the caller.  Errors: those of nif_query,
+ * plus NIF_ERR_STATIC_LIMIT. */
+#define NIF_STATIC_MAX_RAYS      2097152
+#define NIF_STATIC_SCRATCH_BYTES 25166336      /* 64 B header + 8 MiB bins + 8 B per ray, rounded as nif_query_workspace_bytes */
+int nif_query_static(const nif_bvh* bvh, const nif_net* net, const nif_ray_batch* rays,
+                     const nif_query_out* out, unsigned flags, void* stream);
 
 /* -------- diagnostics --------------------------------------------------------------------- */
 

@@ -99,6 +99,7 @@ def lib() -> C.CDLL:
         L.nif_query_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_query.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut),
                                 C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
+        L.nif_query_static.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_RayBatch), C.POINTER(_QueryOut), C.c_uint, C.c_void_p]
         L.nif_query_poses_workspace_bytes.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.nif_query_poses.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_void_p, C.POINTER(_RayBatch), C.c_void_p,
                                       C.POINTER(_QueryOut), C.c_void_p, C.c_size_t, C.c_uint, C.c_void_p]
@@ -304,6 +305,22 @@ def nif_query(bvh: Bvh, net: Net | None, origin: torch.Tensor, direction: torch.
     _check(lib().nif_query(bvh.handle, net.handle if net is not None else None, C.byref(rb), C.byref(q),
                            workspace.data_ptr(), workspace.numel(), flags, _stream_ptr(stream)), "nif_query")
     return workspace
+
+
+NIF_STATIC_MAX_RAYS = 2097152          # include/nif.h
+
+
+def nif_query_static(bvh: Bvh, net: Net | None, origin: torch.Tensor, direction: torch.Tensor, out: dict,
+                     flags: int = 0, stream=None) -> None:
+    """nif_query with the scratch in the library's own fixed device array: no allocation, at most
+    NIF_STATIC_MAX_RAYS rays, calls that overlap on the GPU race (include/nif.h)."""
+    n = origin.shape[0]
+    assert origin.is_cuda and direction.is_cuda and origin.dtype == torch.float32
+    assert origin.is_contiguous() and direction.is_contiguous() and direction.shape[0] == n
+    rb = _RayBatch(n, origin.data_ptr(), direction.data_ptr())
+    q = _out_struct(out)
+    _check(lib().nif_query_static(bvh.handle, net.handle if net is not None else None, C.byref(rb), C.byref(q),
+                                  flags, _stream_ptr(stream)), "nif_query_static")
 
 
 def nif_query_poses_workspace_bytes(n: int) -> int:

@@ -14,7 +14,7 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 INCLUDE = HERE.parent / "include"
 LIB = HERE / "libnif.so"
-SOURCES = ["nif_api.cu", "nif_build.cu", "nif_traverse.cu", "nif_mlp_ffma.cu", "nif_fused_tc.cu", "nif_probe.cu", "nif_walk.cu"]
+SOURCES = ["nif_api.cu", "nif_build.cu", "nif_traverse.cu", "nif_mlp_ffma.cu", "nif_fused_tc.cu", "nif_probe.cu", "nif_walk.cu", "nif_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

@@ -42,6 +42,7 @@ extern "C" const char* nif_error_string(int status)
         case NIF_ERR_WORKSPACE: return "workspace too small or misaligned";
         case NIF_ERR_CUDA: return "CUDA runtime error";
         case NIF_ERR_INTERNAL: return "internal limit exceeded (traversal stack overflow): results invalid";
+        case NIF_ERR_STATIC_LIMIT: return "batch exceeds NIF_STATIC_MAX_RAYS, the size nif_query_static's fixed scratch serves";
         default: return "unknown status";
     }
 }
