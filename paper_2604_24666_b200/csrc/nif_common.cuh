@@ -75,7 +75,8 @@ struct nif_net {
 struct NifQueryScratch {
     unsigned long long n_hit;          // cursor of the bin allocation = hit rays once k_bin_offsets has run
     unsigned int tile_counter;         // dynamic ray fetch counter of the traversal kernel
-    unsigned int pad[13];
+    unsigned int pad[13];              // [0] coherent decision, [1] votes, [2] finished blocks, [3] stack overflow status,
+                                       // [4] tile counter of the encode kernel, [5] image width (0: batch is not an image), [6] its detection
 };
 static_assert(sizeof(NifQueryScratch) == 64, "scratch header is 64 bytes");
 

@@ -230,3 +230,62 @@ def test_axis_parallel_rays_in_lattice_planes(oracle, H, P):
         P.assert_traversal(m)
         assert m["t_in_bit_mismatch"] == 0 and m["t_out_bit_mismatch"] == 0, m
     assert (vid >= 0).sum() > 1000
+
+
+def _query_with_workspace(nif, case, o, d, flags):
+    od, dd = torch.from_numpy(o).cuda(), torch.from_numpy(d).cuda()
+    out = nif.alloc_outputs(len(o))
+    for v in out.values():
+        v.fill_(float("nan") if v.dtype.is_floating_point else -7)
+    ws = nif.nif_query(case.bvh, None, od, dd, out, flags=nif.NIF_TRAVERSE_ONLY | flags)
+    torch.cuda.synchronize()
+    header = ws[:64].view(torch.int32).cpu().numpy()         # NifQueryScratch: n_hit (8 B), tile counter, pad[13]
+    return {k: out[k].cpu().numpy() for k in ("voxel_id", "t_in", "t_out")}, int(header[3 + 5])   # pad[5] = image width
+
+
+@pytest.mark.parametrize("width,height,expect", [
+    (256, 128, 256),        # an image: walked in 8 x 4 pixel tiles per warp
+    (1920, 1080, 1920),     # configs[1]'s frame
+    (40, 36, 40),           # the smallest shapes that tile: width 40, one row of tiles high ...
+    (64, 32, 64),
+    (64, 4, None),          # a 16:1 strip (pixel steps vary 40-fold along the row): whatever is decided, same result
+    (250, 120, 0),          # width not a multiple of 8: plain assignment
+    (256, 126, 0),          # height not a multiple of 4
+    (24, 64, 0),            # rows shorter than a warp
+])
+def test_image_shaped_batches_are_recognised_and_give_the_same_result(H, width, height, expect):
+    """k_ray_coherence recognises a row-major image and k_traverse_simple then assigns 8 x 4 pixel tiles to warps.
+    That is a re-assignment of rays to threads only: ids and t must be bit-equal to the persistent kernel's, which
+    never looks at the width, on every ray -- recognised or not."""
+    import paper_2604_24666_b200 as nif
+    case = H.make_case(1, n_rays=16, with_net=False)
+    info = case.bvh.info()
+    o, d = I.camera_rays(width, height, 0.5 * (np.asarray(info["lo"]) + np.asarray(info["hi"])))
+    auto, w_auto = _query_with_workspace(nif, case, o, d, 0)
+    ref, w_ref = _query_with_workspace(nif, case, o, d, nif.NIF_TRAVERSE_INCOHERENT)
+    assert expect is None or w_auto == expect, (w_auto, expect)
+    for k in ("voxel_id", "t_in", "t_out"):
+        assert np.array_equal(auto[k].view(np.int32), ref[k].view(np.int32)), k
+    assert (auto["voxel_id"] >= 0).sum() > (0 if expect is None else min(200, width * height // 50))
+
+
+def test_batches_that_are_not_images_are_left_alone(H):
+    import paper_2604_24666_b200 as nif
+    case = H.make_case(1, n_rays=16, with_net=False)
+    info = case.bvh.info()
+    o, d = I.camera_rays(256, 128, 0.5 * (np.asarray(info["lo"]) + np.asarray(info["hi"])))
+    rng = np.random.default_rng(3)
+    perm = rng.permutation(len(o))
+    shuffled, w = _query_with_workspace(nif, case, o[perm], d[perm], nif.NIF_TRAVERSE_COHERENT)    # forced onto the simple kernel
+    assert w == 0
+    plain, w2 = _query_with_workspace(nif, case, o, d, 0)
+    assert w2 == 256
+    for k in ("voxel_id", "t_in", "t_out"):
+        assert np.array_equal(shuffled[k].view(np.int32), plain[k][perm].view(np.int32)), k
+    # a transposed image (column-major pixel order): consecutive rays are a pixel apart as well, rows are 128 long
+    ot = o.reshape(128, 256, 3).transpose(1, 0, 2).reshape(-1, 3).copy(); dt = d.reshape(128, 256, 3).transpose(1, 0, 2).reshape(-1, 3).copy()
+    tr, w3 = _query_with_workspace(nif, case, ot, dt, 0)
+    assert w3 == 128
+    back = {k: tr[k].reshape(256, 128).T.reshape(-1) for k in tr}
+    for k in ("voxel_id", "t_in", "t_out"):
+        assert np.array_equal(back[k].view(np.int32), plain[k].view(np.int32)), k
