@@ -46,18 +46,26 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
 // (nif_build.cu) and the ray carries inverses clamped to +-FLT_MAX, so a ray parallel to a slab and exactly
 // on the voxel's boundary plane lies strictly inside the inflated slab and 0 * inv is 0, never NaN -- the
 // NaN handling of axis_interval (a third of the node step's instructions) is not needed.  Same operation
-// sequence otherwise, so monotone rounding keeps every enclosed voxel's interval inside the node's.
-__device__ __forceinline__ bool slab_node(float lx, float ly, float lz, float hx, float hy, float hz,
-                                          const Ray& r, float& bn)
+// sequence otherwise, so monotone rounding keeps every enclosed voxel's interval inside the node's:
+//   t0 = (lo - o) * inv, t1 = (hi - o) * inv per axis, tmin = max of the three min(t0, t1), tmax = min of the three max.
+// It is evaluated with the six planes already in the ray's order: n* = the plane of each axis the ray meets first (lo when
+// the inverse direction is positive, hi when it is negative), f* = the other one.  Rounding is monotone and the clamped
+// inverse is never 0 or NaN, so (near - o) * inv <= (far - o) * inv holds on the computed values too: the per-axis
+// fminf/fmaxf would always pick exactly these two numbers, and leaving them out changes no bit of tmin or tmax
+// (6 of the 9 min/max per child gone; the ALU pipe that executes them is the busiest unit of the traversal kernels).
+__device__ __forceinline__ bool slab_node_ordered(float nx, float ny, float nz, float fx, float fy, float fz,
+                                                  const Ray& r, float& bn)
 {
-    const float x0 = __fmul_rn(__fsub_rn(lx, r.ox), r.ix), x1 = __fmul_rn(__fsub_rn(hx, r.ox), r.ix);
-    const float y0 = __fmul_rn(__fsub_rn(ly, r.oy), r.iy), y1 = __fmul_rn(__fsub_rn(hy, r.oy), r.iy);
-    const float z0 = __fmul_rn(__fsub_rn(lz, r.oz), r.iz), z1 = __fmul_rn(__fsub_rn(hz, r.oz), r.iz);
-    const float tmin = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fminf(z0, z1));
-    const float tmax = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fmaxf(z0, z1));
+    const float x0 = __fmul_rn(__fsub_rn(nx, r.ox), r.ix), x1 = __fmul_rn(__fsub_rn(fx, r.ox), r.ix);
+    const float y0 = __fmul_rn(__fsub_rn(ny, r.oy), r.iy), y1 = __fmul_rn(__fsub_rn(fy, r.oy), r.iy);
+    const float z0 = __fmul_rn(__fsub_rn(nz, r.oz), r.iz), z1 = __fmul_rn(__fsub_rn(fz, r.oz), r.iz);
+    const float tmin = fmaxf(fmaxf(x0, y0), z0);
+    const float tmax = fminf(fminf(x1, y1), z1);
     bn = fmaxf(tmin, 0.0f);
     return (tmin <= tmax) && (tmax >= 0.0f);
 }
+// offset (in float4) of an axis' near-plane block inside a node: lo planes start at 0, hi planes at 6
+__device__ __forceinline__ int near_block(float inv) { return (int)(__float_as_uint(inv) >> 31) * 6; }
 
 // r.ix/iy/iz are the CLAMPED inverses (node tests); the exact ones (+-inf for a zero component), which the
 // root box and the voxel's own box need (R10), are recomputed where used
@@ -336,10 +344,13 @@ k_traverse_persistent(const TravParams p)
                     const uint2 e = stack[--sp];
                     const NifNode* nd = pv.nodes(p, pose) + e.x;
                     const float4* f4 = reinterpret_cast<const float4*>(nd);
+                    // lo[] / hi[] hold the NEAR / FAR planes of this ray (slab_node_ordered); the successor rounds keep
+                    // lo / hi proper for the exact test
+                    const int nb3[3] = {AFTER ? 0 : near_block(r.ix), AFTER ? 0 : near_block(r.iy), AFTER ? 0 : near_block(r.iz)};
 #pragma unroll
                     for (int a = 0; a < 3; ++a) {
-                        const float4 l0 = __ldg(f4 + 2 * a), l1 = __ldg(f4 + 2 * a + 1);
-                        const float4 h0 = __ldg(f4 + 6 + 2 * a), h1 = __ldg(f4 + 6 + 2 * a + 1);
+                        const float4 l0 = __ldg(f4 + nb3[a] + 2 * a), l1 = __ldg(f4 + nb3[a] + 2 * a + 1);
+                        const float4 h0 = __ldg(f4 + (6 - nb3[a]) + 2 * a), h1 = __ldg(f4 + (6 - nb3[a]) + 2 * a + 1);
                         lo[a][0] = l0.x; lo[a][1] = l0.y; lo[a][2] = l0.z; lo[a][3] = l0.w;
                         lo[a][4] = l1.x; lo[a][5] = l1.y; lo[a][6] = l1.z; lo[a][7] = l1.w;
                         hi[a][0] = h0.x; hi[a][1] = h0.y; hi[a][2] = h0.z; hi[a][3] = h0.w;
@@ -365,7 +376,7 @@ k_traverse_persistent(const TravParams p)
                         if constexpr (AFTER)
                             ok = slab(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn, cf);
                         else
-                            ok = slab_node(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn);
+                            ok = slab_node_ordered(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn);
                         ok = ok && ((meta.x >> c) & 1u) && !(cn > best_in) && !(AFTER && cf < after_t);
                         // cn >= 0: its bit pattern orders like an integer; the 3 low mantissa bits make
                         // room for the octant (t_near only gets smaller: pruning stays conservative).  ~
@@ -479,9 +490,10 @@ k_traverse_simple(const TravParams p)
         const float4* f4 = reinterpret_cast<const float4*>(nd);
         float lo[3][8], hi[3][8];
 #pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const float4 l0 = __ldg(f4 + 2 * a), l1 = __ldg(f4 + 2 * a + 1);
-            const float4 h0 = __ldg(f4 + 6 + 2 * a), h1 = __ldg(f4 + 6 + 2 * a + 1);
+        for (int a = 0; a < 3; ++a) {                             // lo = near planes, hi = far planes of this ray
+            const int nb = near_block(a == 0 ? r.ix : a == 1 ? r.iy : r.iz);
+            const float4 l0 = __ldg(f4 + nb + 2 * a), l1 = __ldg(f4 + nb + 2 * a + 1);
+            const float4 h0 = __ldg(f4 + (6 - nb) + 2 * a), h1 = __ldg(f4 + (6 - nb) + 2 * a + 1);
             lo[a][0] = l0.x; lo[a][1] = l0.y; lo[a][2] = l0.z; lo[a][3] = l0.w;
             lo[a][4] = l1.x; lo[a][5] = l1.y; lo[a][6] = l1.z; lo[a][7] = l1.w;
             hi[a][0] = h0.x; hi[a][1] = h0.y; hi[a][2] = h0.z; hi[a][3] = h0.w;
@@ -497,7 +509,7 @@ k_traverse_simple(const TravParams p)
         for (int c = 0; c < 8; ++c) {
             if (!((meta.x >> c) & 1u)) continue;
             float cn;
-            if (slab_node(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn) && !(cn > best_in)) {
+            if (slab_node_ordered(lo[0][c], lo[1][c], lo[2][c], hi[0][c], hi[1][c], hi[2][c], r, cn) && !(cn > best_in)) {
                 if (sp >= STACK_MAX) { *p.overflow_flag = 1u; continue; }   // see k_traverse_persistent
                 int q = sp++;
                 while (q > sp0 && __uint_as_float(stack[q - 1].y) < cn) { stack[q] = stack[q - 1]; --q; }
@@ -508,10 +520,6 @@ k_traverse_simple(const TravParams p)
     retire_ray(p, ray, best_id, best_in, best_out);
 }
 
-// Decides which traversal kernel runs (device-side: nif_query never synchronises).  Sampled groups
-// of 32 consecutive rays vote "coherent" when every direction is within ~8 degrees of the group's
-// first and all origins lie within a tenth of the object's size of each other; the batch is coherent
-// when most groups are.  NIF_TRAVERSE_COHERENT / NIF_TRAVERSE_INCOHERENT override the vote.
 // squared step from ray i to ray j: direction change plus origin change in units of the object's size
 __device__ __forceinline__ float ray_step2(const float* __restrict__ origin, const float* __restrict__ dir, float inv_extent,
                                            long long i, long long j)
@@ -525,6 +533,10 @@ __device__ __forceinline__ float ray_step2(const float* __restrict__ origin, con
     return s;
 }
 
+// Decides which traversal kernel runs (device-side: nif_query never synchronises).  Sampled groups
+// of 32 consecutive rays vote "coherent" when every direction is within ~8 degrees of the group's
+// first and all origins lie within a tenth of the object's size of each other; the batch is coherent
+// when most groups are.  NIF_TRAVERSE_COHERENT / NIF_TRAVERSE_INCOHERENT override the vote.
 __global__ void __launch_bounds__(256)
 k_ray_coherence(long long n, const float* __restrict__ origin, const float* __restrict__ dir, float extent,
                 int n_groups, unsigned flags, unsigned int* __restrict__ votes, unsigned int* __restrict__ flag_out,
