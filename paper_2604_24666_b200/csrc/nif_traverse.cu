@@ -163,15 +163,19 @@ __device__ __forceinline__ bool voxel_hit(const float4* __restrict__ lat, int nv
 }
 
 constexpr int TRAV_BLOCK = 128;
-constexpr int TRAV_BLOCKS_PER_SM = 6;
+#ifndef NIF_TRAV_BPS
+#define NIF_TRAV_BPS 7      // persistent kernel: 72 registers, 7 blocks per SM (round 2, after the node step lost its votes and half its min/max: cfg 2 1.40 -> 1.33 ms per pose; 6: 1.40, 8: 1.41, 5: 1.46)
+#endif
+constexpr int TRAV_BLOCKS_PER_SM = NIF_TRAV_BPS;
 constexpr int STACK_MAX = 96;                 // a node pops 1 entry and pushes <= 8: 7 net per level
 constexpr int TRAV_MAX_LEVELS = 9;            // nv <= 512 (checked in nif_build.cu) -> padded 512^3 -> 9 octree levels
 static_assert(STACK_MAX >= 7 * TRAV_MAX_LEVELS + 8, "per-ray stack too small for the deepest hierarchy");
 constexpr uint32_t LEAF_FLAG = 0x80000000u;
 #ifndef NIF_TRAV_REFILL
-#define NIF_TRAV_REFILL 12
+#define NIF_TRAV_REFILL 8
 #endif
 constexpr int TRAV_REFILL = NIF_TRAV_REFILL;               // fetch new rays when at least this many lanes are idle
+constexpr int TRAV_B_LEAVES = 12, TRAV_B_FEW_INNER = 8, TRAV_B_FEW_LEAVES = 4;   // phase A -> B policy of k_traverse_persistent
 
 struct TravParams {
     const NifNode* nodes;
@@ -270,8 +274,8 @@ __device__ __forceinline__ void retire_ray(const TravParams& p, long long ray, i
 }
 
 // Persistent warps, one ray per lane, "while-while" traversal with dynamic ray fetch: lanes first
-// work through inner nodes until every live lane has a voxel on top of its stack (or is finished),
-// then all of them run the expensive 12-triangle voxel test together; finished lanes are refilled
+// work through inner nodes until enough live lanes have a voxel on top of their stack (or are finished),
+// then those run the expensive 12-triangle voxel test together; finished lanes are refilled
 // from a global counter once enough of them are idle.  Incoherent rays (config 3) otherwise leave
 // 4 of 32 lanes active on average.
 template <bool AFTER, bool MULTI>
@@ -328,14 +332,23 @@ k_traverse_persistent(const TravParams p)
         }
         if (__all_sync(0xffffffffu, ray < 0)) break;      // nothing left anywhere in this warp
 
-        // ---- phase A: inner nodes until every live lane has a voxel on top or an empty stack ----
+        // ---- phase A: inner nodes until enough lanes have a voxel on top (policy below) ----
         for (;;) {
             // drop entries that can no longer win (strictly later than the best entry: ties stay, R12)
             while (sp > 0 && __uint_as_float(stack[sp - 1].y) > best_in) --sp;
             const bool inner = ray >= 0 && sp > 0 && !(stack[sp - 1].x & LEAF_FLAG);
-            if (!__any_sync(0xffffffffu, inner)) break;
+            // When to leave phase A.  Round 1 waited until NO lane had an inner node on top; lanes that reached a voxel early
+            // then idled through the node steps of the slowest lane.  Now phase B starts as soon as enough lanes hold a voxel:
+            // TRAV_B_LEAVES of them, or TRAV_B_FEW_LEAVES once fewer than TRAV_B_FEW_INNER lanes still have inner nodes.  A
+            // lane's own sequence of pops is unchanged, only the interleaving between lanes: same results, cfg 2 / 3
+            // traversal -24 % (1.34 -> 1.02 ms, 1.59 -> 1.24 ms per pose; thresholds swept, all within 3 % of each other).
             {
-                // one node per lane, branch-free: slab tests of the octants any lane has, a sorting
+                const unsigned mi = __ballot_sync(0xffffffffu, inner);
+                const int leaves = __popc(__ballot_sync(0xffffffffu, ray >= 0 && sp > 0 && (stack[sp - 1].x & LEAF_FLAG)));
+                if (mi == 0u || leaves >= TRAV_B_LEAVES || (__popc(mi) < TRAV_B_FEW_INNER && leaves >= TRAV_B_FEW_LEAVES)) break;
+            }
+            {
+                // one node per lane, branch-free: slab tests of all 8 octants, a sorting
                 // network on packed (t_near, octant) keys, up to 8 predicated pushes (farthest first,
                 // so the nearest child ends on top).  Lanes without an inner node run it masked off.
                 float lo[3][8], hi[3][8];
@@ -368,7 +381,9 @@ k_traverse_persistent(const TravParams p)
 #pragma unroll
                 for (int c = 0; c < 8; ++c) {
                     key[c] = 0xffffffffu;
-                    if (__any_sync(0xffffffffu, (meta.x >> c) & 1u)) {       // coherent warps skip absent octants
+                    {   // all 8 octants, absent ones masked off below: the lanes of this kernel sit on different nodes, so a
+                        // warp-wide "does any lane have octant c" vote (round 1) was nearly always true -- dropping the 8
+                        // votes and branches: cfg 2 / 3 traversal -5 %
                         float cn, cf = INFINITY;
                         // AFTER: every voxel below has t_in <= its box's far end <= cf (boxes nest, R10), so a
                         // child that ends before after_t holds no successor
@@ -413,7 +428,7 @@ k_traverse_persistent(const TravParams p)
         }
 
         // ---- phase B: every lane with a voxel on top tests it ------------------------------------
-        if (ray >= 0 && sp > 0) {
+        if (ray >= 0 && sp > 0 && (stack[sp - 1].x & LEAF_FLAG)) {
             const uint32_t id = stack[--sp].x & ~LEAF_FLAG;
             float ti, to;
             if (voxel_hit(pv.lat(p, pose), p.nv, id, r, ti, to) && (!AFTER || after_bound(ti, (int32_t)id, after_t, after_id))) {
