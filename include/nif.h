@@ -68,7 +68,9 @@ enum {
     /* The traversal has two kernels: one thread per ray with static assignment (best for coherent
      * batches such as camera rays) and persistent warps with dynamic ray fetch (best for incoherent
      * batches).  By default a device-side vote over sampled ray groups picks one; these force it.
-     * Results are identical either way. */
+     * Results are identical either way.  A batch that is a row-major image (n = width x height, width a multiple of
+     * 8, height of 4, consecutive rays one pixel apart) is recognised on the device as well, and the static kernel then
+     * gives each warp a tile of 8 x 4 pixels instead of 32 pixels of a row: faster, same results; nothing to set. */
     NIF_TRAVERSE_COHERENT   = 8u,
     NIF_TRAVERSE_INCOHERENT = 16u,
     /* Diagnostic: the tensor-core kernel fills its A operand with a constant instead of gathering from
