@@ -72,6 +72,20 @@ def test_argument_validation_without_touching_the_device(lib):
     assert lib.nif_stage_create(0, C.byref(h)) == -1
 
 
+def test_static_query_checks_its_limit_before_any_device_work(lib):
+    # nif_query_static: argument errors and the size limit are decided on the host, before the first CUDA call
+    from paper_2604_24666_b200 import binding as B
+    assert lib.nif_query_static(None, None, None, None, 0, None) == -1
+    fake = C.c_void_p(256)                                   # handles are only null-checked before the limit check
+    q = B._QueryOut()
+    for name, _ in B._QueryOut._fields_:
+        setattr(q, name, 256)
+    for n, expect in ((B.NIF_STATIC_MAX_RAYS + 1, -7), (-1, -1), (0, 0)):
+        rb = B._RayBatch(n, 256, 256)
+        assert lib.nif_query_static(fake, fake, C.byref(rb), C.byref(q), 0, None) == expect, n
+    assert b"NIF_STATIC_MAX_RAYS" in lib.nif_error_string(-7)
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
 def test_no_gpu_means_unsupported_not_a_fallback(lib):
     import numpy as np
